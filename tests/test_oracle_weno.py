@@ -1,0 +1,294 @@
+"""Pins for the WENO characteristic branch (pins i-v)."""
+import os
+
+import numpy as np
+import pytest
+import sympy as sp
+
+import workloads as W
+from oracle import oracle as O
+from tests.helpers import random_periodic_case
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+GAMMA = 1.4
+
+
+# ------------------------------------------------------------------ eigenvectors
+def _flux(wc, d, gamma=GAMMA):
+    rho, m, E = wc[0], wc[1:4], wc[4]
+    vel = m / rho
+    p = (gamma - 1) * (E - 0.5 * rho * np.sum(vel * vel))
+    f = np.array([m[d], m[0] * vel[d], m[1] * vel[d], m[2] * vel[d], (E + p) * vel[d]], dtype=wc.dtype)
+    f[1 + d] += p
+    return f
+
+
+def _jacobian(wc, d):
+    """dF_d/dw by complex-step differentiation of the plain flux definition."""
+    A = np.zeros((5, 5))
+    for j in range(5):
+        z = wc.astype(complex)
+        z[j] += 1e-30j
+        A[:, j] = np.imag(_flux(z, d)) / 1e-30
+    return A
+
+
+def _state_from(vel, H, rho=1.0):
+    q2 = np.dot(vel, vel)
+    E = (H + (GAMMA - 1) * 0.5 * q2) / GAMMA      # H = gamma E - (gamma-1) q^2/2 per unit mass
+    return np.array([rho, rho * vel[0], rho * vel[1], rho * vel[2], rho * E])
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_eigenvectors_are_inverse_and_diagonalise_the_jacobian(d):
+    rng = np.random.default_rng(d)
+    for _ in range(5):
+        vel = rng.uniform(-1.5, 1.5, 3)
+        H = 0.5 * np.dot(vel, vel) + rng.uniform(1.5, 4.0)
+        Lm, Rm = O.eigenvectors(d, vel, H, GAMMA)
+        assert np.max(np.abs(Lm @ Rm - np.eye(5))) < 1e-14
+        c = np.sqrt((GAMMA - 1) * (H - 0.5 * np.dot(vel, vel)))
+        lam = np.diag([vel[d] - c, vel[d], vel[d], vel[d], vel[d] + c])
+        A = _jacobian(_state_from(vel, H), d)
+        assert np.max(np.abs(Rm @ lam @ Lm - A)) < 1e-12 * np.max(np.abs(A))
+
+
+# ------------------------------------------------------------------ reconstruction
+def _derive_weno(r):
+    """Jiang-Shu construction in exact rationals: candidate values q_k at x=+1/2, smoothness
+    indicators beta_k = sum_m int_{-1/2}^{1/2} (d^m p_k/dx^m)^2 dx, and linear weights d_k."""
+    x = sp.symbols("x")
+    v = sp.symbols(f"v0:{2 * r - 1}")           # v[j] is cell j - (r-1)
+    def fit(cells):
+        co = sp.symbols(f"c0:{len(cells)}")
+        poly = sum(co[n] * x ** n for n in range(len(cells)))
+        eqs = [sp.integrate(poly, (x, j - sp.Rational(1, 2), j + sp.Rational(1, 2))) - v[j + r - 1] for j in cells]
+        sol = sp.solve(eqs, co)
+        return sp.expand(poly.subs(sol))
+    qs, betas = [], []
+    for k in range(r):
+        cells = list(range(-(r - 1) + k, k + 1))
+        pk = fit(cells)
+        qs.append(sp.expand(pk.subs(x, sp.Rational(1, 2))))
+        betas.append(sp.expand(sum(sp.integrate(sp.diff(pk, x, m) ** 2, (x, -sp.Rational(1, 2), sp.Rational(1, 2)))
+                                   for m in range(1, r))))
+    full = sp.expand(fit(list(range(-(r - 1), r))).subs(x, sp.Rational(1, 2)))
+    dk = sp.symbols(f"d0:{r}")
+    eqs = sp.Poly(sp.expand(sum(dk[k] * qs[k] for k in range(r)) - full), *v).coeffs()
+    dsol = sp.solve(eqs, dk)
+    return v, qs, betas, [dsol[s] for s in dk], full
+
+
+@pytest.mark.parametrize("r", [2, 3, 4])
+def test_weno_matches_exact_rational_derivation(r):
+    v, qs, betas, dks, full = _derive_weno(r)
+    rng = np.random.default_rng(r)
+    for _ in range(4):
+        vals = rng.uniform(-1, 1, 2 * r - 1)
+        sub = dict(zip(v, [sp.Float(float(t), 30) for t in vals]))
+        beta_ref = np.array([float(b.subs(sub)) for b in betas])
+        _, beta = O.weno_reconstruct(vals, r)
+        assert np.allclose(beta, beta_ref, rtol=1e-12, atol=1e-14)
+        # linear weights reproduce the full (2r-1)-order reconstruction
+        val_lin, _ = O.weno_reconstruct(vals, r, linear=True)
+        assert abs(val_lin - float(full.subs(sub))) < 1e-13
+        # nonlinear: omega_k = alpha_k / sum alpha, alpha_k = d_k / (eps + beta_k)^2
+        eps = 1e-6
+        al = np.array([float(dks[k]) for k in range(r)]) / (eps + beta_ref) ** 2
+        q_ref = np.array([float(q.subs(sub)) for q in qs])
+        val, _ = O.weno_reconstruct(vals, r, eps=eps)
+        assert abs(val - np.sum(al / al.sum() * q_ref)) < 1e-12
+
+
+def test_weno5_linear_stencil_is_the_printed_one():
+    """linear weights give (2,-13,47,27,-3)/60."""
+    c = [O.weno_reconstruct(np.eye(5)[m], 3, linear=True)[0] for m in range(5)]
+    assert np.allclose(c, np.array([2, -13, 47, 27, -3]) / 60.0, atol=1e-16)
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4])
+def test_polynomials_up_to_degree_r_minus_1_are_reconstructed_exactly(r):
+    """O3 pin (iii): any weights reproduce degree <= r-1 data (point values = cell averages of h)."""
+    x = sp.symbols("x")
+    rng = np.random.default_rng(10 + r)
+    for deg in range(r):
+        co = rng.uniform(-1, 1, deg + 1)
+        h = sum(sp.Float(float(co[n])) * x ** n for n in range(deg + 1))
+        cells = np.arange(-(r - 1), r)
+        vals = [float(sp.integrate(h, (x, int(j) - sp.Rational(1, 2), int(j) + sp.Rational(1, 2)))) for j in cells]
+        val, _ = O.weno_reconstruct(np.array(vals), r, eps=1e-6)
+        assert abs(val - float(h.subs(x, sp.Rational(1, 2)))) < 1e-12
+
+
+def test_weno_picks_the_smooth_side_of_a_jump():
+    val, beta = O.weno_reconstruct(np.array([1.0, 1.0, 1.0, 0.0, 0.0]), 3)
+    assert abs(val - 1.0) < 1e-6 and beta[0] == 0.0 and beta[1] > 0 and beta[2] > 0
+
+
+# ------------------------------------------------------------------ linear-weight flux, brute force
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_linear_weight_flux_brute_force(d):
+    """O3 pin (ii): with omega_k = d_k the WENO flux is
+    1/2 (Lin+ + Lin-)(F) + 1/2 R |Lambda|_LF L (Lin+ - Lin-)(w), independent of the eigenbasis of
+    the repeated eigenvalue.  R |Lambda| L is formed here from the
+    complex-step Jacobian at the Roe state through its spectral projectors, not from the
+    oracle's eigenvectors."""
+    case, (rho, u, v, w, p) = random_periodic_case(9, 8, 10, seed=20 + d, flux_mode=W.FLUX_WENO, amp=0.1)
+    o = O.Oracle(case, kind="serial", dbg_flags=O.DBG_WENO_LINEAR)
+    R = o.rhs(parts=1 << d)
+    axis = 2 - d
+    n = rho.shape[axis]
+    h = (case.lx / case.nx, case.ly / case.ny, case.lz / case.nz)[d]
+    wc = case.w0
+    cs = np.sqrt(GAMMA * p / rho)
+    ud = (u, v, w)[d]
+    H = (wc[4] + p) / rho
+    cplus = np.array([2, -13, 47, 27, -3]) / 60.0          # nodes i-2 .. i+2
+    mv = lambda a: np.moveaxis(a, axis, -1)
+    wcm = np.stack([mv(wc[q]) for q in range(5)], axis=-1)  # [..., n, 5]
+    shape = wcm.shape[:-2]
+    flux = np.zeros(shape + (n, 5))
+    um, vm, wm, Hm, rm, cm, udm = map(mv, (u, v, w, H, rho, cs, ud))
+    for idx in np.ndindex(*shape):
+        W1 = wcm[idx]                                        # [n, 5]
+        F1 = np.array([_flux(W1[i], d) for i in range(n)])
+        for i in range(n):
+            il, ir = i, (i + 1) % n
+            rw = np.sqrt(rm[idx][ir] / rm[idx][il])
+            roe = lambda a: (a[idx][il] + rw * a[idx][ir]) / (1 + rw)
+            vel = np.array([roe(um), roe(vm), roe(wm)])
+            Hb = roe(Hm)
+            A = _jacobian(_state_from(vel, Hb), d)
+            st = [(i + m) % n for m in range(-2, 4)]          # 2r stencil nodes
+            l_minus = np.max(np.abs(udm[idx][st] - cm[idx][st]))
+            l_zero = np.max(np.abs(udm[idx][st]))
+            l_plus = np.max(np.abs(udm[idx][st] + cm[idx][st]))
+            # spectral projectors of the diagonalisable Jacobian (eigenvalues un-c, un, un+c) by
+            # Lagrange interpolation in A: no eigenvector formula is used
+            cb = np.sqrt((GAMMA - 1) * (Hb - 0.5 * np.dot(vel, vel)))
+            e = [vel[d] - cb, vel[d], vel[d] + cb]
+            I5 = np.eye(5)
+            P = [(A - e[b] * I5) @ (A - e[c_] * I5) / ((e[a] - e[b]) * (e[a] - e[c_]))
+                 for a, b, c_ in ((0, 1, 2), (1, 0, 2), (2, 0, 1))]
+            M = l_minus * P[0] + l_zero * P[1] + l_plus * P[2]
+            sp_nodes = [(i + m) % n for m in range(-2, 3)]    # left-biased
+            sm_nodes = [(i + 3 - m) % n for m in range(5)]    # mirror: i+3 .. i-1
+            Fp = cplus @ F1[sp_nodes]
+            Fm = cplus @ F1[sm_nodes]
+            Wp = cplus @ W1[sp_nodes]
+            Wm = cplus @ W1[sm_nodes]
+            flux[idx + (i,)] = 0.5 * (Fp + Fm) + 0.5 * M @ (Wp - Wm)
+    ref = -(flux - np.roll(flux, 1, axis=-2)) / h             # [..., n, 5]
+    for q in range(5):
+        got = mv(R[q])
+        err = np.max(np.abs(got - ref[..., q])) / np.max(np.abs(ref[..., q]))
+        assert err < 1e-11, (q, err)
+
+
+# ------------------------------------------------------------------ permutation symmetry
+@pytest.mark.parametrize("mode,visc", [(W.FLUX_WENO, W.VISC_NONE), (W.FLUX_HYBRID, W.VISC_SUTHERLAND),
+                                       (W.FLUX_CENTRAL, W.VISC_SUTHERLAND)])
+def test_cyclic_permutation_of_axes_permutes_the_rhs(mode, visc):
+    """O3 pin (iv): rotating the data x->y->z rotates the result (uniform grid)."""
+    kw = dict(flux_mode=mode, visc_law=visc, mu_ref=0.02, sensor_threshold=0.1, u_ref=1.0, l_ref=10.0)
+    case, (rho, u, v, w, p) = random_periodic_case(9, 10, 11, seed=31, lx=0.9, ly=1.0, lz=1.1, **kw)
+    R = O.Oracle(case).rhs()
+    # new axes: x' = y, y' = z, z' = x  =>  arrays [z', y', x'] = old [x, z, y]
+    tr = lambda a: np.ascontiguousarray(np.transpose(a, (2, 0, 1)))
+    case2 = case.replace(nx=case.ny, ny=case.nz, nz=case.nx, lx=case.ly, ly=case.lz, lz=case.lx,
+                         w0=W.conserved_from_primitive(tr(rho), tr(v), tr(w), tr(u), tr(p), case.gamma))
+    R2 = O.Oracle(case2).rhs()
+    expect = [tr(R[0]), tr(R[2]), tr(R[3]), tr(R[1]), tr(R[4])]
+    for q in range(5):
+        assert np.max(np.abs(R2[q] - expect[q])) < 1e-11 * np.max(np.abs(expect[q]))
+
+
+# ------------------------------------------------------------------ Sod shock tube
+def _sod_exact(xi):
+    """Exact Sod solution at similarity coordinate xi = (x - x0)/t (Toro, ch. 4): star state by
+    Newton iteration on the pressure function, then sampling."""
+    g = GAMMA
+    rl, pl, rr, pr = 1.0, 1.0, 0.125, 0.1
+    cl, cr = np.sqrt(g * pl / rl), np.sqrt(g * pr / rr)
+    def fK(pz, rk, pk, ck):
+        if pz > pk:
+            A, B = 2 / ((g + 1) * rk), (g - 1) / (g + 1) * pk
+            return (pz - pk) * np.sqrt(A / (pz + B))
+        return 2 * ck / (g - 1) * ((pz / pk) ** ((g - 1) / (2 * g)) - 1)
+    ps = 0.3
+    for _ in range(60):
+        f = fK(ps, rl, pl, cl) + fK(ps, rr, pr, cr)
+        df = (fK(ps + 1e-7, rl, pl, cl) + fK(ps + 1e-7, rr, pr, cr) - f) / 1e-7
+        ps -= f / df
+    us = 0.5 * (fK(ps, rr, pr, cr) - fK(ps, rl, pl, cl))
+    rsl = rl * (ps / pl) ** (1 / g)
+    rsr = rr * ((ps / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * ps / pr + 1))
+    csl = cl * (ps / pl) ** ((g - 1) / (2 * g))
+    S = cr * np.sqrt((g + 1) / (2 * g) * ps / pr + (g - 1) / (2 * g))     # right shock speed (u_R = 0)
+    rho = np.empty_like(xi)
+    for n, s in enumerate(xi):
+        if s < -cl:
+            rho[n] = rl
+        elif s < us - csl:
+            cfan = 2 / (g + 1) * (cl - (g - 1) / 2 * s)
+            rho[n] = rl * (cfan / cl) ** (2 / (g - 1))
+        elif s < us:
+            rho[n] = rsl
+        elif s < S:
+            rho[n] = rsr
+        else:
+            rho[n] = rr
+    return rho, dict(p_star=ps, u_star=us, rho_star_L=rsl, rho_star_R=rsr)
+
+
+def test_sod_star_state_matches_golden_table():
+    gold = dict((t.split()[0], float(t.split()[1])) for t in open(os.path.join(GOLD, "sod_exact.txt"))
+                if not t.startswith("#"))
+    _, star = _sod_exact(np.array([0.0]))
+    for k, val in gold.items():
+        assert abs(star[k] - val) < 6e-6, (k, star[k], val)
+
+
+def _run_sod(nx, direction=0):
+    g = GAMMA
+    x = (np.arange(nx) + 0.0) * (2.0 / nx)
+    left = (x >= 0.5) & (x < 1.5)
+    rho1 = np.where(left, 1.0, 0.125)
+    p1 = np.where(left, 1.0, 0.1)
+    shp = [3, 3, 3]
+    shp[2 - direction] = nx
+    bshape = [1, 1, 1]
+    bshape[2 - direction] = nx
+    rho = np.broadcast_to(rho1.reshape(bshape), shp).copy()
+    p = np.broadcast_to(p1.reshape(bshape), shp).copy()
+    z = np.zeros(shp)
+    dx = 2.0 / nx
+    nsteps = int(np.ceil(0.2 / (0.4 * dx / 2.2)))
+    L = [0.1, 0.1, 0.1]
+    L[direction] = 2.0
+    case = W.Case(name="sod", nx=shp[2], ny=shp[1], nz=shp[0], lx=L[0], ly=L[1], lz=L[2], flux_mode=W.FLUX_WENO,
+                  dt_fixed=0.2 / nsteps, w0=W.conserved_from_primitive(rho, z, z, z, p, g))
+    o = O.Oracle(case)
+    o.step(nsteps)
+    w = o.get_fields()
+    line = np.moveaxis(w[0], 2 - direction, -1)[0, 0]
+    sel = x >= 1.0
+    exact, _ = _sod_exact((x[sel] - (1.5 - 0.5 * dx)) / 0.2)   # jump sits midway between two nodes
+    return float(np.mean(np.abs(line[sel] - exact))), line, w
+
+
+def test_sod_shock_tube_converges_to_exact_solution():
+    """O3 pin (v): L1 error O(dx), no new extrema beyond ~1 %, transverse momentum stays zero."""
+    e1, line1, _ = _run_sod(100)
+    e2, line2, w2 = _run_sod(200)
+    assert e2 < 0.012 and e1 / e2 > 1.5, (e1, e2)
+    assert line2.min() > 0.125 * 0.99 and line2.max() < 1.01
+    assert np.all(w2[2] == 0.0) and np.all(w2[3] == 0.0)
+    # the mirrored Riemann problem at x = 0.5 is the reflection of the one at x = 1.5
+    assert np.allclose(line2[0:100], line2[199:99:-1], atol=1e-10)
+
+
+def test_sod_in_z_matches_sod_in_x():
+    e_x, line_x, _ = _run_sod(100, 0)
+    e_z, line_z, _ = _run_sod(100, 2)
+    assert np.allclose(line_x, line_z, atol=1e-12)
