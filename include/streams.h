@@ -1,0 +1,130 @@
+/* =============================================================================
+ * streams.h -- C ABI of the B200-native STREAmS-2 hot path.
+ *
+ * One library, libstreams.so (sm_100a), exposing the per-time-step right-hand side
+ * of the 3-D compressible Navier-Stokes equations on a structured Cartesian grid
+ * and the low-storage RK3 update that applies it, as the paper describes the
+ * method (arXiv 2304.05494; section 2):
+ *   - central energy-preserving split convective flux of order 2L
+ *   - WENO characteristic reconstruction where a Ducros-type sensor fires
+ *   - viscous terms in Laplacian form, central differences, stretched y
+ *   - third-order low-storage Runge-Kutta
+ *   - time-step max-reduction
+ *   - conserved array w(x,y,z,v) with ghost layers, x unit-stride
+ * The paper prints no formulas; the exact reading of each operation is listed in
+ * DESIGN.md ("Readings", tags O1..O6 / S1..S16 of SURVEY.md section 8(c)).
+ *
+ * Conventions
+ *   - fp64 everywhere.  Interior arrays are C order [v][k][j][i]
+ *     = [5][nz][ny][nx] (conserved rho, rho u, rho v, rho w, rho E) or [nz][ny][nx].
+ *   - Every pointer argument says whether it is HOST or DEVICE memory.
+ *   - The caller owns the workspace and the CUDA stream and keeps both alive until
+ *     streams_destroy.  The library never allocates device memory itself.
+ *   - Host arrays passed in (y_nodes, the structs) are copied before the call returns.
+ *   - Calls enqueue work on the caller's stream.  Calls that return host scalars or
+ *     copy to host memory synchronise that stream before returning.
+ *   - Errors: negative return code, text via streams_last_error(); nothing aborts or
+ *     throws across this boundary.  There is no CPU fallback: without a CUDA device
+ *     every compute entry point fails with STREAMS_ECUDA.
+ * ============================================================================= */
+#ifndef STREAMS_H
+#define STREAMS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct streams_ctx streams_ctx; /* opaque, owned by the library */
+
+enum { STREAMS_OK = 0, STREAMS_EINVAL = -1, STREAMS_ENOMEM = -2, STREAMS_ECUDA = -3,
+       STREAMS_ESTATE = -4, STREAMS_ENAN = -5 };
+enum { STREAMS_BC_PERIODIC = 0, STREAMS_BC_WALL_ISOTHERMAL = 1, STREAMS_BC_FREESTREAM = 2 };
+enum { STREAMS_VISC_NONE = 0, STREAMS_VISC_POWER = 1, STREAMS_VISC_SUTHERLAND = 2 };
+enum { STREAMS_FLUX_CENTRAL = 0, STREAMS_FLUX_WENO = 1, STREAMS_FLUX_HYBRID = 2 };
+
+/* Grid ("Cartesian coordinates", "evaluation of grid metrics").
+ * Uniform directions: spacing l/n, node i at i*l/n.  y is stretched when y_nodes != NULL. */
+typedef struct {
+  int nx, ny, nz;
+  double lx, ly, lz;          /* domain lengths; ly is the period when y is periodic            */
+  const double* y_nodes;      /* HOST, ny node coordinates, NULL = uniform; copied at init      */
+  double y_wall_lo, y_wall_hi;/* boundary planes in y for wall / free-stream sides (staggered:  */
+                              /* the plane lies midway between the last node and the first ghost)*/
+  int bc_x, bc_y_lo, bc_y_hi, bc_z; /* STREAMS_BC_*; walls are supported in y only              */
+  double t_wall_lo, t_wall_hi;/* isothermal wall temperatures                                   */
+} streams_grid;
+
+/* Gas and flow parameters (PAPER:36 ideal gas; PAPER:40 calorically perfect branch). */
+typedef struct {
+  double gamma, rgas, prandtl;
+  int visc_law;               /* STREAMS_VISC_*                                                 */
+  double mu_ref, t_ref;       /* mu(t_ref) = mu_ref                                             */
+  double suth_s_over_tref;    /* Sutherland: mu = mu_ref t^1.5 (1+s)/(t+s), t = T/t_ref         */
+  double pow_exp;             /* power law:  mu = mu_ref t^pow_exp                              */
+  double u_ref, l_ref;        /* sensor regulariser eps_s = (u_ref/l_ref)^2                     */
+  double freestream[5];       /* conserved free-stream state for STREAMS_BC_FREESTREAM ghosts   */
+} streams_gas;
+
+/* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5). */
+typedef struct {
+  int central_order;          /* 2L: 2, 4, 6, 8                                                 */
+  int weno_order;             /* 2r-1: 1, 3, 5, 7; ignored when flux_mode == CENTRAL            */
+  int visc_order;             /* 2, 4, 6, 8; ignored when visc_law == NONE                      */
+  int flux_mode;              /* STREAMS_FLUX_*                                                 */
+  double sensor_threshold;    /* node flagged iff theta > threshold (strict)                    */
+  double weno_eps;            /* epsilon of the Jiang-Shu weights                               */
+  double cfl;                 /* dt = cfl / max rate                                            */
+  double dt_fixed;            /* > 0 overrides the CFL time step                                */
+  int dt_every;               /* recompute dt every dt_every steps (10 in production)*/
+} streams_scheme;
+
+/* Bytes of DEVICE workspace streams_init needs for this grid/gas/scheme; 0 on invalid input. */
+size_t streams_workspace_bytes(const streams_grid* grid, const streams_gas* gas,
+                               const streams_scheme* scheme);
+
+/* Create a context.  workspace_dev: DEVICE buffer of at least streams_workspace_bytes(), 256-byte
+ * aligned, owned by the caller.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Unsupported order / boundary combinations fail here with STREAMS_EINVAL, not later. */
+int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas* gas,
+                 const streams_scheme* scheme, void* workspace_dev, size_t workspace_bytes,
+                 void* cuda_stream);
+
+/* Load the conserved state w[5][nz][ny][nx] (interior).  src_is_device: 0 = HOST, 1 = DEVICE.
+ * Resets time and the step counter. */
+int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device);
+
+/* One right-hand-side evaluation R(w) of the current state (ghost fill, primitives, sensor,
+ * convective x/y/z, viscous).  rhs_out_dev: DEVICE [5][nz][ny][nx], may be NULL.
+ * Never changes the interior of w.  STREAMS_ESTATE before streams_set_fields. */
+int streams_rhs(streams_ctx* ctx, double* rhs_out_dev);
+
+/* nsteps full RK3 steps (3 RHS + 3 updates each, dt per scheme).  dt_last, time: HOST, nullable.
+ * Returns STREAMS_ENAN if the time step or the state became non-finite. */
+int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time);
+
+/* Copy the conserved state out, w_out[5][nz][ny][nx].  dst_is_device: 0 = HOST, 1 = DEVICE. */
+int streams_get_fields(streams_ctx* ctx, double* w_out, int dst_is_device);
+
+/* Sensor of the current state: theta_out [nz][ny][nx] doubles and/or mask_out [nz][ny][nx] bytes
+ * (1 = node flagged), either may be NULL.  Evaluates ghost fill + primitives + sensor. */
+int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_out,
+                       int dst_is_device);
+
+/* Diagnostics of the last RHS evaluation, HOST outputs, nullable: number of flagged nodes and
+ * number of nodes handled by the shock-capturing kernel (any adjacent interface flagged). */
+int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes);
+
+/* Number of kernels the library has launched on this context since streams_init. */
+long long streams_kernel_launches(const streams_ctx* ctx);
+
+/* Text of the last error on this context ("" if none); ctx may be NULL for init failures. */
+const char* streams_last_error(const streams_ctx* ctx);
+
+int streams_destroy(streams_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STREAMS_H */

@@ -1,0 +1,197 @@
+"""Thin ctypes binding of include/streams.h: argument marshalling only.
+
+Every step of the path runs in the kernels of libstreams.so.  PyTorch is used for device memory
+(the workspace tensor) and the CUDA stream, nothing else.  There is no CPU fallback: if the
+library or a CUDA device is missing, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
+
+STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
+EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
+           "streams_get_fields", "streams_get_sensor", "streams_get_activation", "streams_kernel_launches",
+           "streams_last_error", "streams_destroy")
+
+_dp = C.POINTER(C.c_double)
+
+
+class streams_grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
+                ("y_nodes", _dp), ("y_wall_lo", C.c_double), ("y_wall_hi", C.c_double),
+                ("bc_x", C.c_int), ("bc_y_lo", C.c_int), ("bc_y_hi", C.c_int), ("bc_z", C.c_int),
+                ("t_wall_lo", C.c_double), ("t_wall_hi", C.c_double)]
+
+
+class streams_gas(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("rgas", C.c_double), ("prandtl", C.c_double),
+                ("visc_law", C.c_int), ("mu_ref", C.c_double), ("t_ref", C.c_double),
+                ("suth_s_over_tref", C.c_double), ("pow_exp", C.c_double),
+                ("u_ref", C.c_double), ("l_ref", C.c_double), ("freestream", C.c_double * 5)]
+
+
+class streams_scheme(C.Structure):
+    _fields_ = [("central_order", C.c_int), ("weno_order", C.c_int), ("visc_order", C.c_int),
+                ("flux_mode", C.c_int), ("sensor_threshold", C.c_double), ("weno_eps", C.c_double),
+                ("cfl", C.c_double), ("dt_fixed", C.c_double), ("dt_every", C.c_int)]
+
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen libstreams.so and declare the prototypes of include/streams.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with `python -m paper_2304_05494_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    gp, ap, sp = C.POINTER(streams_grid), C.POINTER(streams_gas), C.POINTER(streams_scheme)
+    lib.streams_workspace_bytes.restype = C.c_size_t
+    lib.streams_workspace_bytes.argtypes = [gp, ap, sp]
+    lib.streams_init.argtypes = [C.POINTER(C.c_void_p), gp, ap, sp, C.c_void_p, C.c_size_t, C.c_void_p]
+    lib.streams_set_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+    lib.streams_rhs.argtypes = [C.c_void_p, C.c_void_p]
+    lib.streams_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
+    lib.streams_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+    lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+    lib.streams_get_activation.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    lib.streams_kernel_launches.restype = C.c_longlong
+    lib.streams_kernel_launches.argtypes = [C.c_void_p]
+    lib.streams_last_error.restype = C.c_char_p
+    lib.streams_last_error.argtypes = [C.c_void_p]
+    lib.streams_destroy.argtypes = [C.c_void_p]
+    _lib = lib
+    return lib
+
+
+def structs_from_case(case):
+    """workloads.Case -> (streams_grid, streams_gas, streams_scheme, keepalive)."""
+    g, a, s = streams_grid(), streams_gas(), streams_scheme()
+    for n in ("nx", "ny", "nz", "lx", "ly", "lz", "y_wall_lo", "y_wall_hi", "bc_x", "bc_y_lo", "bc_y_hi", "bc_z",
+              "t_wall_lo", "t_wall_hi"):
+        setattr(g, n, getattr(case, n))
+    keep = None
+    if case.y_nodes is not None:
+        keep = np.ascontiguousarray(case.y_nodes, dtype=np.float64)
+        g.y_nodes = keep.ctypes.data_as(_dp)
+    for n in ("gamma", "rgas", "prandtl", "visc_law", "mu_ref", "t_ref", "suth_s_over_tref", "pow_exp", "u_ref", "l_ref"):
+        setattr(a, n, getattr(case, n))
+    for q in range(5):
+        a.freestream[q] = case.freestream[q]
+    for n in ("central_order", "weno_order", "visc_order", "flux_mode", "sensor_threshold", "weno_eps", "cfl",
+              "dt_fixed", "dt_every"):
+        setattr(s, n, getattr(case, n))
+    return g, a, s, keep
+
+
+class StreamsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"streams error {code}: {msg}")
+        self.code = code
+
+
+class Streams:
+    """One solver context on the current CUDA device.  Method names follow the C ABI."""
+
+    def __init__(self, case, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: libstreams has no CPU fallback")
+        self.lib = load_library()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.case = case
+        self.shape = (case.nz, case.ny, case.nx)
+        g, a, s, self._keep = structs_from_case(case)
+        nbytes = self.lib.streams_workspace_bytes(C.byref(g), C.byref(a), C.byref(s))
+        if nbytes == 0:
+            raise StreamsError(STREAMS_EINVAL, self.lib.streams_last_error(None).decode())
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        h = C.c_void_p()
+        rc = self.lib.streams_init(C.byref(h), C.byref(g), C.byref(a), C.byref(s), C.c_void_p(ptr), nbytes,
+                                   C.c_void_p(self.stream.cuda_stream))
+        if rc != STREAMS_OK:
+            raise StreamsError(rc, self.lib.streams_last_error(None).decode())
+        self.h = h
+        self.workspace_bytes = nbytes
+        if case.w0 is not None:
+            self.set_fields(case.w0)
+
+    # -- helpers
+    def _check(self, rc):
+        if rc != STREAMS_OK:
+            raise StreamsError(rc, self.lib.streams_last_error(self.h).decode())
+
+    @staticmethod
+    def _ptr(x):
+        """(pointer, is_device) of a numpy array or torch tensor."""
+        if isinstance(x, np.ndarray):
+            assert x.flags["C_CONTIGUOUS"]
+            return C.c_void_p(x.ctypes.data), 0
+        assert x.is_contiguous()
+        return C.c_void_p(x.data_ptr()), int(x.is_cuda)
+
+    # -- C ABI
+    def set_fields(self, w):
+        if isinstance(w, np.ndarray):
+            w = np.ascontiguousarray(w, dtype=np.float64)
+        assert tuple(w.shape) == (5,) + self.shape
+        p, dev = self._ptr(w)
+        self._check(self.lib.streams_set_fields(self.h, p, dev))
+
+    def rhs(self, out=None):
+        if out is None:
+            out = self.torch.empty((5,) + self.shape, dtype=self.torch.float64, device=self.device)
+        assert out.is_cuda
+        self._check(self.lib.streams_rhs(self.h, C.c_void_p(out.data_ptr())))
+        return out
+
+    def step(self, nsteps):
+        dt, t = C.c_double(), C.c_double()
+        self._check(self.lib.streams_step(self.h, int(nsteps), C.byref(dt), C.byref(t)))
+        return dt.value, t.value
+
+    def get_fields(self, out=None):
+        if out is None:
+            out = np.empty((5,) + self.shape, dtype=np.float64)
+        p, dev = self._ptr(out)
+        self._check(self.lib.streams_get_fields(self.h, p, dev))
+        return out
+
+    def get_sensor(self):
+        theta = np.empty(self.shape, dtype=np.float64)
+        mask = np.empty(self.shape, dtype=np.uint8)
+        self._check(self.lib.streams_get_sensor(self.h, C.c_void_p(theta.ctypes.data), C.c_void_p(mask.ctypes.data), 0))
+        return theta, mask
+
+    def get_activation(self):
+        a, b = C.c_longlong(), C.c_longlong()
+        self._check(self.lib.streams_get_activation(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def kernel_launches(self):
+        return int(self.lib.streams_kernel_launches(self.h))
+
+    def destroy(self):
+        if getattr(self, "h", None):
+            self.lib.streams_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,401 @@
+// C ABI of libstreams (include/streams.h): context, workspace carving, y metrics, and the host
+// driver that sequences the kernels of one RK3 step.  No compute happens on the host.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/streams.h"
+#include "streams_dev.cuh"
+#include "streams_launch.h"
+
+using namespace streams;
+
+namespace {
+
+thread_local char g_init_error[256] = "";
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Sizes {
+  int L, Lv, r, ng, ox, px, py, pz;
+  size_t fs;            // doubles per padded field
+  size_t N;
+  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_list, off_counters, off_R, off_metrics,
+      off_scal, total;
+  int nq;
+};
+
+void fd1(int L, double* a) {
+  const double t[4][4] = {{1.0 / 2.0, 0, 0, 0},
+                          {2.0 / 3.0, -1.0 / 12.0, 0, 0},
+                          {3.0 / 4.0, -3.0 / 20.0, 1.0 / 60.0, 0},
+                          {4.0 / 5.0, -1.0 / 5.0, 4.0 / 105.0, -1.0 / 280.0}};
+  for (int l = 0; l < 4; ++l) a[l] = (L >= 1 && L <= 4) ? t[L - 1][l] : 0.0;
+}
+void fd2(int L, double* b) {
+  const double t[4][4] = {{1.0, 0, 0, 0},
+                          {4.0 / 3.0, -1.0 / 12.0, 0, 0},
+                          {3.0 / 2.0, -3.0 / 20.0, 1.0 / 90.0, 0},
+                          {8.0 / 5.0, -1.0 / 5.0, 8.0 / 315.0, -1.0 / 560.0}};
+  for (int l = 0; l < 4; ++l) b[l] = (L >= 1 && L <= 4) ? t[L - 1][l] : 0.0;
+}
+
+bool valid_bc(int b) { return b == STREAMS_BC_PERIODIC || b == STREAMS_BC_WALL_ISOTHERMAL || b == STREAMS_BC_FREESTREAM; }
+
+// Validates the problem and lays out the workspace.  Returns NULL on success, else a message.
+const char* plan(const streams_grid* g, const streams_gas* gas, const streams_scheme* sc, Sizes& S) {
+  if (!g || !gas || !sc) return "null argument";
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid extents must be positive";
+  if ((long long)g->nx * g->ny * g->nz > 2000000000LL) return "grid too large for 32-bit node indices";
+  if (!(g->lx > 0) || !(g->lz > 0)) return "lx, lz must be positive";
+  if (!valid_bc(g->bc_x) || !valid_bc(g->bc_y_lo) || !valid_bc(g->bc_y_hi) || !valid_bc(g->bc_z)) return "bad bc code";
+  if (g->bc_x == STREAMS_BC_WALL_ISOTHERMAL || g->bc_z == STREAMS_BC_WALL_ISOTHERMAL) return "walls are supported in y only";
+  if ((g->bc_y_lo == STREAMS_BC_PERIODIC) != (g->bc_y_hi == STREAMS_BC_PERIODIC)) return "y periodic on one side only";
+  if (g->bc_y_lo == STREAMS_BC_PERIODIC && !(g->ly > 0)) return "ly must be positive";
+  if (g->bc_y_lo != STREAMS_BC_PERIODIC && !(g->y_wall_hi > g->y_wall_lo)) return "y_wall_hi must exceed y_wall_lo";
+  if (sc->central_order < 2 || sc->central_order > 8 || sc->central_order % 2) return "central_order must be 2, 4, 6 or 8";
+  if (sc->flux_mode < 0 || sc->flux_mode > 2) return "bad flux_mode";
+  if (gas->visc_law < 0 || gas->visc_law > 2) return "bad visc_law";
+  if (sc->flux_mode != STREAMS_FLUX_CENTRAL && (sc->weno_order < 1 || sc->weno_order > 7 || sc->weno_order % 2 == 0))
+    return "weno_order must be 1, 3, 5 or 7";
+  if (gas->visc_law != STREAMS_VISC_NONE && (sc->visc_order < 2 || sc->visc_order > 8 || sc->visc_order % 2))
+    return "visc_order must be 2, 4, 6 or 8";
+  if (!(gas->gamma > 1) || !(gas->rgas > 0)) return "gamma must exceed 1 and rgas be positive";
+  if (gas->visc_law != STREAMS_VISC_NONE && (!(gas->prandtl > 0) || !(gas->t_ref > 0))) return "prandtl, t_ref must be positive";
+  if (sc->flux_mode == STREAMS_FLUX_HYBRID && !(gas->l_ref > 0)) return "l_ref must be positive";
+  if (!(sc->dt_fixed > 0) && !(sc->cfl > 0)) return "cfl must be positive when dt_fixed is not set";
+  S.L = sc->central_order / 2;
+  S.Lv = gas->visc_law == STREAMS_VISC_NONE ? 0 : sc->visc_order / 2;
+  S.r = sc->flux_mode == STREAMS_FLUX_CENTRAL ? 0 : (sc->weno_order + 1) / 2;
+  S.ng = S.L > S.Lv ? S.L : S.Lv;
+  if (S.r > S.ng) S.ng = S.r;
+  if (!rhs_supported(S.L, S.Lv, S.r, sc->flux_mode, gas->visc_law))
+    return "this build instantiates central order 6, WENO order 5, viscous order 6 only";
+  if (g->nx < S.ng || g->ny < S.ng || g->nz < S.ng) return "each extent must be at least the ghost width";
+  S.ox = 16;                                              // interior i = 0 starts a 128-byte line
+  S.px = (int)align_up((size_t)S.ox + g->nx + S.ng, 16);
+  S.py = g->ny + 2 * S.ng;
+  S.pz = g->nz + 2 * S.ng;
+  S.fs = align_up((size_t)S.px * S.py * S.pz, 32);
+  S.N = (size_t)g->nx * g->ny * g->nz;
+  S.nq = NQ;
+  const bool hyb = sc->flux_mode == STREAMS_FLUX_HYBRID;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  S.off_w = take(5 * S.fs * 8);
+  S.off_q = take((size_t)S.nq * S.fs * 8);
+  S.off_div = take(S.fs * 8);
+  S.off_theta = take(S.N * 8);
+  S.off_mask = take(S.fs);
+  S.off_nflag = take(hyb ? S.N : 256);
+  S.off_list = take(hyb ? S.N * 4 : 256);
+  S.off_counters = take(256);
+  S.off_R = take(5 * S.N * 8);
+  S.off_metrics = take(3 * (size_t)g->ny * 8);
+  S.off_scal = take(S_COUNT * 8);
+  S.total = off;
+  return nullptr;
+}
+
+}  // namespace
+
+struct streams_ctx {
+  streams_grid grid;
+  streams_gas gas;
+  streams_scheme scheme;
+  Sizes S;
+  DevP P;
+  cudaStream_t stream;
+  char* base;
+  bool have_fields;
+  long long step_count;     // steps since set_fields (host mirror; decides when dt is recomputed)
+  long long launches;
+  char err[256];
+};
+
+namespace {
+
+int fail(streams_ctx* c, int code, const char* msg) {
+  if (c) std::snprintf(c->err, sizeof c->err, "%s", msg);
+  else std::snprintf(g_init_error, sizeof g_init_error, "%s", msg);
+  return code;
+}
+int cuda_fail(streams_ctx* c, cudaError_t e, const char* where) {
+  char buf[256];
+  std::snprintf(buf, sizeof buf, "%s: %s", where, cudaGetErrorString(e));
+  return fail(c, STREAMS_ECUDA, buf);
+}
+#define CU(call)                                                   \
+  do {                                                             \
+    cudaError_t e__ = (call);                                      \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);     \
+  } while (0)
+
+// y metrics on the host (O4 / S3), same evaluation order as the definition:
+// D = a_1 (y_{+1} - y_{-1}); D = D + a_l (y_{+l} - y_{-l}); eta_y = 1 / D;
+// eta_yy = -(D2) eta_y^3 with D2 = sum_l b_l ((y_{+l} - 2 y_0) + y_{-l}).
+void build_metrics(const streams_ctx* c, const double* y_nodes, std::vector<double>& eyc, std::vector<double>& eyv,
+                   std::vector<double>& eyyv) {
+  const streams_grid& g = c->grid;
+  const int ny = g.ny, ng = c->S.ng, L = c->S.L, Lv = c->S.Lv;
+  eyc.assign(ny, 0.0); eyv.assign(ny, 0.0); eyyv.assign(ny, 0.0);
+  const bool per = g.bc_y_lo == STREAMS_BC_PERIODIC;
+  if (!y_nodes) {
+    const double inv_dy = per ? (double)ny / g.ly : (double)ny / (g.y_wall_hi - g.y_wall_lo);
+    for (int j = 0; j < ny; ++j) { eyc[j] = inv_dy; eyv[j] = inv_dy; }
+    return;
+  }
+  std::vector<double> yn(ny + 2 * ng);
+  for (int j = 0; j < ny; ++j) yn[j + ng] = y_nodes[j];
+  for (int m = 0; m < ng; ++m) {
+    if (per) {
+      yn[ng - 1 - m] = y_nodes[ny - 1 - m] - g.ly;
+      yn[ng + ny + m] = y_nodes[m] + g.ly;
+    } else {
+      yn[ng - 1 - m] = 2.0 * g.y_wall_lo - y_nodes[m];
+      yn[ng + ny + m] = 2.0 * g.y_wall_hi - y_nodes[ny - 1 - m];
+    }
+  }
+  for (int j = 0; j < ny; ++j) {
+    const double* y = &yn[j + ng];
+    double acc = c->P.a1[0] * (y[1] - y[-1]);
+    for (int l = 2; l <= L; ++l) acc = acc + c->P.a1[l - 1] * (y[l] - y[-l]);
+    eyc[j] = 1.0 / acc;
+    if (Lv > 0) {
+      double d1 = c->P.a1v[0] * (y[1] - y[-1]);
+      for (int l = 2; l <= Lv; ++l) d1 = d1 + c->P.a1v[l - 1] * (y[l] - y[-l]);
+      double d2 = c->P.b2v[0] * ((y[1] - 2.0 * y[0]) + y[-1]);
+      for (int l = 2; l <= Lv; ++l) d2 = d2 + c->P.b2v[l - 1] * ((y[l] - 2.0 * y[0]) + y[-l]);
+      const double ey = 1.0 / d1;
+      eyv[j] = ey;
+      eyyv[j] = -d2 * ((ey * ey) * ey);
+    }
+  }
+}
+
+// ghost fill + primitives (+ dt) + sensor + flags: everything a stage needs before the RHS kernels
+int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
+  const DevP& P = ctx->P;
+  ctx->launches += launch_fill_prim(P, ctx->stream);
+  if (want_dt) ctx->launches += launch_dt(P, ctx->scheme.dt_fixed, ctx->stream);
+  const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
+  const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
+  if (hyb || visc || theta) ctx->launches += launch_sensor(P, ctx->S.L, hyb || theta, theta, ctx->stream);
+  if (hyb) ctx->launches += launch_flags(P, ctx->S.r, ctx->stream);
+  return STREAMS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t streams_workspace_bytes(const streams_grid* grid, const streams_gas* gas, const streams_scheme* scheme) {
+  Sizes S;
+  const char* msg = plan(grid, gas, scheme, S);
+  if (msg) { fail(nullptr, STREAMS_EINVAL, msg); return 0; }
+  return S.total;
+}
+
+int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas* gas, const streams_scheme* scheme,
+                 void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return fail(nullptr, STREAMS_EINVAL, "out is null");
+  *out = nullptr;
+  Sizes S;
+  const char* msg = plan(grid, gas, scheme, S);
+  if (msg) return fail(nullptr, STREAMS_EINVAL, msg);
+  if (!workspace_dev || workspace_bytes < S.total) return fail(nullptr, STREAMS_ENOMEM, "workspace too small");
+  if (((uintptr_t)workspace_dev) % 256) return fail(nullptr, STREAMS_EINVAL, "workspace must be 256-byte aligned");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, STREAMS_ECUDA, "no CUDA device");
+  streams_ctx* ctx = new (std::nothrow) streams_ctx();
+  if (!ctx) return fail(nullptr, STREAMS_ENOMEM, "host allocation failed");
+  ctx->grid = *grid; ctx->gas = *gas; ctx->scheme = *scheme; ctx->S = S;
+  ctx->grid.y_nodes = nullptr;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->base = (char*)workspace_dev;
+  ctx->have_fields = false; ctx->step_count = 0; ctx->launches = 0; ctx->err[0] = 0;
+  if (ctx->scheme.dt_every < 1) ctx->scheme.dt_every = 1;
+  DevP& P = ctx->P;
+  std::memset(&P, 0, sizeof P);
+  P.nx = grid->nx; P.ny = grid->ny; P.nz = grid->nz; P.ng = S.ng; P.ox = S.ox;
+  P.px = S.px; P.py = S.py; P.pz = S.pz;
+  P.sy = S.px; P.sz = (long long)S.px * S.py; P.fs = (long long)S.fs; P.N = (long long)S.N;
+  P.w = (double*)(ctx->base + S.off_w);
+  P.q = (double*)(ctx->base + S.off_q);
+  P.div = (double*)(ctx->base + S.off_div);
+  P.theta = (double*)(ctx->base + S.off_theta);
+  P.mask = (unsigned char*)(ctx->base + S.off_mask);
+  P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
+  P.list = (int*)(ctx->base + S.off_list);
+  P.counters = (int*)(ctx->base + S.off_counters);
+  P.R = (double*)(ctx->base + S.off_R);
+  double* met = (double*)(ctx->base + S.off_metrics);
+  P.eta_y_c = met; P.eta_y_v = met + grid->ny; P.eta_yy_v = met + 2 * (size_t)grid->ny;
+  P.scal = (double*)(ctx->base + S.off_scal);
+  P.inv_dx = (double)grid->nx / grid->lx;
+  P.inv_dz = (double)grid->nz / grid->lz;
+  fd1(S.L, P.a1); fd1(S.Lv, P.a1v); fd2(S.Lv, P.b2v);
+  P.gamma = gas->gamma; P.gm1 = gas->gamma - 1.0; P.rgas = gas->rgas; P.prandtl = gas->prandtl;
+  P.kfac = (gas->gamma * gas->rgas / (gas->gamma - 1.0)) / gas->prandtl;
+  P.mu_ref = gas->mu_ref; P.t_ref = gas->t_ref; P.suth_s = gas->suth_s_over_tref; P.pow_exp = gas->pow_exp;
+  const double rr = gas->u_ref / gas->l_ref;
+  P.eps_s = rr * rr;
+  P.thr = scheme->sensor_threshold; P.weno_eps = scheme->weno_eps; P.cfl = scheme->cfl;
+  for (int q = 0; q < 5; ++q) P.fsw[q] = gas->freestream[q];
+  P.t_wall_lo = grid->t_wall_lo; P.t_wall_hi = grid->t_wall_hi;
+  P.bc_x = grid->bc_x; P.bc_y_lo = grid->bc_y_lo; P.bc_y_hi = grid->bc_y_hi; P.bc_z = grid->bc_z;
+  P.visc_law = gas->visc_law; P.flux_mode = scheme->flux_mode;
+
+  std::vector<double> eyc, eyv, eyyv;
+  build_metrics(ctx, grid->y_nodes, eyc, eyv, eyyv);
+  cudaError_t e = cudaMemsetAsync(ctx->base, 0, S.total, ctx->stream);   // defined ghosts / scalars from the start
+  if (e == cudaSuccess) e = cudaMemcpyAsync(met, eyc.data(), grid->ny * 8, cudaMemcpyHostToDevice, ctx->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(met + grid->ny, eyv.data(), grid->ny * 8, cudaMemcpyHostToDevice, ctx->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(met + 2 * (size_t)grid->ny, eyyv.data(), grid->ny * 8, cudaMemcpyHostToDevice, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);          // host vectors go out of scope
+  if (e != cudaSuccess) {
+    cuda_fail(nullptr, e, "streams_init");
+    delete ctx;
+    return STREAMS_ECUDA;
+  }
+  *out = ctx;
+  return STREAMS_OK;
+}
+
+int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
+  if (!ctx || !w) return fail(ctx, STREAMS_EINVAL, "null argument");
+  const DevP& P = ctx->P;
+  const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  for (int q = 0; q < 5; ++q) {
+    cudaMemcpy3DParms p;
+    std::memset(&p, 0, sizeof p);
+    p.srcPtr = make_cudaPitchedPtr((void*)(w + (size_t)q * P.N), (size_t)P.nx * 8, P.nx, P.ny);
+    p.dstPtr = make_cudaPitchedPtr((void*)(P.w + q * P.fs), (size_t)P.px * 8, P.px, P.py);
+    p.dstPos = make_cudaPos((size_t)P.ox * 8, P.ng, P.ng);
+    p.extent = make_cudaExtent((size_t)P.nx * 8, P.ny, P.nz);
+    p.kind = kind;
+    CU(cudaMemcpy3DAsync(&p, ctx->stream));
+  }
+  CU(cudaMemsetAsync(P.scal, 0, S_COUNT * 8, ctx->stream));
+  if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));   // the host buffer may be reused on return
+  ctx->have_fields = true;
+  ctx->step_count = 0;
+  return STREAMS_OK;
+}
+
+int streams_get_fields(streams_ctx* ctx, double* w_out, int dst_is_device) {
+  if (!ctx || !w_out) return fail(ctx, STREAMS_EINVAL, "null argument");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
+  const DevP& P = ctx->P;
+  const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  for (int q = 0; q < 5; ++q) {
+    cudaMemcpy3DParms p;
+    std::memset(&p, 0, sizeof p);
+    p.srcPtr = make_cudaPitchedPtr((void*)(P.w + q * P.fs), (size_t)P.px * 8, P.px, P.py);
+    p.srcPos = make_cudaPos((size_t)P.ox * 8, P.ng, P.ng);
+    p.dstPtr = make_cudaPitchedPtr((void*)(w_out + (size_t)q * P.N), (size_t)P.nx * 8, P.nx, P.ny);
+    p.extent = make_cudaExtent((size_t)P.nx * 8, P.ny, P.nz);
+    p.kind = kind;
+    CU(cudaMemcpy3DAsync(&p, ctx->stream));
+  }
+  if (!dst_is_device) CU(cudaStreamSynchronize(ctx->stream));
+  return STREAMS_OK;
+}
+
+int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_rhs before streams_set_fields");
+  enqueue_prepare(ctx, false, false);
+  StageArgs sa;
+  sa.gam = 0.0; sa.rhk = 0.0; sa.update_w = 0; sa.read_prev = 0; sa.write_r = 1;
+  sa.r_out = rhs_out_dev ? rhs_out_dev : ctx->P.R;
+  const int n = launch_rhs(ctx->P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, ctx->stream);
+  if (n < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
+  ctx->launches += n;
+  CU(cudaGetLastError());
+  return STREAMS_OK;
+}
+
+int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_step before streams_set_fields");
+  if (nsteps < 0) return fail(ctx, STREAMS_EINVAL, "nsteps must be non-negative");
+  // Wray's low-storage RK3 (O5 / S12)
+  const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+  const double rhk[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+  for (int s = 0; s < nsteps; ++s) {
+    const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
+    for (int l = 0; l < 3; ++l) {
+      enqueue_prepare(ctx, want_dt && l == 0, false);
+      StageArgs sa;
+      sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
+      sa.r_out = ctx->P.R;
+      const int n = launch_rhs(ctx->P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, ctx->stream);
+      if (n < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
+      ctx->launches += n;
+    }
+    ctx->launches += launch_step_end(ctx->P, ctx->stream);
+    ctx->step_count += 1;
+  }
+  CU(cudaGetLastError());
+  double h[S_COUNT];
+  CU(cudaMemcpyAsync(h, ctx->P.scal, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (dt_last) *dt_last = h[S_DT];
+  if (time) *time = h[S_TIME];
+  if (h[S_NAN] != 0.0 || !std::isfinite(h[S_DT]) || !std::isfinite(h[S_TIME]))
+    return fail(ctx, STREAMS_ENAN, "non-finite time step");
+  return STREAMS_OK;
+}
+
+int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_out, int dst_is_device) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
+  const DevP& P = ctx->P;
+  ctx->launches += launch_fill_prim(P, ctx->stream);
+  ctx->launches += launch_sensor(P, ctx->S.L, true, true, ctx->stream);
+  CU(cudaGetLastError());
+  const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  if (theta_out) CU(cudaMemcpyAsync(theta_out, P.theta, (size_t)P.N * 8, kind, ctx->stream));
+  if (mask_out) {
+    cudaMemcpy3DParms p;
+    std::memset(&p, 0, sizeof p);
+    p.srcPtr = make_cudaPitchedPtr((void*)P.mask, (size_t)P.px, P.px, P.py);
+    p.srcPos = make_cudaPos((size_t)P.ox, P.ng, P.ng);
+    p.dstPtr = make_cudaPitchedPtr((void*)mask_out, (size_t)P.nx, P.nx, P.ny);
+    p.extent = make_cudaExtent((size_t)P.nx, P.ny, P.nz);
+    p.kind = kind;
+    CU(cudaMemcpy3DAsync(&p, ctx->stream));
+  }
+  if (!dst_is_device) CU(cudaStreamSynchronize(ctx->stream));
+  return STREAMS_OK;
+}
+
+int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  int h[2] = {0, 0};
+  if (ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID) {
+    CU(cudaMemcpyAsync(h, ctx->P.counters, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+  } else if (ctx->scheme.flux_mode == STREAMS_FLUX_WENO) {
+    h[0] = (int)ctx->P.N; h[1] = (int)ctx->P.N;
+  }
+  if (shock_nodes) *shock_nodes = h[0];
+  if (flagged_nodes) *flagged_nodes = h[1];
+  return STREAMS_OK;
+}
+
+long long streams_kernel_launches(const streams_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* streams_last_error(const streams_ctx* ctx) { return ctx ? ctx->err : g_init_error; }
+
+int streams_destroy(streams_ctx* ctx) {
+  if (!ctx) return STREAMS_EINVAL;
+  cudaStreamSynchronize(ctx->stream);
+  delete ctx;
+  return STREAMS_OK;
+}
+
+}  // extern "C"

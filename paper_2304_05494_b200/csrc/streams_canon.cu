@@ -1,0 +1,340 @@
+// Kernels whose arithmetic decides an integer (the shock-sensor mask) or feeds it:
+// ghost fill + conservative->primitive, sensor/mask, interface flags, time-step reduction.
+// This translation unit is compiled with -fmad=false so that every operation is a single
+// IEEE fp64 operation in source order: the
+// mask is then bit-identical to any IEEE evaluation of the same formulas on the same state.
+#include "streams_dev.cuh"
+#include "streams_launch.h"
+
+namespace streams {
+
+// ---------------------------------------------------------------------------------------------
+// a1 + a2: ghost / boundary fill and conservative -> primitive in one pass over the padded box.
+// Each padded node finds the interior node it images (periodic wrap, wall mirror) or takes the
+// free-stream state, rebuilds the conserved ghost state (isothermal no-slip wall: u -> -u,
+// T -> 2 T_w - T, p -> p, rho = p/(R T); O6) and then the primitives.
+// HBM: 40 B read (interior) + 8 B x (#primitive fields) write per padded node.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double viscosity(const DevP& P, double T) {
+  const double t = T / P.t_ref;
+  if (P.visc_law == VISC_SUTHERLAND) return ((P.mu_ref * (t * sqrt(t))) * (1.0 + P.suth_s)) / (t + P.suth_s);
+  return P.mu_ref * pow(t, P.pow_exp);
+}
+
+template <bool VISC, bool STORE_C>
+__global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
+  if (i < -P.ng || i >= P.nx + P.ng) return;
+  int is = i, js = j, ks = k;
+  bool fsx = false, fsy = false, fsz = false;
+  double t_wall = 0.0;
+  bool wall = false;
+  if (i < 0) { if (P.bc_x == BC_PERIODIC) is = i + P.nx; else { fsx = true; is = 0; } }
+  else if (i >= P.nx) { if (P.bc_x == BC_PERIODIC) is = i - P.nx; else { fsx = true; is = P.nx - 1; } }
+  if (j < 0) {
+    if (P.bc_y_lo == BC_PERIODIC) js = j + P.ny;
+    else if (P.bc_y_lo == BC_WALL) { js = -1 - j; wall = true; t_wall = P.t_wall_lo; }
+    else { fsy = true; js = 0; }
+  } else if (j >= P.ny) {
+    if (P.bc_y_hi == BC_PERIODIC) js = j - P.ny;
+    else if (P.bc_y_hi == BC_WALL) { js = 2 * P.ny - 1 - j; wall = true; t_wall = P.t_wall_hi; }
+    else { fsy = true; js = P.ny - 1; }
+  }
+  if (k < 0) { if (P.bc_z == BC_PERIODIC) ks = k + P.nz; else { fsz = true; ks = 0; } }
+  else if (k >= P.nz) { if (P.bc_z == BC_PERIODIC) ks = k - P.nz; else { fsz = true; ks = P.nz - 1; } }
+
+  const long long ns = pidx(P, is, js, ks);
+  double s[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) s[q] = P.w[q * P.fs + ns];
+  if (fsx) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
+  }
+  if (fsy) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
+  } else if (wall) {
+    const double rho = s[0];
+    const double uu = s[1] / rho, vv = s[2] / rho, wv = s[3] / rho;
+    const double ke = 0.5 * ((uu * uu + vv * vv) + wv * wv);
+    const double pp = P.gm1 * (s[4] - rho * ke);
+    const double TT = pp / (rho * P.rgas);
+    double Tg = 2.0 * t_wall - TT;
+    const double Tmin = 0.1 * t_wall;
+    if (Tg < Tmin) Tg = Tmin;
+    const double rg = pp / (P.rgas * Tg);
+    s[0] = rg;
+    s[1] = -(rg * uu);
+    s[2] = -(rg * vv);
+    s[3] = -(rg * wv);
+    s[4] = pp / P.gm1 + rg * ke;
+  }
+  if (fsz) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
+  }
+  const long long n = pidx(P, i, j, k);
+  const bool ghost = (is != i) || (js != j) || (ks != k) || fsx || fsy || fsz;
+  if (ghost) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) P.w[q * P.fs + n] = s[q];
+  }
+  const double rho = s[0];
+  const double uu = s[1] / rho, vv = s[2] / rho, wv = s[3] / rho;
+  const double ke = 0.5 * ((uu * uu + vv * vv) + wv * wv);
+  const double pp = P.gm1 * (s[4] - rho * ke);
+  P.q[Q_U * P.fs + n] = uu;
+  P.q[Q_V * P.fs + n] = vv;
+  P.q[Q_W * P.fs + n] = wv;
+  P.q[Q_H * P.fs + n] = (s[4] + pp) / rho;
+  P.q[Q_P * P.fs + n] = pp;
+  P.q[Q_RHO * P.fs + n] = rho;
+  if (VISC) {
+    const double TT = pp / (rho * P.rgas);
+    P.q[Q_T * P.fs + n] = TT;
+    P.q[Q_MU * P.fs + n] = viscosity(P, TT);
+  }
+  if (STORE_C) P.q[Q_C * P.fs + n] = sqrt(P.gamma * pp / rho);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3: Ducros-type sensor, node mask and dilatation (O2).  One thread per interior node.
+// Canonical order: delta_l = f(+l) - f(-l); acc = a_1 delta_1; acc = acc + a_l delta_l; d = acc * metric;
+// div = (u_x + v_y) + w_z; s = (((div^2 + ox^2) + oy^2) + oz^2) + eps_s; theta = max(-div/sqrt(s), 0).
+// Threads next to a face also write the ghost images of div / mask (periodic wrap, else constant
+// extrapolation; S6).  HBM: 24 B read + 8 B (div) + 1 B (mask) write per node.
+// ---------------------------------------------------------------------------------------------
+template <int L>
+__device__ __forceinline__ double ddc(const DevP& P, const double* __restrict__ f, long long n, long long s, double metric) {
+  double acc = P.a1[0] * (f[n + s] - f[n - s]);
+#pragma unroll
+  for (int l = 2; l <= L; ++l) acc = acc + P.a1[l - 1] * (f[n + l * s] - f[n - l * s]);
+  return acc * metric;
+}
+
+template <class T>
+__device__ __forceinline__ void write_images(const DevP& P, T* f, T val, int i, int j, int k, long long n) {
+  const int g = P.ng;
+  if (P.bc_x == BC_PERIODIC) {
+    if (i < g) f[n + P.nx] = val;
+    if (i >= P.nx - g) f[n - P.nx] = val;
+  } else {
+    if (i == 0) for (int m = 1; m <= g; ++m) f[n - m] = val;
+    if (i == P.nx - 1) for (int m = 1; m <= g; ++m) f[n + m] = val;
+  }
+  if (P.bc_y_lo == BC_PERIODIC) { if (j >= P.ny - g) f[n - (long long)P.ny * P.sy] = val; }
+  else if (j == 0) for (int m = 1; m <= g; ++m) f[n - m * P.sy] = val;
+  if (P.bc_y_hi == BC_PERIODIC) { if (j < g) f[n + (long long)P.ny * P.sy] = val; }
+  else if (j == P.ny - 1) for (int m = 1; m <= g; ++m) f[n + m * P.sy] = val;
+  if (P.bc_z == BC_PERIODIC) {
+    if (k < g) f[n + (long long)P.nz * P.sz] = val;
+    if (k >= P.nz - g) f[n - (long long)P.nz * P.sz] = val;
+  } else {
+    if (k == 0) for (int m = 1; m <= g; ++m) f[n - m * P.sz] = val;
+    if (k == P.nz - 1) for (int m = 1; m <= g; ++m) f[n + m * P.sz] = val;
+  }
+}
+
+template <int L, bool MASK, bool THETA>
+__global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= P.nx || j >= P.ny) return;
+  const long long n = pidx(P, i, j, k);
+  const double* __restrict__ u = P.q + Q_U * P.fs;
+  const double* __restrict__ v = P.q + Q_V * P.fs;
+  const double* __restrict__ w = P.q + Q_W * P.fs;
+  const double my = P.eta_y_c[j];
+  const double ux = ddc<L>(P, u, n, 1, P.inv_dx), uy = ddc<L>(P, u, n, P.sy, my), uz = ddc<L>(P, u, n, P.sz, P.inv_dz);
+  const double vx = ddc<L>(P, v, n, 1, P.inv_dx), vy = ddc<L>(P, v, n, P.sy, my), vz = ddc<L>(P, v, n, P.sz, P.inv_dz);
+  const double wx = ddc<L>(P, w, n, 1, P.inv_dx), wy = ddc<L>(P, w, n, P.sy, my), wz = ddc<L>(P, w, n, P.sz, P.inv_dz);
+  const double dv = (ux + vy) + wz;
+  P.div[n] = dv;
+  write_images<double>(P, P.div, dv, i, j, k, n);
+  if (MASK || THETA) {
+    const double ox = wy - vz, oy = uz - wx, oz = vx - uy;
+    const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
+    double th = -dv / sqrt(s);
+    if (!(th > 0.0)) th = 0.0;
+    if (THETA) P.theta[iidx(P, i, j, k)] = th;
+    if (MASK) {
+      const unsigned char m = (th > P.thr) ? 1 : 0;
+      P.mask[n] = m;
+      write_images<unsigned char>(P, P.mask, m, i, j, k, n);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Interface flags (O2 / S5): interface n+1/2 along d uses WENO iff any node of its 2r-node
+// stencil {n-r+1..n+r} is flagged.  Per interior node the six adjacent interfaces are packed in a
+// byte (bit 2d: minus side, bit 2d+1: plus side); nodes with any bit set are appended to the
+// shock-node list (warp-aggregated atomic; order is irrelevant, each node is computed independently).
+// ---------------------------------------------------------------------------------------------
+template <int R>
+__global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  const bool in = (i < P.nx && j < P.ny);
+  unsigned f = 0, own = 0;
+  long long o = 0;
+  if (in) {
+    const long long n = pidx(P, i, j, k);
+    o = iidx(P, i, j, k);
+    const long long st[3] = {1, P.sy, P.sz};
+    own = P.mask[n];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      unsigned mid = 0;
+#pragma unroll
+      for (int m = -R + 1; m <= R - 1; ++m) mid |= P.mask[n + m * st[d]];
+      const unsigned lo = mid | P.mask[n - R * st[d]];
+      const unsigned hi = mid | P.mask[n + R * st[d]];
+      f |= (lo ? 1u : 0u) << (2 * d);
+      f |= (hi ? 1u : 0u) << (2 * d + 1);
+    }
+    P.nflag[o] = (unsigned char)f;
+  }
+  const unsigned ball = __ballot_sync(0xffffffffu, f != 0);
+  const unsigned ballm = __ballot_sync(0xffffffffu, own != 0);
+  const int lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31;
+  int base = 0;
+  if (lane == 0) {
+    if (ball) base = atomicAdd(&P.counters[0], __popc(ball));
+    if (ballm) atomicAdd(&P.counters[1], __popc(ballm));
+  }
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (f != 0) P.list[base + __popc(ball & ((1u << lane) - 1u))] = (int)o;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a9: time-step reduction (O5 / S13): max over interior nodes and directions of
+// (|u_d| + c) m_d, nu m_d^2, gamma nu m_d^2 / Pr.  Warp-shuffle max on the bit patterns (rates are
+// non-negative, so unsigned order = numeric order, and a NaN wins and is detected), one atomicMax
+// per block.  HBM: ~56 B read per node.
+// ---------------------------------------------------------------------------------------------
+template <bool VISC>
+__global__ void __launch_bounds__(256) dt_kernel(const DevP P) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  double rmax = 0.0;
+  if (i < P.nx && j < P.ny) {
+    const long long n = pidx(P, i, j, k);
+    const double rho = P.q[Q_RHO * P.fs + n];
+    const double pp = P.q[Q_P * P.fs + n];
+    const double c = sqrt(P.gamma * pp / rho);
+    const double md[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+    const double vel[3] = {P.q[Q_U * P.fs + n], P.q[Q_V * P.fs + n], P.q[Q_W * P.fs + n]};
+    double nu = 0.0;
+    if (VISC) nu = P.q[Q_MU * P.fs + n] / rho;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      rmax = fmax(rmax, (fabs(vel[d]) + c) * md[d]);
+      if (VISC) {
+        rmax = fmax(rmax, nu * (md[d] * md[d]));
+        rmax = fmax(rmax, (P.gamma * nu / P.prandtl) * (md[d] * md[d]));
+      }
+    }
+    if (!(rmax == rmax) || !(c == c)) rmax = __longlong_as_double(0x7ff8000000000000LL);
+  }
+  unsigned long long bits = (unsigned long long)__double_as_longlong(rmax);
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) {
+    const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
+    bits = o > bits ? o : bits;
+  }
+  __shared__ unsigned long long sm[8];
+  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+  if ((tid & 31) == 0) sm[tid >> 5] = bits;
+  __syncthreads();
+  if (tid < 32) {
+    bits = tid < (int)((blockDim.x * blockDim.y + 31) >> 5) ? sm[tid] : 0ull;
+#pragma unroll
+    for (int s = 4; s > 0; s >>= 1) {
+      const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
+      bits = o > bits ? o : bits;
+    }
+    if (tid == 0) atomicMax(reinterpret_cast<unsigned long long*>(P.scal + S_RATE), bits);
+  }
+}
+
+__global__ void dt_finalize_kernel(const DevP P, double dt_fixed) {
+  const double rate = P.scal[S_RATE];
+  const double dt = dt_fixed > 0.0 ? dt_fixed : P.cfl / rate;
+  P.scal[S_DT] = dt;
+  P.scal[S_RATE] = 0.0;
+  if (!isfinite(dt)) P.scal[S_NAN] = 1.0;
+}
+
+__global__ void step_end_kernel(const DevP P) {
+  P.scal[S_TIME] = P.scal[S_TIME] + P.scal[S_DT];
+  P.scal[S_NSTEP] = P.scal[S_NSTEP] + 1.0;
+}
+
+__global__ void reset_counters_kernel(const DevP P) { P.counters[0] = 0; P.counters[1] = 0; }
+
+// -------------------------------------------------------------------------- launch wrappers
+static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }
+
+int launch_fill_prim(const DevP& P, cudaStream_t st) {
+  dim3 b(128), g((P.px + 127) / 128, P.py, P.pz);
+  const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
+  if (visc && sc) fill_prim_kernel<true, true><<<g, b, 0, st>>>(P);
+  else if (visc) fill_prim_kernel<true, false><<<g, b, 0, st>>>(P);
+  else if (sc) fill_prim_kernel<false, true><<<g, b, 0, st>>>(P);
+  else fill_prim_kernel<false, false><<<g, b, 0, st>>>(P);
+  return 1;
+}
+
+template <int L>
+static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st) {
+  dim3 b(64, 4), g = grid2d(P, b);
+  if (theta) sensor_kernel<L, true, true><<<g, b, 0, st>>>(P);
+  else if (mask) sensor_kernel<L, true, false><<<g, b, 0, st>>>(P);
+  else sensor_kernel<L, false, false><<<g, b, 0, st>>>(P);
+  return 1;
+}
+int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st) {
+  switch (L) {
+    case 1: return launch_sensor_L<1>(P, mask, theta, st);
+    case 2: return launch_sensor_L<2>(P, mask, theta, st);
+    case 3: return launch_sensor_L<3>(P, mask, theta, st);
+    default: return launch_sensor_L<4>(P, mask, theta, st);
+  }
+}
+
+int launch_flags(const DevP& P, int r, cudaStream_t st) {
+  dim3 b(64, 4), g = grid2d(P, b);
+  reset_counters_kernel<<<1, 1, 0, st>>>(P);
+  switch (r) {
+    case 1: flags_kernel<1><<<g, b, 0, st>>>(P); break;
+    case 2: flags_kernel<2><<<g, b, 0, st>>>(P); break;
+    case 3: flags_kernel<3><<<g, b, 0, st>>>(P); break;
+    default: flags_kernel<4><<<g, b, 0, st>>>(P); break;
+  }
+  return 2;
+}
+
+int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st) {
+  int n = 0;
+  if (!(dt_fixed > 0.0)) {
+    dim3 b(64, 4), g = grid2d(P, b);
+    if (P.visc_law != VISC_NONE) dt_kernel<true><<<g, b, 0, st>>>(P);
+    else dt_kernel<false><<<g, b, 0, st>>>(P);
+    ++n;
+  }
+  dt_finalize_kernel<<<1, 1, 0, st>>>(P, dt_fixed);
+  return n + 1;
+}
+
+int launch_step_end(const DevP& P, cudaStream_t st) {
+  step_end_kernel<<<1, 1, 0, st>>>(P);
+  return 1;
+}
+
+}  // namespace streams

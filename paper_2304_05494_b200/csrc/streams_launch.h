@@ -1,0 +1,27 @@
+// Host-side launch wrappers implemented by the kernel translation units.
+// Each returns the number of kernels it launched.
+#pragma once
+#include <cuda_runtime.h>
+#include "streams_dev.cuh"
+
+namespace streams {
+
+// RK stage description for the fused RHS + update kernels.
+struct StageArgs {
+  double gam, rhk;      // w += dt (gam R + rhk R_prev)            (O5)
+  int update_w;         // 0: RHS only (streams_rhs)
+  int read_prev;        // stage uses the previous-stage RHS
+  int write_r;          // keep R for the next stage
+  double* r_out;        // where R goes when write_r (interior [5][N])
+};
+
+int launch_fill_prim(const DevP& P, cudaStream_t st);
+int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st);
+int launch_flags(const DevP& P, int r, cudaStream_t st);
+int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);
+int launch_step_end(const DevP& P, cudaStream_t st);
+// returns < 0 if the (L, Lv, r) combination is not instantiated
+int launch_rhs(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
+bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law);
+
+}  // namespace streams

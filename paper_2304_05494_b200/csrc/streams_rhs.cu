@@ -1,0 +1,486 @@
+// a4-a8: the fused right-hand side + RK update.  One pass over the primitives produces, per
+// interior node, the convective terms in x, y, z (central split form, O1), the viscous
+// terms (O4) and the low-storage RK3 update (O5), so R is written once and w is updated in place
+// (stencils read the primitive copy q, never w, so no ping-pong buffer is needed).
+//
+//   rhs_main_kernel  : every node, central scheme; in hybrid mode nodes that touch a flagged
+//                      interface are left to
+//   rhs_shock_kernel : the compacted list of such nodes (or every node in full-WENO mode); each of
+//                      the node's six interfaces is WENO (O3) or central according to its flag.
+// Both kernels end in the same finish(): viscous combination, R store, w update.
+#include "streams_dev.cuh"
+#include "streams_launch.h"
+
+namespace streams {
+
+struct VAcc {          // velocity / temperature / viscosity / dilatation derivatives at a node
+  double g[3][3];      // g[a][b] = d u_a / d x_b
+  double gT[3], gmu[3], gdiv[3];
+  double lap[3], lapT;
+};
+
+template <int D>
+__device__ __forceinline__ double pick(double a, double b, double c) { return D == 0 ? a : (D == 1 ? b : c); }
+
+// ---------------------------------------------------------------------------------------------
+// One direction at one node.  Convective part in pair-difference form: with
+//   Pq(a,b) = (rho_a+rho_b)(ud_a+ud_b)(phi_a+phi_b)  the flux difference telescopes to
+//   f_{n+1/2} - f_{n-1/2} = 1/4 sum_l a_l [P(n, n+l) - P(n-l, n)]   (+ sum_l a_l (p_{n+l} - p_{n-l}))
+// which is the same sum as the oracle's interface-flux form (O1) in another order.
+// Viscous part: first derivatives of u, v, w, T, mu, div and second derivatives of u, v, w, T.
+// c0 = (rho, u, v, w, H, p) at the node.
+// ---------------------------------------------------------------------------------------------
+template <int D, int L, int LV, bool CONV, bool VISC>
+__device__ __forceinline__ void dir_terms(const DevP& P, long long n, long long s, double met_c, double met_v,
+                                          double eyy, const double c0[6], double T0, double r[5], VAcc& V) {
+  const double* __restrict__ RHO = P.q + Q_RHO * P.fs + n;
+  const double* __restrict__ U = P.q + Q_U * P.fs + n;
+  const double* __restrict__ Vv = P.q + Q_V * P.fs + n;
+  const double* __restrict__ W = P.q + Q_W * P.fs + n;
+  const double* __restrict__ Hh = P.q + Q_H * P.fs + n;
+  const double* __restrict__ Pp = P.q + Q_P * P.fs + n;
+  const double* __restrict__ Tt = P.q + Q_T * P.fs + n;
+  const double* __restrict__ Mu = P.q + Q_MU * P.fs + n;
+  const double* __restrict__ Dv = P.div + n;
+  constexpr int LC = CONV ? L : 0;
+  constexpr int LVV = VISC ? LV : 0;
+  constexpr int LM = LC > LVV ? LC : LVV;
+  double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, SP = 0.0;
+  double d1[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // u v w T mu div
+  double d2[4] = {0.0, 0.0, 0.0, 0.0};             // u v w T
+  const double ud0 = pick<D>(c0[1], c0[2], c0[3]);
+#pragma unroll
+  for (int l = 1; l <= LM; ++l) {
+    const long long off = l * s;
+    const double ub = U[off], ua = U[-off];
+    const double vb = Vv[off], va = Vv[-off];
+    const double wb = W[off], wa = W[-off];
+    if (l <= LC) {
+      const double rb = RHO[off], ra = RHO[-off];
+      const double hb = Hh[off], ha = Hh[-off];
+      const double pb = Pp[off], pa = Pp[-off];
+      const double mb = (c0[0] + rb) * (ud0 + pick<D>(ub, vb, wb));
+      const double ma = (ra + c0[0]) * (pick<D>(ua, va, wa) + ud0);
+      const double al = P.a1[l - 1];
+      S[0] += al * (mb - ma);
+      S[1] += al * (mb * (c0[1] + ub) - ma * (ua + c0[1]));
+      S[2] += al * (mb * (c0[2] + vb) - ma * (va + c0[2]));
+      S[3] += al * (mb * (c0[3] + wb) - ma * (wa + c0[3]));
+      S[4] += al * (mb * (c0[4] + hb) - ma * (ha + c0[4]));
+      SP += al * (pb - pa);
+    }
+    if (l <= LVV) {
+      const double tb = Tt[off], ta = Tt[-off];
+      const double a = P.a1v[l - 1], b = P.b2v[l - 1];
+      d1[0] += a * (ub - ua);  d2[0] += b * ((ub - 2.0 * c0[1]) + ua);
+      d1[1] += a * (vb - va);  d2[1] += b * ((vb - 2.0 * c0[2]) + va);
+      d1[2] += a * (wb - wa);  d2[2] += b * ((wb - 2.0 * c0[3]) + wa);
+      d1[3] += a * (tb - ta);  d2[3] += b * ((tb - 2.0 * T0) + ta);
+      d1[4] += a * (Mu[off] - Mu[-off]);
+      d1[5] += a * (Dv[off] - Dv[-off]);
+    }
+  }
+  if (CONV) {
+    r[0] -= met_c * (0.5 * S[0]);
+    r[1] -= met_c * (0.25 * S[1]);
+    r[2] -= met_c * (0.25 * S[2]);
+    r[3] -= met_c * (0.25 * S[3]);
+    r[4] -= met_c * (0.25 * S[4]);
+    r[1 + D] -= met_c * SP;
+  }
+  if (VISC) {
+    const double m2 = met_v * met_v;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      V.g[a][D] = d1[a] * met_v;
+      double sec = d2[a] * m2;
+      if (D == 1) sec += eyy * d1[a];
+      V.lap[a] += sec;
+    }
+    V.gT[D] = d1[3] * met_v;
+    double secT = d2[3] * m2;
+    if (D == 1) secT += eyy * d1[3];
+    V.lapT += secT;
+    V.gmu[D] = d1[4] * met_v;
+    V.gdiv[D] = d1[5] * met_v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Viscous combination (O4), R store and RK update (O5) for one node.
+// ---------------------------------------------------------------------------------------------
+template <bool VISC>
+__device__ __forceinline__ void finish(const DevP& P, const StageArgs& sa, long long n, long long o,
+                                       const double c0[6], double mu0, double r[5], const VAcc& V) {
+  if (VISC) {
+    const double dv = (V.g[0][0] + V.g[1][1]) + V.g[2][2];
+    double vm[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      double cross = 0.0;
+#pragma unroll
+      for (int b = 0; b < 3; ++b) cross += V.gmu[b] * (V.g[a][b] + V.g[b][a]);
+      vm[a] = mu0 * V.lap[a] + cross - (2.0 / 3.0) * V.gmu[a] * dv + mu0 * V.gdiv[a] * (1.0 / 3.0);
+    }
+    const double s01 = V.g[0][1] + V.g[1][0], s02 = V.g[0][2] + V.g[2][0], s12 = V.g[1][2] + V.g[2][1];
+    const double phi = mu0 * (2.0 * (V.g[0][0] * V.g[0][0] + V.g[1][1] * V.g[1][1] + V.g[2][2] * V.g[2][2]) +
+                              s01 * s01 + s02 * s02 + s12 * s12 - (2.0 / 3.0) * dv * dv);
+    const double cond = P.kfac * (mu0 * V.lapT + (V.gmu[0] * V.gT[0] + V.gmu[1] * V.gT[1] + V.gmu[2] * V.gT[2]));
+    r[1] += vm[0];
+    r[2] += vm[1];
+    r[3] += vm[2];
+    r[4] += (c0[1] * vm[0] + c0[2] * vm[1] + c0[3] * vm[2]) + phi + cond;
+  }
+  if (sa.update_w) {
+    const double dt = P.scal[S_DT];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      double inc = sa.gam * r[q];
+      if (sa.read_prev) inc += sa.rhk * P.R[q * P.N + o];
+      double* wp = P.w + q * P.fs + n;
+      *wp = *wp + dt * inc;
+    }
+  }
+  if (sa.write_r) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) sa.r_out[q * P.N + o] = r[q];
+  }
+}
+
+__device__ __forceinline__ void load_centre(const DevP& P, long long n, double c0[6]) {
+  c0[0] = P.q[Q_RHO * P.fs + n];
+  c0[1] = P.q[Q_U * P.fs + n];
+  c0[2] = P.q[Q_V * P.fs + n];
+  c0[3] = P.q[Q_W * P.fs + n];
+  c0[4] = P.q[Q_H * P.fs + n];
+  c0[5] = P.q[Q_P * P.fs + n];
+}
+
+__device__ __forceinline__ void zero_vacc(VAcc& V) {
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    V.lap[a] = 0.0; V.gT[a] = 0.0; V.gmu[a] = 0.0; V.gdiv[a] = 0.0;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) V.g[a][b] = 0.0;
+  }
+  V.lapT = 0.0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// rhs_main_kernel: BX x BY x BZ nodes per block.  Blocks are numbered so that a slab of `slab`
+// block-rows in y is swept through all of z before the next slab starts: the 2 ng z-neighbour
+// planes of a slab then stay in L2.
+// ---------------------------------------------------------------------------------------------
+template <int L, int LV, bool VISC, bool HYB, int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX * BY * BZ) rhs_main_kernel(const DevP P, const StageArgs sa, int nbx, int nby,
+                                                               int nbz, int slab) {
+  // decode block id -> (bx, by, bz), slab-major
+  long long bid = blockIdx.x;
+  const long long per_slab = (long long)nbx * slab * nbz;
+  const int sl = (int)(bid / per_slab);
+  const int rows = min(slab, nby - sl * slab);
+  bid -= (long long)sl * per_slab;
+  // inside a slab: x fastest, then y (rows of this slab), then z
+  const int bx = (int)(bid % nbx);
+  const long long t = bid / nbx;
+  const int byl = (int)(t % rows);
+  const int bz = (int)(t / rows);
+  if (bz >= nbz) return;
+  const int tx = threadIdx.x % BX, ty = (threadIdx.x / BX) % BY, tz = threadIdx.x / (BX * BY);
+  const int i = bx * BX + tx, j = (sl * slab + byl) * BY + ty, k = bz * BZ + tz;
+  if (i >= P.nx || j >= P.ny || k >= P.nz) return;
+  const long long o = iidx(P, i, j, k);
+  if (HYB) { if (P.nflag[o]) return; }
+  const long long n = pidx(P, i, j, k);
+  double c0[6];
+  load_centre(P, n, c0);
+  double T0 = 0.0, mu0 = 0.0, eyv = 0.0, eyy = 0.0;
+  if (VISC) { T0 = P.q[Q_T * P.fs + n]; mu0 = P.q[Q_MU * P.fs + n]; eyv = P.eta_y_v[j]; eyy = P.eta_yy_v[j]; }
+  double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  VAcc V;
+  zero_vacc(V);
+  dir_terms<0, L, LV, true, VISC>(P, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
+  dir_terms<1, L, LV, true, VISC>(P, n, P.sy, P.eta_y_c[j], eyv, eyy, c0, T0, r, V);
+  dir_terms<2, L, LV, true, VISC>(P, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
+  finish<VISC>(P, sa, n, o, c0, mu0, r, V);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Central interface flux, full form (O1), used next to WENO interfaces.
+// ---------------------------------------------------------------------------------------------
+template <int D, int L>
+__device__ __forceinline__ void central_flux(const DevP& P, long long n, long long s, double f[5]) {
+  const double* __restrict__ RHO = P.q + Q_RHO * P.fs;
+  const double* __restrict__ U = P.q + Q_U * P.fs;
+  const double* __restrict__ Vv = P.q + Q_V * P.fs;
+  const double* __restrict__ W = P.q + Q_W * P.fs;
+  const double* __restrict__ Hh = P.q + Q_H * P.fs;
+  const double* __restrict__ Pp = P.q + Q_P * P.fs;
+  const double* __restrict__ UD = D == 0 ? U : (D == 1 ? Vv : W);
+  double fs[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ps = 0.0;
+#pragma unroll
+  for (int l = 1; l <= L; ++l) {
+    double in[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, pin = 0.0;
+#pragma unroll
+    for (int m = 0; m < l; ++m) {
+      const long long a = n - m * s, b = a + l * s;
+      const double ru = (RHO[a] + RHO[b]) * (UD[a] + UD[b]);
+      in[0] += ru * 2.0;
+      in[1] += ru * (U[a] + U[b]);
+      in[2] += ru * (Vv[a] + Vv[b]);
+      in[3] += ru * (W[a] + W[b]);
+      in[4] += ru * (Hh[a] + Hh[b]);
+      pin += Pp[a] + Pp[b];
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) fs[q] += P.a1[l - 1] * in[q];
+    ps += P.a1[l - 1] * pin;
+  }
+#pragma unroll
+  for (int q = 0; q < 5; ++q) f[q] = 0.25 * fs[q];
+  f[1 + D] += ps;
+}
+
+// ---------------------------------------------------------------------------------------------
+// WENO reconstruction of order 2R-1 with Jiang-Shu weights (O3 step 4); v[0..2R-2] upwind->downwind,
+// value at the interface between v[R-1] and v[R].
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double sq(double x) { return x * x; }
+
+template <int R>
+__device__ __forceinline__ double weno_rec(const double* v, double eps);
+
+template <>
+__device__ __forceinline__ double weno_rec<1>(const double* v, double) { return v[0]; }
+
+template <>
+__device__ __forceinline__ double weno_rec<2>(const double* v, double eps) {
+  const double q0 = 0.5 * (3.0 * v[1] - v[0]), q1 = 0.5 * (v[1] + v[2]);
+  const double a0 = (1.0 / 3.0) / sq(eps + sq(v[1] - v[0]));
+  const double a1 = (2.0 / 3.0) / sq(eps + sq(v[2] - v[1]));
+  return (a0 * q0 + a1 * q1) / (a0 + a1);
+}
+
+template <>
+__device__ __forceinline__ double weno_rec<3>(const double* v, double eps) {
+  const double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) * (1.0 / 6.0);
+  const double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) * (1.0 / 6.0);
+  const double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) * (1.0 / 6.0);
+  const double b0 = (13.0 / 12.0) * sq(v[0] - 2.0 * v[1] + v[2]) + 0.25 * sq(v[0] - 4.0 * v[1] + 3.0 * v[2]);
+  const double b1 = (13.0 / 12.0) * sq(v[1] - 2.0 * v[2] + v[3]) + 0.25 * sq(v[1] - v[3]);
+  const double b2 = (13.0 / 12.0) * sq(v[2] - 2.0 * v[3] + v[4]) + 0.25 * sq(3.0 * v[2] - 4.0 * v[3] + v[4]);
+  const double a0 = 0.1 / sq(eps + b0), a1 = 0.6 / sq(eps + b1), a2 = 0.3 / sq(eps + b2);
+  return (a0 * q0 + a1 * q1 + a2 * q2) / ((a0 + a1) + a2);
+}
+
+template <>
+__device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
+  const double q0 = (-3.0 * v[0] + 13.0 * v[1] - 23.0 * v[2] + 25.0 * v[3]) * (1.0 / 12.0);
+  const double q1 = (v[1] - 5.0 * v[2] + 13.0 * v[3] + 3.0 * v[4]) * (1.0 / 12.0);
+  const double q2 = (-v[2] + 7.0 * v[3] + 7.0 * v[4] - v[5]) * (1.0 / 12.0);
+  const double q3 = (3.0 * v[3] + 13.0 * v[4] - 5.0 * v[5] + v[6]) * (1.0 / 12.0);
+  const double k = 1.0 / 240.0;
+  const double b0 = k * (v[0] * (547.0 * v[0] - 3882.0 * v[1] + 4642.0 * v[2] - 1854.0 * v[3]) +
+                         v[1] * (7043.0 * v[1] - 17246.0 * v[2] + 7042.0 * v[3]) +
+                         v[2] * (11003.0 * v[2] - 9402.0 * v[3]) + 2107.0 * v[3] * v[3]);
+  const double b1 = k * (v[1] * (267.0 * v[1] - 1642.0 * v[2] + 1602.0 * v[3] - 494.0 * v[4]) +
+                         v[2] * (2843.0 * v[2] - 5966.0 * v[3] + 1922.0 * v[4]) +
+                         v[3] * (3443.0 * v[3] - 2522.0 * v[4]) + 547.0 * v[4] * v[4]);
+  const double b2 = k * (v[2] * (547.0 * v[2] - 2522.0 * v[3] + 1922.0 * v[4] - 494.0 * v[5]) +
+                         v[3] * (3443.0 * v[3] - 5966.0 * v[4] + 1602.0 * v[5]) +
+                         v[4] * (2843.0 * v[4] - 1642.0 * v[5]) + 267.0 * v[5] * v[5]);
+  const double b3 = k * (v[3] * (2107.0 * v[3] - 9402.0 * v[4] + 7042.0 * v[5] - 1854.0 * v[6]) +
+                         v[4] * (11003.0 * v[4] - 17246.0 * v[5] + 4642.0 * v[6]) +
+                         v[5] * (7043.0 * v[5] - 3882.0 * v[6]) + 547.0 * v[6] * v[6]);
+  const double a0 = (1.0 / 35.0) / sq(eps + b0), a1 = (12.0 / 35.0) / sq(eps + b1);
+  const double a2 = (18.0 / 35.0) / sq(eps + b2), a3 = (4.0 / 35.0) / sq(eps + b3);
+  return (a0 * q0 + a1 * q1 + a2 * q2 + a3 * q3) / (((a0 + a1) + a2) + a3);
+}
+
+// ---------------------------------------------------------------------------------------------
+// WENO characteristic flux at interface n+1/2 along D (O3).  Characteristic projections are formed
+// from primitives: l.W = rho (l0 + l1 u + l2 v + l3 w + l4 H) - l4 p and
+// l.F = u_D (l.W) + p (l_{1+D} + l4 u_D), since F = u_D W + p (0, e_D, u_D).  One characteristic
+// field at a time (5 x 2 reconstructions), so only the 2R stencil primitives stay in registers.
+// ---------------------------------------------------------------------------------------------
+template <int D, int R>
+__device__ __forceinline__ void weno_flux(const DevP& P, long long n, long long s, double f[5]) {
+  constexpr int NS = 2 * R;
+  double rho[NS], vel[3][NS], H[NS], p[NS], c[NS];
+#pragma unroll
+  for (int m = 0; m < NS; ++m) {
+    const long long a = n + (long long)(m - R + 1) * s;
+    rho[m] = P.q[Q_RHO * P.fs + a];
+    vel[0][m] = P.q[Q_U * P.fs + a];
+    vel[1][m] = P.q[Q_V * P.fs + a];
+    vel[2][m] = P.q[Q_W * P.fs + a];
+    H[m] = P.q[Q_H * P.fs + a];
+    p[m] = P.q[Q_P * P.fs + a];
+    c[m] = P.q[Q_C * P.fs + a];
+  }
+  // Roe average of nodes n (slot R-1) and n+1 (slot R)
+  const double rw = sqrt(rho[R] / rho[R - 1]);
+  const double iden = 1.0 / (1.0 + rw);
+  double vb[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) vb[a] = (vel[a][R - 1] + rw * vel[a][R]) * iden;
+  const double Hb = (H[R - 1] + rw * H[R]) * iden;
+  const double qq = 0.5 * (vb[0] * vb[0] + vb[1] * vb[1] + vb[2] * vb[2]);
+  const double c2 = P.gm1 * (Hb - qq);
+  const double cb = sqrt(c2);
+  const double b1 = P.gm1 / c2, b2 = qq * b1;
+  const double un = vb[D], ic = 1.0 / cb;
+  constexpr int T1 = (D == 0) ? 1 : 0;
+  constexpr int T2 = (D == 2) ? 1 : 2;
+  double lam_m = 0.0, lam_0 = 0.0, lam_p = 0.0;
+#pragma unroll
+  for (int m = 0; m < NS; ++m) {
+    lam_m = fmax(lam_m, fabs(vel[D][m] - c[m]));
+    lam_0 = fmax(lam_0, fabs(vel[D][m]));
+    lam_p = fmax(lam_p, fabs(vel[D][m] + c[m]));
+  }
+#pragma unroll
+  for (int q = 0; q < 5; ++q) f[q] = 0.0;
+#pragma unroll
+  for (int sc = 0; sc < 5; ++sc) {
+    double l0, lv[3], l4, lam;
+    if (sc == 0 || sc == 4) {
+      const double sg = (sc == 0) ? 1.0 : -1.0;
+      l0 = 0.5 * (b2 + sg * un * ic);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) lv[a] = 0.5 * (-b1 * vb[a] - (a == D ? sg * ic : 0.0));
+      l4 = 0.5 * b1;
+      lam = (sc == 0) ? lam_m : lam_p;
+    } else if (sc == 1) {
+      l0 = 1.0 - b2;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) lv[a] = b1 * vb[a];
+      l4 = -b1;
+      lam = lam_0;
+    } else {
+      const int t = (sc == 2) ? T1 : T2;
+      l0 = -vb[t];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) lv[a] = (a == t) ? 1.0 : 0.0;
+      l4 = 0.0;
+      lam = lam_0;
+    }
+    double gp[NS], gm[NS];
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      const double lw = rho[m] * (l0 + lv[0] * vel[0][m] + lv[1] * vel[1][m] + lv[2] * vel[2][m] + l4 * H[m]) - l4 * p[m];
+      const double lf = vel[D][m] * lw + p[m] * (lv[D] + l4 * vel[D][m]);
+      gp[m] = 0.5 * (lf + lam * lw);
+      gm[NS - 1 - m] = 0.5 * (lf - lam * lw);      // mirrored: gm[0] is node n+R
+    }
+    const double gh = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+    // right eigenvector of this field
+    if (sc == 0 || sc == 4) {
+      const double sg = (sc == 0) ? -1.0 : 1.0;
+      f[0] += gh;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) f[1 + a] += gh * (vb[a] + (a == D ? sg * cb : 0.0));
+      f[4] += gh * (Hb + sg * un * cb);
+    } else if (sc == 1) {
+      f[0] += gh;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) f[1 + a] += gh * vb[a];
+      f[4] += gh * qq;
+    } else {
+      const int t = (sc == 2) ? T1 : T2;
+      f[1 + t] += gh;
+      f[4] += gh * vb[t];
+    }
+  }
+}
+
+// One direction of a shock node: both adjacent interfaces central -> pair-difference form, else
+// interface fluxes one by one.
+template <int D, int L, int LV, int R, bool VISC>
+__device__ __forceinline__ void shock_dir(const DevP& P, unsigned fl, long long n, long long s, double met_c,
+                                          double met_v, double eyy, const double c0[6], double T0, double r[5],
+                                          VAcc& V) {
+  if (fl == 0) {
+    dir_terms<D, L, LV, true, VISC>(P, n, s, met_c, met_v, eyy, c0, T0, r, V);
+    return;
+  }
+  if (VISC) dir_terms<D, L, LV, false, true>(P, n, s, met_c, met_v, eyy, c0, T0, r, V);
+  double fp[5], fm[5];
+  if (fl & 2u) weno_flux<D, R>(P, n, s, fp); else central_flux<D, L>(P, n, s, fp);
+  if (fl & 1u) weno_flux<D, R>(P, n - s, s, fm); else central_flux<D, L>(P, n - s, s, fm);
+#pragma unroll
+  for (int q = 0; q < 5; ++q) r[q] -= (fp[q] - fm[q]) * met_c;
+}
+
+template <int L, int LV, int R, bool VISC, bool DENSE>
+__global__ void __launch_bounds__(128) rhs_shock_kernel(const DevP P, const StageArgs sa) {
+  const long long count = DENSE ? P.N : (long long)P.counters[0];
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += (long long)gridDim.x * blockDim.x) {
+    const long long o = DENSE ? t : (long long)P.list[t];
+    const unsigned fl = DENSE ? 0x3fu : (unsigned)P.nflag[o];
+    const int i = (int)(o % P.nx);
+    const long long t2 = o / P.nx;
+    const int j = (int)(t2 % P.ny), k = (int)(t2 / P.ny);
+    const long long n = pidx(P, i, j, k);
+    double c0[6];
+    load_centre(P, n, c0);
+    double T0 = 0.0, mu0 = 0.0, eyv = 0.0, eyy = 0.0;
+    if (VISC) { T0 = P.q[Q_T * P.fs + n]; mu0 = P.q[Q_MU * P.fs + n]; eyv = P.eta_y_v[j]; eyy = P.eta_yy_v[j]; }
+    double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    VAcc V;
+    zero_vacc(V);
+    shock_dir<0, L, LV, R, VISC>(P, fl & 3u, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
+    shock_dir<1, L, LV, R, VISC>(P, (fl >> 2) & 3u, n, P.sy, P.eta_y_c[j], eyv, eyy, c0, T0, r, V);
+    shock_dir<2, L, LV, R, VISC>(P, (fl >> 4) & 3u, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
+    finish<VISC>(P, sa, n, o, c0, mu0, r, V);
+  }
+}
+
+// -------------------------------------------------------------------------- launch
+constexpr int MBX = 32, MBY = 4, MBZ = 4;
+
+template <int L, int LV, int R>
+static int launch_rhs_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+  const bool visc = P.visc_law != VISC_NONE;
+  int launches = 0;
+  if (P.flux_mode != FLUX_WENO) {
+    const int nbx = (P.nx + MBX - 1) / MBX, nby = (P.ny + MBY - 1) / MBY, nbz = (P.nz + MBZ - 1) / MBZ;
+    int slab = 8;                                  // 8 block rows = 32 grid rows per slab
+    if (slab > nby) slab = nby;
+    const int nslab = (nby + slab - 1) / slab;
+    const long long nblocks = (long long)nslab * nbx * slab * nbz;
+    dim3 b(MBX * MBY * MBZ), g((unsigned)nblocks);
+    const bool hyb = P.flux_mode == FLUX_HYBRID;
+    if (visc && hyb) rhs_main_kernel<L, LV, true, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+    else if (visc) rhs_main_kernel<L, LV, true, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+    else if (hyb) rhs_main_kernel<L, LV, false, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+    else rhs_main_kernel<L, LV, false, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+    ++launches;
+  }
+  if (P.flux_mode == FLUX_HYBRID) {
+    dim3 b(128), g(148 * 8);
+    if (visc) rhs_shock_kernel<L, LV, R, true, false><<<g, b, 0, st>>>(P, sa);
+    else rhs_shock_kernel<L, LV, R, false, false><<<g, b, 0, st>>>(P, sa);
+    ++launches;
+  } else if (P.flux_mode == FLUX_WENO) {
+    const long long nb = (P.N + 127) / 128;
+    dim3 b(128), g((unsigned)nb);
+    if (visc) rhs_shock_kernel<L, LV, R, true, true><<<g, b, 0, st>>>(P, sa);
+    else rhs_shock_kernel<L, LV, R, false, true><<<g, b, 0, st>>>(P, sa);
+    ++launches;
+  }
+  return launches;
+}
+
+bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
+  const int lv = visc_law == VISC_NONE ? 3 : Lv;
+  const int rr = flux_mode == FLUX_CENTRAL ? 3 : r;
+  return L == 3 && lv == 3 && rr == 3;
+}
+
+int launch_rhs(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
+  if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
+  return launch_rhs_T<3, 3, 3>(P, sa, st);
+}
+
+}  // namespace streams

@@ -1,0 +1,131 @@
+"""GPU-vs-oracle parity through the C ABI (BASELINE north_star tolerances):
+max field-normalised error <= 1e-11 after one RHS, <= 1e-9 after 10 RK steps, bit-identical mask."""
+import numpy as np
+import pytest
+
+import workloads as W
+from tests.helpers import field_err, natural_scales
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS = 1e-11
+TOL_STEP = 1e-9
+
+
+@pytest.fixture(scope="module")
+def S():
+    from paper_2304_05494_b200 import build, binding
+    build.build()
+    return binding.Streams
+
+
+def _oracle(case):
+    from oracle.oracle import Oracle
+    return Oracle(case)
+
+
+def check_case(S, case, nsteps, tol_rhs=TOL_RHS, tol_step=TOL_STEP, expect_activation=None):
+    gpu = S(case)
+    ora = _oracle(case)
+    floor_w, floor_r = natural_scales(case)
+    # one RHS
+    r_gpu = gpu.rhs().cpu().numpy()
+    r_ora = ora.rhs()
+    errs = [field_err(r_gpu[q], r_ora[q], floor_r[q]) for q in range(5)]
+    assert max(errs) <= tol_rhs, ("rhs", case.name, errs)
+    # streams_rhs must not change the interior
+    assert np.array_equal(gpu.get_fields(), case.w0)
+    # sensor mask, bit-identical
+    if case.flux_mode == W.FLUX_HYBRID:
+        th_g, mk_g = gpu.get_sensor()
+        th_o, mk_o, _ = ora.sensor()
+        assert np.array_equal(th_g, th_o), ("theta", float(np.max(np.abs(th_g - th_o))))
+        assert np.array_equal(mk_g, mk_o)
+        frac = float(mk_o.mean())
+        if expect_activation is not None:
+            assert expect_activation[0] <= frac <= expect_activation[1], frac
+        flagged, shock = gpu.get_activation()
+        assert flagged == int(mk_o.sum())
+    # nsteps RK3 steps
+    dt_g, t_g = gpu.step(nsteps)
+    dt_o, t_o = ora.step(nsteps)
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o and abs(t_g - t_o) <= 1e-12 * t_o
+    w_g, w_o = gpu.get_fields(), ora.get_fields()
+    errs = [field_err(w_g[q], w_o[q], floor_w[q]) for q in range(5)]
+    assert max(errs) <= tol_step, ("step", case.name, errs)
+    # mask of the evolved state (S14): may differ only at nodes whose theta sits within 1e-10 of the
+    # threshold, because the two states now differ by round-off
+    if case.flux_mode == W.FLUX_HYBRID:
+        th_g, mk_g = gpu.get_sensor()
+        ora.rhs()
+        th_o, mk_o, _ = ora.sensor()
+        near = np.abs(th_o - case.sensor_threshold) < 1e-10
+        assert np.array_equal(mk_g[~near], mk_o[~near])
+        assert np.max(np.abs(th_g - th_o)) < 1e-9
+    gpu.destroy()
+    return errs
+
+
+def test_purely_solenoidal_start_then_shocklets_form(S):
+    """configs 1/4 as specified start solenoidal (theta = 0); the sensor wakes up as the flow evolves."""
+    case = W.isotropic_turbulence(nx=40, ny=40, nz=40, mach_t=0.8, k0=4.0, kmax=12, seed=4)
+    check_case(S, case, 10, expect_activation=(0.0, 0.05))
+
+
+def test_config0_taylor_green_full_size(S):
+    check_case(S, W.config(0), 10)
+
+
+@pytest.mark.parametrize("shape", [(40, 36, 33), (35, 67, 20)])
+def test_periodic_inviscid_central_ragged(S, shape):
+    case = W.isotropic_turbulence(nx=shape[0], ny=shape[1], nz=shape[2], mach_t=0.3, k0=3.0, kmax=8, seed=11,
+                                  flux_mode=W.FLUX_CENTRAL, viscous=False)
+    check_case(S, case, 10)
+
+
+def test_periodic_viscous_central(S):
+    case = W.isotropic_turbulence(nx=37, ny=34, nz=41, mach_t=0.3, k0=3.0, kmax=8, seed=12, flux_mode=W.FLUX_CENTRAL)
+    check_case(S, case, 10)
+
+
+def test_periodic_full_weno_inviscid(S):
+    case = W.isotropic_turbulence(nx=34, ny=33, nz=35, mach_t=0.5, k0=3.0, kmax=8, seed=13,
+                                  flux_mode=W.FLUX_WENO, viscous=False)
+    check_case(S, case, 10)
+
+
+def test_config1_replica_hybrid_viscous(S):
+    case = W.isotropic_turbulence(nx=48, ny=44, nz=41, mach_t=0.6, k0=4.0, kmax=12, seed=1, dilatational=0.5)
+    check_case(S, case, 10, expect_activation=(0.005, 0.6))
+
+
+def test_config2_replica_channel(S):
+    case = W.channel(48, 40, 36, seed=2)
+    check_case(S, case, 10)
+
+
+def test_config3_replica_boundary_layer(S):
+    case = W.boundary_layer(96, 40, 36, seed=3, nblobs=6)
+    check_case(S, case, 10, expect_activation=(0.0005, 0.5))
+
+
+def test_config4_replica(S):
+    case = W.isotropic_turbulence(nx=40, ny=40, nz=40, mach_t=0.8, k0=8.0, kmax=16, seed=4, dilatational=0.3)
+    check_case(S, case, 10, expect_activation=(0.01, 0.8))
+
+
+def test_state_errors(S):
+    from paper_2304_05494_b200 import binding
+    case = W.config(0)
+    gpu = S(case.replace(w0=None))
+    with pytest.raises(binding.StreamsError) as e:
+        gpu.rhs()
+    assert e.value.code == binding.STREAMS_ESTATE
+    with pytest.raises(binding.StreamsError):
+        gpu.step(1)
+    bad = case.w0.copy()
+    bad[0, 3, 3, 3] = np.nan
+    gpu.set_fields(bad)
+    with pytest.raises(binding.StreamsError) as e:
+        gpu.step(1)
+    assert e.value.code == binding.STREAMS_ENAN

@@ -119,9 +119,11 @@ def taylor_green(n: int = 32, nsteps: int = 10, mach: float = 0.1) -> Case:
 # ----------------------------------------------------------------------------------------
 # random band-limited solenoidal velocity, E(k) ~ k^4 exp(-2 (k/k0)^2)
 # ----------------------------------------------------------------------------------------
-def solenoidal_velocity(nx, ny, nz, k0, kmax, seed):
+def solenoidal_velocity(nx, ny, nz, k0, kmax, seed, dilatational=0.0):
     """Real solenoidal field on [0,2pi)^3 from Gaussian Fourier coefficients on integer
-    wavevectors |k| <= kmax projected perpendicular to k, amplitude ~ sqrt(E(k))/k."""
+    wavevectors |k| <= kmax projected perpendicular to k, amplitude ~ sqrt(E(k))/k.
+    dilatational > 0 keeps that fraction of the component along k (parity tests use it so that the
+    shock sensor fires at step 0; the BASELINE configs are purely solenoidal)."""
     import scipy.fft as sfft
     rng = np.random.default_rng(seed)
     K = int(min(kmax, nx // 2 - 1, ny // 2 - 1, nz // 2 - 1))
@@ -136,6 +138,7 @@ def solenoidal_velocity(nx, ny, nz, k0, kmax, seed):
     c = [(rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) * amp for _ in range(3)]
     ksq = np.where(inside, kmag * kmag, 1.0)
     kdotc = (KX * c[0] + KY * c[1] + KZ * c[2]) / ksq
+    kdotc = (1.0 - dilatational) * kdotc
     c = [c[0] - KX * kdotc, c[1] - KY * kdotc, c[2] - KZ * kdotc]
     out = []
     for comp in c:
@@ -154,7 +157,7 @@ def solenoidal_velocity(nx, ny, nz, k0, kmax, seed):
 
 def isotropic_turbulence(n=128, mach_t=0.6, k0=4.0, kmax=32, seed=1, nsteps=50,
                          re_lambda=100.0, flux_mode=FLUX_HYBRID, viscous=True,
-                         nx=None, ny=None, nz=None, name=None) -> Case:
+                         nx=None, ny=None, nz=None, name=None, dilatational=0.0) -> Case:
     """configs 1 and 4: decaying compressible isotropic turbulence in a periodic box."""
     nx = nx or n
     ny = ny or n
@@ -162,7 +165,7 @@ def isotropic_turbulence(n=128, mach_t=0.6, k0=4.0, kmax=32, seed=1, nsteps=50,
     gamma = 1.4
     c0 = math.sqrt(gamma)           # rho0 = T0 = R = 1
     two_pi = 2.0 * math.pi
-    u, v, w = solenoidal_velocity(nx, ny, nz, k0, kmax, seed)
+    u, v, w = solenoidal_velocity(nx, ny, nz, k0, kmax, seed, dilatational)
     rms = math.sqrt(float(np.mean(u * u + v * v + w * w)))
     scale = mach_t * c0 / rms
     u *= scale
