@@ -1,0 +1,393 @@
+"""bench.py -- throughput of the STREAmS-2 hot path (RHS + RK3) on B200, in grid-point RK-step updates/s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one full low-storage RK3 step of the whole hot path over the whole grid: 3 x (ghost fill +
+primitives, sensor/mask, interface flags, fused convective x/y/z + viscous RHS + RK update) and the dt
+reduction.  value = grid points x K / device time of streams_step(K)
+(= 1e8 / the paper's "grind time").  The workload is BASELINE.json configs[1] (128^3 decaying
+compressible isotropic turbulence, hybrid WENO, Sutherland viscosity) unless --config says otherwise.
+N > 1: the path is single-GPU by design (north_star); ranks run independent replicas with different
+seeds and no data-path collective ("replicas only"), value = sum over ranks / max time.
+
+One JSON line on stdout from rank 0; keys as the driver's contract plus `roofline` and `cpu_baseline`.
+`--impl reference` times the CPU oracle (oracle/, the only "reference" that exists for this paper) on the
+host cores on the same workload and prints the same line with "impl": "reference".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as W  # noqa: E402
+
+METRIC = "fp64 grid-point RK-step updates/sec"
+UNIT = "point-steps/s"
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written); fallback per B200_PROFILING.md."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def make_case(index: int, seed_offset: int = 0):
+    """BASELINE.json configs[index] with the rank's seed (replicas differ only by seed)."""
+    if index == 0:
+        return W.config(0)
+    if index == 1:
+        return W.isotropic_turbulence(n=128, mach_t=0.6, k0=4.0, kmax=32, seed=1 + 100 * seed_offset, nsteps=50,
+                                      name="cfg1_iso_128")
+    if index == 2:
+        return W.channel(256, 192, 128, seed=2 + 100 * seed_offset, nsteps=50)
+    if index == 3:
+        return W.boundary_layer(1024, 256, 256, seed=3 + 100 * seed_offset, nsteps=20)
+    if index == 4:
+        return W.isotropic_turbulence(n=640, mach_t=0.8, k0=8.0, kmax=64, seed=4 + 100 * seed_offset, nsteps=10,
+                                      name="cfg4_iso_640")
+    raise SystemExit(f"unknown config {index}")
+
+
+WORKLOAD_TEXT = {
+    0: "configs[0]: inviscid Taylor-Green vortex 32^3 periodic, central L=3, CFL 0.5",
+    1: "configs[1]: viscous decaying compressible isotropic turbulence 128^3 periodic, Mach_t 0.6, k0=4, "
+       "Sutherland, Pr 0.72, hybrid WENO5/central6 thr 0.2",
+    2: "configs[2]: supersonic isothermal-wall channel 256x192x128, tanh-stretched y, hybrid",
+    3: "configs[3]: supersonic flat-plate boundary-layer box 1024x256x256, stretched y, hybrid, seeded shocklets",
+    4: "configs[4]: capacity run 640^3 periodic compressible turbulence Mach_t 0.8, k0=8, hybrid",
+}
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks line")
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes per launch of each kernel class
+# ------------------------------------------------------------------------------------------------
+def algorithmic_bytes(case, alpha_shock: float):
+    """Bytes the method itself must move per launch of each kernel class, averaged over the three RK
+    stages of a step: every input field read once, every output written once, no halo re-reads.
+    alpha_shock = fraction of interior nodes handled by the shock-capturing half."""
+    ng = 3
+    N = case.npoints
+    Np = (case.nx + 2 * ng) * (case.ny + 2 * ng) * (case.nz + 2 * ng)
+    visc = case.visc_law != W.VISC_NONE
+    hyb = case.flux_mode == W.FLUX_HYBRID
+    weno = case.flux_mode != W.FLUX_CENTRAL
+    nprim = 6 + (2 if visc else 0) + (1 if weno else 0)        # rho u v w H p [T mu] [c]
+    out = {}
+    out["fill_prim"] = Np * (40 + 8 * nprim) + (Np - N) * 40   # read w, write primitives, write ghost w
+    out["sensor"] = N * (24 + 8 + (1 if hyb else 0))           # read u v w, write div [mask]
+    out["flags"] = N * (1 + 1) + alpha_shock * N * 4           # read mask, write flags byte, append to list
+    # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
+    # read R_prev (stages 2, 3), write R (stages 1, 2)
+    per_point = 48 + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40
+    main_nodes = N * (1.0 - alpha_shock) if hyb else (0 if case.flux_mode == W.FLUX_WENO else N)
+    shock_nodes = alpha_shock * N if hyb else (N if case.flux_mode == W.FLUX_WENO else 0)
+    out["rhs_main"] = main_nodes * per_point + (N if hyb else 0)          # + the flags byte
+    out["rhs_shock"] = shock_nodes * (per_point + 8 + 1 + 4)             # + c, flags byte, list entry
+    out["dt"] = N * (40 + (8 if visc else 0))                            # rho p u v w [mu]
+    out["misc"] = 0
+    return out, per_point
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm = the oracle on the host cores
+# ------------------------------------------------------------------------------------------------
+def oracle_throughput(case, budget_s: float, max_steps: int):
+    """Times oracle RK3 steps of `case` (OpenMP build, as it stands) until budget_s is used or max_steps done."""
+    from oracle.oracle import Oracle, load
+    cores = int(load("omp").oracle_num_threads())
+    ora = Oracle(case, kind="omp")
+    done, t_used = 0, 0.0
+    while done < max_steps and (done == 0 or t_used < budget_s):
+        t0 = time.perf_counter()
+        ora.step(1)
+        t_used += time.perf_counter() - t0
+        done += 1
+    ora.close()
+    return case.npoints * done / t_used, cores, done, t_used
+
+
+def oracle_case_for(index: int):
+    """The reference arm's bounded sample: the full workload when an oracle RK3 step takes seconds
+    (configs 0-2), otherwise the same recipe on a grid cut to ~8 M points (CPU throughput per point does
+    not depend on the grid size beyond cache effects)."""
+    if index == 3:
+        return W.boundary_layer(512, 128, 128, seed=3, nsteps=20), "same recipe on 512x128x128 (1/8 of the points)"
+    if index == 4:
+        return (W.isotropic_turbulence(n=200, mach_t=0.8, k0=8.0, kmax=64, seed=4, nsteps=10, name="cfg4_iso_200"),
+                "same recipe on 200^3 (1/33 of the points)")
+    return make_case(index), "the full grid"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    case, what = oracle_case_for(args.config)
+    from oracle.oracle import Oracle, load
+    cores = int(load("omp").oracle_num_threads())
+    ora = Oracle(case, kind="omp")
+    for _ in range(args.warmup):
+        ora.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ora.step(1)
+    dt = time.perf_counter() - t0
+    value = case.npoints * args.steps / dt
+    sample = f"{args.steps} RK3 steps (3 RHS + update + dt each) of {what}, oracle OpenMP build"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_TEXT[args.config], "grid": [case.nx, case.ny, case.nz],
+                   "points": case.npoints, "sample": what, "device": "host CPU"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm: libstreams.so on the GPU through the C ABI
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2304_05494_b200 import binding, build as kbuild
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libstreams has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        kbuild.build()
+    if dist is not None:
+        dist.barrier()
+
+    case = make_case(args.config, seed_offset=rank)
+    N = case.npoints
+    gpu = binding.Streams(case, device=f"cuda:{local}")
+    dev = gpu.device
+    state_bytes = 5 * N * 8
+
+    def sync_all():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(ms: float) -> float:
+        if dist is None:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident throughput: inputs already in HBM, K steps in one streams_step call
+    for _ in range(args.warmup):
+        gpu.step(1)
+    gpu.profile(True, max_records=8 * 3 * args.steps + 64)
+    l0 = gpu.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sync_all()
+    clocks = ClockSampler(local) if rank == 0 else None
+    e0.record(gpu.stream)
+    gpu.step(args.steps)
+    e1.record(gpu.stream)
+    sync_all()
+    clk = clocks.stop() if clocks else None
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    launches = gpu.kernel_launches() - l0
+    prof, dropped = gpu.get_profile()
+    gpu.profile(False)
+    flagged_sum, shock_sum, evals = gpu.get_activation_totals()
+    alpha_shock = shock_sum / (evals * N) if evals else (1.0 if case.flux_mode == W.FLUX_WENO else 0.0)
+    alpha_nodes = flagged_sum / (evals * N) if evals else 0.0
+    value = world * N * args.steps / (ms * 1e-3)
+
+    # the same K steps with the event pairs off (how much the per-kernel timing costs)
+    sync_all()
+    e0.record(gpu.stream)
+    gpu.step(args.steps)
+    e1.record(gpu.stream)
+    sync_all()
+    ms_noprof = max_over_ranks(e0.elapsed_time(e1))
+
+    # ---- end to end through the C ABI with HOST buffers: h2d of the state, one step, d2h of the state
+    h_in = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
+    h_out = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
+    h_in.numpy()[...] = case.w0
+    n_e2e = max(3, min(args.steps, 20))
+    for _ in range(2):
+        gpu.set_fields(h_in.numpy()); gpu.step(1); gpu.get_fields(h_out.numpy())
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        gpu.set_fields(h_in.numpy())      # host -> device (synchronous on return)
+        gpu.step(1)
+        gpu.get_fields(h_out.numpy())     # device -> host (synchronous on return)
+    torch.cuda.synchronize(dev)
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+    e2e_value = world * N * n_e2e / (e2e_ms * 1e-3)
+    assert np.isfinite(h_out.numpy()).all()
+
+    if rank != 0:
+        gpu.destroy()
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- per-kernel roofline from the event pairs of the timed region
+    peak, peak_src = load_peaks()
+    abytes, per_point = algorithmic_bytes(case, alpha_shock)
+    kernels = {}
+    for name, (kms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        avg_ms = kms / cnt
+        gbs = abytes[name] / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
+        kernels[name] = {"launches": cnt, "avg_ms": avg_ms, "share": kms / ms, "alg_bytes": abytes[name],
+                         "gbs": gbs, "frac_hbm": gbs / peak}
+    dom = max(kernels, key=lambda k: kernels[k]["avg_ms"] * kernels[k]["launches"])
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac_hbm"], "traffic": None, "peak_source": peak_src,
+                "alg_bytes_per_point": per_point, "kernels": kernels, "events_dropped": dropped}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):           # dram bytes per launch from the committed ncu --set full capture
+        with open(traffic_file) as f:
+            tr = json.load(f)
+        key = f"cfg{args.config}:{dom}"
+        if key in tr:
+            roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
+            roofline["traffic_source"] = tr[key].get("source")
+
+    # ---- the oracle on this box's host cores (bounded sample, rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        ocase, what = oracle_case_for(args.config)
+        v, cores, done, used = oracle_throughput(ocase, budget_s=12.0, max_steps=args.steps)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{done} RK3 steps of {what} ({used:.1f} s), oracle OpenMP build as it stands"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_TEXT[args.config], "grid": [case.nx, case.ny, case.nz], "points": N,
+                   "orders": "central 6 / WENO 5 / viscous 6", "parallelism": "1 GPU" if world == 1 else
+                   f"{world} independent replicas (no data-path collective)",
+                   "l2": "inputs larger than L2 (workspace %.2f GB vs 126 MB)" % (gpu.workspace_bytes / 1e9)
+                   if gpu.workspace_bytes > 4 * 126e6 else "workspace %.1f MB is L2-resident; latency point, not a roofline point"
+                   % (gpu.workspace_bytes / 1e6),
+                   "weno_activation": {"flagged_nodes": alpha_nodes, "shock_kernel_nodes": alpha_shock}},
+        "clocks": clk,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
+                "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "point_stages_per_s": 3 * value,
+        "value_events_off": world * N * args.steps / (ms_noprof * 1e-3),
+        "paper_context": "A100 1.06e8 (central) / 7.05e7 (WENO) point-steps/s on 420x250x320, PAPER:398-404 (other hardware)",
+    }
+    print(json.dumps(line), flush=True)
+    gpu.destroy()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -116,8 +116,33 @@ int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_
  * number of nodes handled by the shock-capturing kernel (any adjacent interface flagged). */
 int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes);
 
+/* The same counts summed over every sensor evaluation since streams_set_fields (hybrid mode; zeros
+ * otherwise), and the number of evaluations: the paper's "WENO activation", which is
+ * "not known a priori and may even vary".  HOST outputs, nullable.  Synchronises the stream. */
+int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum,
+                                  long long* evaluations);
+
 /* Number of kernels the library has launched on this context since streams_init. */
 long long streams_kernel_launches(const streams_ctx* ctx);
+
+/* Per-kernel device timing, the measurement of BASELINE metric part 2 ("per-kernel % of roofline";
+ * the paper's analogue is its per-kernel table).  Kernel classes: */
+enum { STREAMS_K_FILL_PRIM = 0, STREAMS_K_DT = 1, STREAMS_K_SENSOR = 2, STREAMS_K_FLAGS = 3,
+       STREAMS_K_RHS_MAIN = 4, STREAMS_K_RHS_SHOCK = 5, STREAMS_K_MISC = 6, STREAMS_K_COUNT = 7 };
+
+/* enable != 0: from now on every launch is bracketed by a CUDA event pair on the context's stream
+ * (at most max_records launches between two streams_get_profile calls are recorded, the rest are
+ * counted as dropped; max_records <= 0 means 4096).  enable == 0: stop.  Either way the totals are
+ * reset.  Synchronises the stream. */
+int streams_profile(streams_ctx* ctx, int enable, int max_records);
+
+/* Totals since streams_profile: ms[STREAMS_K_COUNT] device milliseconds and count[STREAMS_K_COUNT]
+ * recorded launch groups per class, *dropped = launches not recorded.  HOST outputs, each nullable.
+ * Synchronises the stream. */
+int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long long* dropped);
+
+/* Name of a kernel class ("" if out of range); static storage. */
+const char* streams_kernel_name(int kind);
 
 /* Text of the last error on this context ("" if none); ctx may be NULL for init failures. */
 const char* streams_last_error(const streams_ctx* ctx);

@@ -16,8 +16,11 @@ LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
 
 STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
-           "streams_get_fields", "streams_get_sensor", "streams_get_activation", "streams_kernel_launches",
+           "streams_get_fields", "streams_get_sensor", "streams_get_activation", "streams_get_activation_totals",
+           "streams_kernel_launches",
+           "streams_profile", "streams_get_profile", "streams_kernel_name",
            "streams_last_error", "streams_destroy")
+STREAMS_K_COUNT = 7
 
 _dp = C.POINTER(C.c_double)
 
@@ -65,8 +68,13 @@ def load_library(path: str = LIB_PATH):
     lib.streams_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_activation.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    lib.streams_get_activation_totals.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 3
     lib.streams_kernel_launches.restype = C.c_longlong
     lib.streams_kernel_launches.argtypes = [C.c_void_p]
+    lib.streams_profile.argtypes = [C.c_void_p, C.c_int, C.c_int]
+    lib.streams_get_profile.argtypes = [C.c_void_p, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    lib.streams_kernel_name.restype = C.c_char_p
+    lib.streams_kernel_name.argtypes = [C.c_int]
     lib.streams_last_error.restype = C.c_char_p
     lib.streams_last_error.argtypes = [C.c_void_p]
     lib.streams_destroy.argtypes = [C.c_void_p]
@@ -182,8 +190,26 @@ class Streams:
         self._check(self.lib.streams_get_activation(self.h, C.byref(a), C.byref(b)))
         return a.value, b.value
 
+    def get_activation_totals(self):
+        """(flagged nodes, shock-kernel nodes, sensor evaluations) summed since set_fields."""
+        a, b, n = C.c_longlong(), C.c_longlong(), C.c_longlong()
+        self._check(self.lib.streams_get_activation_totals(self.h, C.byref(a), C.byref(b), C.byref(n)))
+        return a.value, b.value, n.value
+
     def kernel_launches(self):
         return int(self.lib.streams_kernel_launches(self.h))
+
+    def profile(self, enable=True, max_records=0):
+        self._check(self.lib.streams_profile(self.h, int(bool(enable)), int(max_records)))
+
+    def get_profile(self):
+        """{kernel class name: (device ms, recorded launch groups)}, and the number of unrecorded launches."""
+        ms = (C.c_double * STREAMS_K_COUNT)()
+        cnt = (C.c_longlong * STREAMS_K_COUNT)()
+        dropped = C.c_longlong()
+        self._check(self.lib.streams_get_profile(self.h, ms, cnt, C.byref(dropped)))
+        out = {self.lib.streams_kernel_name(k).decode(): (ms[k], cnt[k]) for k in range(STREAMS_K_COUNT)}
+        return out, dropped.value
 
     def destroy(self):
         if getattr(self, "h", None):

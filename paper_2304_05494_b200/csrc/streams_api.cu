@@ -113,6 +113,14 @@ struct streams_ctx {
   long long step_count;     // steps since set_fields (host mirror; decides when dt is recomputed)
   long long launches;
   char err[256];
+  // per-kernel device timing (streams_profile): event pairs recorded on the stream around each launch
+  bool prof_on;
+  std::vector<cudaEvent_t> prof_pool;             // 2 events per record
+  std::vector<int> prof_kind;                     // kernel class of record i
+  size_t prof_used;                               // records in flight
+  double prof_ms[STREAMS_K_COUNT];
+  long long prof_n[STREAMS_K_COUNT];
+  long long prof_dropped;
 };
 
 namespace {
@@ -175,16 +183,59 @@ void build_metrics(const streams_ctx* c, const double* y_nodes, std::vector<doub
   }
 }
 
+// Runs one launch wrapper; with profiling on, brackets it with an event pair on the stream.
+template <class F>
+int timed(streams_ctx* ctx, int kind, F&& launch) {
+  const bool rec = ctx->prof_on && 2 * (ctx->prof_used + 1) <= ctx->prof_pool.size();
+  if (ctx->prof_on && !rec) ctx->prof_dropped += 1;
+  if (rec) cudaEventRecord(ctx->prof_pool[2 * ctx->prof_used], ctx->stream);
+  const int n = launch();
+  if (rec) {
+    cudaEventRecord(ctx->prof_pool[2 * ctx->prof_used + 1], ctx->stream);
+    ctx->prof_kind[ctx->prof_used] = kind;
+    ctx->prof_used += 1;
+  }
+  if (n > 0) ctx->launches += n;
+  return n;
+}
+
+// Folds the finished event pairs into the per-class totals (synchronises the stream).
+cudaError_t prof_drain(streams_ctx* ctx) {
+  if (ctx->prof_used == 0) return cudaSuccess;
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return e;
+  for (size_t i = 0; i < ctx->prof_used; ++i) {
+    float ms = 0.f;
+    e = cudaEventElapsedTime(&ms, ctx->prof_pool[2 * i], ctx->prof_pool[2 * i + 1]);
+    if (e != cudaSuccess) return e;
+    ctx->prof_ms[ctx->prof_kind[i]] += ms;
+    ctx->prof_n[ctx->prof_kind[i]] += 1;
+  }
+  ctx->prof_used = 0;
+  return cudaSuccess;
+}
+
 // ghost fill + primitives (+ dt) + sensor + flags: everything a stage needs before the RHS kernels
 int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   const DevP& P = ctx->P;
-  ctx->launches += launch_fill_prim(P, ctx->stream);
-  if (want_dt) ctx->launches += launch_dt(P, ctx->scheme.dt_fixed, ctx->stream);
+  cudaStream_t st = ctx->stream;
+  timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, st); });
+  if (want_dt) timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, st); });
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
-  if (hyb || visc || theta) ctx->launches += launch_sensor(P, ctx->S.L, hyb || theta, theta, ctx->stream);
-  if (hyb) ctx->launches += launch_flags(P, ctx->S.r, ctx->stream);
+  if (hyb || visc || theta)
+    timed(ctx, STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->S.L, hyb || theta, theta, st); });
+  if (hyb) timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.r, st); });
   return STREAMS_OK;
+}
+
+// the fused RHS (+ update) of one stage: central/main half, then the shock-capturing half
+int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
+  const DevP& P = ctx->P;
+  cudaStream_t st = ctx->stream;
+  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
+  const int b = timed(ctx, STREAMS_K_RHS_SHOCK, [&] { return launch_rhs_shock(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
+  return (a < 0 || b < 0) ? -1 : a + b;
 }
 
 }  // namespace
@@ -216,6 +267,8 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->base = (char*)workspace_dev;
   ctx->have_fields = false; ctx->step_count = 0; ctx->launches = 0; ctx->err[0] = 0;
+  ctx->prof_on = false; ctx->prof_used = 0; ctx->prof_dropped = 0;
+  for (int k = 0; k < STREAMS_K_COUNT; ++k) { ctx->prof_ms[k] = 0.0; ctx->prof_n[k] = 0; }
   if (ctx->scheme.dt_every < 1) ctx->scheme.dt_every = 1;
   DevP& P = ctx->P;
   std::memset(&P, 0, sizeof P);
@@ -279,6 +332,7 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
     CU(cudaMemcpy3DAsync(&p, ctx->stream));
   }
   CU(cudaMemsetAsync(P.scal, 0, S_COUNT * 8, ctx->stream));
+  CU(cudaMemsetAsync(P.counters, 0, 256, ctx->stream));
   if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));   // the host buffer may be reused on return
   ctx->have_fields = true;
   ctx->step_count = 0;
@@ -311,9 +365,7 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   StageArgs sa;
   sa.gam = 0.0; sa.rhk = 0.0; sa.update_w = 0; sa.read_prev = 0; sa.write_r = 1;
   sa.r_out = rhs_out_dev ? rhs_out_dev : ctx->P.R;
-  const int n = launch_rhs(ctx->P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, ctx->stream);
-  if (n < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
-  ctx->launches += n;
+  if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
   CU(cudaGetLastError());
   return STREAMS_OK;
 }
@@ -332,11 +384,9 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
       StageArgs sa;
       sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
       sa.r_out = ctx->P.R;
-      const int n = launch_rhs(ctx->P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, ctx->stream);
-      if (n < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
-      ctx->launches += n;
+      if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
     }
-    ctx->launches += launch_step_end(ctx->P, ctx->stream);
+    timed(ctx, STREAMS_K_MISC, [&] { return launch_step_end(ctx->P, ctx->stream); });
     ctx->step_count += 1;
   }
   CU(cudaGetLastError());
@@ -354,8 +404,7 @@ int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
   if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
   const DevP& P = ctx->P;
-  ctx->launches += launch_fill_prim(P, ctx->stream);
-  ctx->launches += launch_sensor(P, ctx->S.L, true, true, ctx->stream);
+  enqueue_prepare(ctx, false, true);
   CU(cudaGetLastError());
   const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
   if (theta_out) CU(cudaMemcpyAsync(theta_out, P.theta, (size_t)P.N * 8, kind, ctx->stream));
@@ -387,13 +436,61 @@ int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long
   return STREAMS_OK;
 }
 
+int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum, long long* evaluations) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  unsigned long long h[3] = {0, 0, 0};
+  if (ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID) {
+    CU(cudaMemcpyAsync(h, ctx->P.counters + 4, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+  }
+  if (shock_sum) *shock_sum = (long long)h[0];
+  if (flagged_sum) *flagged_sum = (long long)h[1];
+  if (evaluations) *evaluations = (long long)h[2];
+  return STREAMS_OK;
+}
+
 long long streams_kernel_launches(const streams_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int streams_profile(streams_ctx* ctx, int enable, int max_records) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  CU(prof_drain(ctx));
+  for (int k = 0; k < STREAMS_K_COUNT; ++k) { ctx->prof_ms[k] = 0.0; ctx->prof_n[k] = 0; }
+  ctx->prof_dropped = 0;
+  ctx->prof_on = enable != 0;
+  if (enable) {
+    const size_t want = 2 * (size_t)(max_records > 0 ? max_records : 4096);
+    while (ctx->prof_pool.size() < want) {
+      cudaEvent_t ev;
+      CU(cudaEventCreate(&ev));
+      ctx->prof_pool.push_back(ev);
+    }
+    ctx->prof_kind.resize(ctx->prof_pool.size() / 2);
+  }
+  return STREAMS_OK;
+}
+
+int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long long* dropped) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  CU(prof_drain(ctx));
+  for (int k = 0; k < STREAMS_K_COUNT; ++k) {
+    if (ms) ms[k] = ctx->prof_ms[k];
+    if (count) count[k] = ctx->prof_n[k];
+  }
+  if (dropped) *dropped = ctx->prof_dropped;
+  return STREAMS_OK;
+}
+
+const char* streams_kernel_name(int kind) {
+  static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "rhs_shock", "misc"};
+  return (kind >= 0 && kind < STREAMS_K_COUNT) ? names[kind] : "";
+}
 
 const char* streams_last_error(const streams_ctx* ctx) { return ctx ? ctx->err : g_init_error; }
 
 int streams_destroy(streams_ctx* ctx) {
   if (!ctx) return STREAMS_EINVAL;
   cudaStreamSynchronize(ctx->stream);
+  for (cudaEvent_t ev : ctx->prof_pool) cudaEventDestroy(ev);
   delete ctx;
   return STREAMS_OK;
 }

@@ -204,8 +204,9 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
   const int lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31;
   int base = 0;
   if (lane == 0) {
-    if (ball) base = atomicAdd(&P.counters[0], __popc(ball));
-    if (ballm) atomicAdd(&P.counters[1], __popc(ballm));
+    unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + 4);   // totals since set_fields
+    if (ball) { base = atomicAdd(&P.counters[0], __popc(ball)); atomicAdd(&cum[0], (unsigned long long)__popc(ball)); }
+    if (ballm) { atomicAdd(&P.counters[1], __popc(ballm)); atomicAdd(&cum[1], (unsigned long long)__popc(ballm)); }
   }
   base = __shfl_sync(0xffffffffu, base, 0);
   if (f != 0) P.list[base + __popc(ball & ((1u << lane) - 1u))] = (int)o;
@@ -276,7 +277,11 @@ __global__ void step_end_kernel(const DevP P) {
   P.scal[S_NSTEP] = P.scal[S_NSTEP] + 1.0;
 }
 
-__global__ void reset_counters_kernel(const DevP P) { P.counters[0] = 0; P.counters[1] = 0; }
+__global__ void reset_counters_kernel(const DevP P) {
+  P.counters[0] = 0;
+  P.counters[1] = 0;
+  reinterpret_cast<unsigned long long*>(P.counters + 4)[2] += 1ull;     // sensor evaluations since set_fields
+}
 
 // -------------------------------------------------------------------------- launch wrappers
 static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }

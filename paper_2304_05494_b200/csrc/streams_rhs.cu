@@ -440,36 +440,40 @@ __global__ void __launch_bounds__(128) rhs_shock_kernel(const DevP P, const Stag
 constexpr int MBX = 32, MBY = 4, MBZ = 4;
 
 template <int L, int LV, int R>
-static int launch_rhs_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+  if (P.flux_mode == FLUX_WENO) return 0;
   const bool visc = P.visc_law != VISC_NONE;
-  int launches = 0;
-  if (P.flux_mode != FLUX_WENO) {
-    const int nbx = (P.nx + MBX - 1) / MBX, nby = (P.ny + MBY - 1) / MBY, nbz = (P.nz + MBZ - 1) / MBZ;
-    int slab = 8;                                  // 8 block rows = 32 grid rows per slab
-    if (slab > nby) slab = nby;
-    const int nslab = (nby + slab - 1) / slab;
-    const long long nblocks = (long long)nslab * nbx * slab * nbz;
-    dim3 b(MBX * MBY * MBZ), g((unsigned)nblocks);
-    const bool hyb = P.flux_mode == FLUX_HYBRID;
-    if (visc && hyb) rhs_main_kernel<L, LV, true, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
-    else if (visc) rhs_main_kernel<L, LV, true, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
-    else if (hyb) rhs_main_kernel<L, LV, false, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
-    else rhs_main_kernel<L, LV, false, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
-    ++launches;
-  }
+  const int nbx = (P.nx + MBX - 1) / MBX, nby = (P.ny + MBY - 1) / MBY, nbz = (P.nz + MBZ - 1) / MBZ;
+  int slab = 8;                                  // 8 block rows = 32 grid rows per slab
+  if (slab > nby) slab = nby;
+  const int nslab = (nby + slab - 1) / slab;
+  const long long nblocks = (long long)nslab * nbx * slab * nbz;
+  dim3 b(MBX * MBY * MBZ), g((unsigned)nblocks);
+  const bool hyb = P.flux_mode == FLUX_HYBRID;
+  if (visc && hyb) rhs_main_kernel<L, LV, true, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  else if (visc) rhs_main_kernel<L, LV, true, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  else if (hyb) rhs_main_kernel<L, LV, false, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  else rhs_main_kernel<L, LV, false, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  return 1;
+}
+
+template <int L, int LV, int R>
+static int launch_shock_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+  const bool visc = P.visc_law != VISC_NONE;
   if (P.flux_mode == FLUX_HYBRID) {
     dim3 b(128), g(148 * 8);
     if (visc) rhs_shock_kernel<L, LV, R, true, false><<<g, b, 0, st>>>(P, sa);
     else rhs_shock_kernel<L, LV, R, false, false><<<g, b, 0, st>>>(P, sa);
-    ++launches;
-  } else if (P.flux_mode == FLUX_WENO) {
+    return 1;
+  }
+  if (P.flux_mode == FLUX_WENO) {
     const long long nb = (P.N + 127) / 128;
     dim3 b(128), g((unsigned)nb);
     if (visc) rhs_shock_kernel<L, LV, R, true, true><<<g, b, 0, st>>>(P, sa);
     else rhs_shock_kernel<L, LV, R, false, true><<<g, b, 0, st>>>(P, sa);
-    ++launches;
+    return 1;
   }
-  return launches;
+  return 0;
 }
 
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
@@ -478,9 +482,13 @@ bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
   return L == 3 && lv == 3 && rr == 3;
 }
 
-int launch_rhs(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
+int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
-  return launch_rhs_T<3, 3, 3>(P, sa, st);
+  return launch_main_T<3, 3, 3>(P, sa, st);
+}
+int launch_rhs_shock(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
+  if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
+  return launch_shock_T<3, 3, 3>(P, sa, st);
 }
 
 }  // namespace streams
