@@ -129,31 +129,53 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # algorithmic bytes per launch of each kernel class
 # ------------------------------------------------------------------------------------------------
-def algorithmic_bytes(case, alpha_shock: float):
-    """Bytes the method itself must move per launch of each kernel class, averaged over the three RK
-    stages of a step: every input field read once, every output written once, no halo re-reads.
-    alpha_shock = fraction of interior nodes handled by the shock-capturing half."""
+# fp64 instructions per unit of work (thread-level DFMA + DADD + DMUL of the straight-line SASS of each
+# kernel, `cuobjdump -sass`, orders 6/5/6)
+FP64_INST = {"rhs_main_cv": 631, "rhs_main_c": 310, "rhs_main_v": 335, "rhs_main_0": 17,
+             "weno_hybrid": 1422, "weno_dense": 1320, "fill_prim": 289, "sensor": 144, "rhs_apply": 111, "dt": 90}
+FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
+
+
+def work_model(case, act):
+    """Per launch of each kernel class, averaged over the three RK stages of a step:
+    bytes = what the method must move (every input field read once, every output written once, no halo
+    re-reads), inst = fp64 thread-instructions.  act: mean fractions of N per sensor evaluation
+    {"shock": nodes next to a flagged interface, "iface": flagged interfaces, all three directions}."""
     ng = 3
     N = case.npoints
     Np = (case.nx + 2 * ng) * (case.ny + 2 * ng) * (case.nz + 2 * ng)
     visc = case.visc_law != W.VISC_NONE
     hyb = case.flux_mode == W.FLUX_HYBRID
     weno = case.flux_mode != W.FLUX_CENTRAL
+    conv = case.flux_mode != W.FLUX_WENO
     nprim = 6 + (2 if visc else 0) + (1 if weno else 0)        # rho u v w H p [T mu] [c]
-    out = {}
-    out["fill_prim"] = Np * (40 + 8 * nprim) + (Np - N) * 40   # read w, write primitives, write ghost w
-    out["sensor"] = N * (24 + 8 + (1 if hyb else 0))           # read u v w, write div [mask]
-    out["flags"] = N * (1 + 1) + alpha_shock * N * 4           # read mask, write flags byte, append to list
+    n_if = act["iface"] * N if hyb else (3 * N if weno else 0)
+    n_sh = act["shock"] * N if hyb else (N if weno else 0)
+    B, I = {}, {}
+    B["fill_prim"] = Np * (40 + 8 * nprim) + (Np - N) * 40     # read w, write primitives, write ghost w
+    I["fill_prim"] = Np * FP64_INST["fill_prim"]
+    B["sensor"] = N * (24 + 8 + (1 if hyb else 0))             # read u v w, write div [mask]
+    I["sensor"] = N * FP64_INST["sensor"]
+    B["flags"] = N * (1 + 1) + n_sh * 4 + n_if * 4             # read mask, write flags byte, append to lists
+    I["flags"] = 0
     # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
     # read R_prev (stages 2, 3), write R (stages 1, 2)
-    per_point = 48 + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40
-    main_nodes = N * (1.0 - alpha_shock) if hyb else (0 if case.flux_mode == W.FLUX_WENO else N)
-    shock_nodes = alpha_shock * N if hyb else (N if case.flux_mode == W.FLUX_WENO else 0)
-    out["rhs_main"] = main_nodes * per_point + (N if hyb else 0)          # + the flags byte
-    out["rhs_shock"] = shock_nodes * (per_point + 8 + 1 + 4)             # + c, flags byte, list entry
-    out["dt"] = N * (40 + (8 if visc else 0))                            # rho p u v w [mu]
-    out["misc"] = 0
-    return out, per_point
+    per_point = (48 if conv else 0) + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40
+    B["rhs_main"] = N * per_point
+    I["rhs_main"] = N * FP64_INST["rhs_main_" + (("c" if conv else "") + ("v" if visc else "") or "0")]
+    # WENO: per flagged interface one new stencil node of 7 fields (runs of flagged interfaces share the
+    # rest), a list entry, 5 flux values out
+    B["weno"] = n_if * (56 + 4 + 40)                           # per timed group: the x, y and z launches of a stage
+    I["weno"] = n_if * FP64_INST["weno_hybrid" if hyb else "weno_dense"]
+    # apply: flags byte + list entry, 2 x 5 flux values per direction (shared with the neighbour: 5),
+    # read-modify-write of w and (2 stages of 3) R
+    B["rhs_apply"] = n_sh * (1 + 4 + 3 * 40 + 80 + (2.0 / 3.0) * 80)
+    I["rhs_apply"] = n_sh * FP64_INST["rhs_apply"]
+    B["dt"] = N * (40 + (8 if visc else 0))                    # rho p u v w [mu]
+    I["dt"] = N * FP64_INST["dt"]
+    B["misc"] = 0
+    I["misc"] = 0
+    return B, I, per_point
 
 
 # ------------------------------------------------------------------------------------------------
@@ -257,53 +279,67 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
+    # Every timed region starts from the same state: the initial field advanced by `warmup` steps (the
+    # workload is not stationary -- shocklets form and the WENO activation grows -- so regions that start
+    # from different states are not comparable).
+    gpu.step(args.warmup)
+    w_start = torch.empty((5,) + gpu.shape, dtype=torch.float64, device=dev)
+    gpu.get_fields(w_start)
+
+    def timed_region(profile: bool):
+        gpu.set_fields(w_start)
+        for _ in range(3):                      # warm caches / clocks on the state itself (untimed)
+            gpu.rhs()
+        gpu.set_fields(w_start)                 # resets the activation totals too
+        if profile:
+            gpu.profile(True, max_records=10 * 3 * args.steps + 64)
+        l0 = gpu.kernel_launches()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sync_all()
+        e0.record(gpu.stream)
+        gpu.step(args.steps)
+        e1.record(gpu.stream)
+        sync_all()
+        return max_over_ranks(e0.elapsed_time(e1)), gpu.kernel_launches() - l0
+
     # ---- device-resident throughput: inputs already in HBM, K steps in one streams_step call
-    for _ in range(args.warmup):
-        gpu.step(1)
-    gpu.profile(True, max_records=8 * 3 * args.steps + 64)
-    l0 = gpu.kernel_launches()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sync_all()
+    timed_region(False)                         # one untimed pass of the whole region
     clocks = ClockSampler(local) if rank == 0 else None
-    e0.record(gpu.stream)
-    gpu.step(args.steps)
-    e1.record(gpu.stream)
-    sync_all()
+    ms, launches = timed_region(True)
     clk = clocks.stop() if clocks else None
-    ms = max_over_ranks(e0.elapsed_time(e1))
-    launches = gpu.kernel_launches() - l0
     prof, dropped = gpu.get_profile()
     gpu.profile(False)
-    flagged_sum, shock_sum, evals = gpu.get_activation_totals()
-    alpha_shock = shock_sum / (evals * N) if evals else (1.0 if case.flux_mode == W.FLUX_WENO else 0.0)
-    alpha_nodes = flagged_sum / (evals * N) if evals else 0.0
+    flagged_sum, shock_sum, iface_sum, evals = gpu.get_activation_totals()
+    act = {"flagged": flagged_sum / (evals * N) if evals else 0.0,
+           "shock": shock_sum / (evals * N) if evals else 0.0,
+           "iface": sum(iface_sum) / (evals * N) if evals else 0.0,
+           "iface_xyz": [x / (evals * N) if evals else 0.0 for x in iface_sum]}
     value = world * N * args.steps / (ms * 1e-3)
 
-    # the same K steps with the event pairs off (how much the per-kernel timing costs)
-    sync_all()
-    e0.record(gpu.stream)
-    gpu.step(args.steps)
-    e1.record(gpu.stream)
-    sync_all()
-    ms_noprof = max_over_ranks(e0.elapsed_time(e1))
+    # the same K steps with the event pairs off (what the per-kernel timing costs)
+    ms_noprof, _ = timed_region(False)
 
-    # ---- end to end through the C ABI with HOST buffers: h2d of the state, one step, d2h of the state
-    h_in = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
-    h_out = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
-    h_in.numpy()[...] = case.w0
+    # ---- end to end through the C ABI with HOST buffers: every step copies the state host -> device,
+    # advances it one RK3 step and copies it back; the state evolves through the host round trips
+    h_a = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
+    h_b = torch.empty((5,) + gpu.shape, dtype=torch.float64).pin_memory()
+    gpu.set_fields(w_start)
+    gpu.get_fields(h_a.numpy())
     n_e2e = max(3, min(args.steps, 20))
     for _ in range(2):
-        gpu.set_fields(h_in.numpy()); gpu.step(1); gpu.get_fields(h_out.numpy())
+        gpu.set_fields(h_a.numpy()); gpu.step(1); gpu.get_fields(h_b.numpy())
+    gpu.get_fields(h_b.numpy())
     sync_all()
     t0 = time.perf_counter()
     for _ in range(n_e2e):
-        gpu.set_fields(h_in.numpy())      # host -> device (synchronous on return)
+        gpu.set_fields(h_a.numpy())       # host -> device (synchronous on return)
         gpu.step(1)
-        gpu.get_fields(h_out.numpy())     # device -> host (synchronous on return)
+        gpu.get_fields(h_b.numpy())       # device -> host (synchronous on return)
+        h_a, h_b = h_b, h_a
     torch.cuda.synchronize(dev)
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
     e2e_value = world * N * n_e2e / (e2e_ms * 1e-3)
-    assert np.isfinite(h_out.numpy()).all()
+    assert np.isfinite(h_a.numpy()).all()
 
     if rank != 0:
         gpu.destroy()
@@ -314,19 +350,32 @@ def run_ours(args):
 
     # ---- per-kernel roofline from the event pairs of the timed region
     peak, peak_src = load_peaks()
-    abytes, per_point = algorithmic_bytes(case, alpha_shock)
+    sm_mhz = (clk or {}).get("sm_mhz") or 1965.0
+    peak_inst = N_SM * FP64_LANES_PER_SM * sm_mhz * 1e6        # fp64 thread-instructions / s at the clock under load
+    B, I, per_point = work_model(case, act)
     kernels = {}
     for name, (kms, cnt) in prof.items():
         if cnt == 0:
             continue
-        avg_ms = kms / cnt
-        gbs = abytes[name] / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
-        kernels[name] = {"launches": cnt, "avg_ms": avg_ms, "share": kms / ms, "alg_bytes": abytes[name],
-                         "gbs": gbs, "frac_hbm": gbs / peak}
+        t = kms / cnt * 1e-3
+        gbs = B[name] / t / 1e9 if t > 0 else 0.0
+        ginst = I[name] / t / 1e9 if t > 0 else 0.0
+        t_hbm, t_alu = B[name] / (peak * 1e9), I[name] / peak_inst
+        kernels[name] = {"launches": cnt, "avg_ms": t * 1e3, "share": kms / ms, "alg_bytes": B[name], "gbs": gbs,
+                         "frac_hbm": gbs / peak, "fp64_ginst_s": ginst, "frac_fp64": ginst * 1e9 / peak_inst,
+                         "bound": "alu" if t_alu > t_hbm else "hbm", "frac": max(t_hbm, t_alu) / t if t > 0 else 0.0}
     dom = max(kernels, key=lambda k: kernels[k]["avg_ms"] * kernels[k]["launches"])
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["frac_hbm"], "traffic": None, "peak_source": peak_src,
-                "alg_bytes_per_point": per_point, "kernels": kernels, "events_dropped": dropped}
+    kd = kernels[dom]
+    if kd["bound"] == "hbm":
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": kd["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": kd["frac_hbm"], "traffic": None, "peak_source": peak_src}
+    else:   # fp64 pipe: 2 flop per instruction slot (DFMA), so 1 inst/s == 2 flop/s of the nominal peak
+        roofline = {"kernel": dom, "bound": "alu", "achieved": 2 * kd["fp64_ginst_s"] / 1e3, "peak": 2 * peak_inst / 1e12,
+                    "unit": "TFLOP/s", "frac": kd["frac_fp64"], "traffic": None,
+                    "peak_source": "148 SM x 64 fp64 FMA lanes x 2 x %.0f MHz (clock under load); achieved counts every "
+                                   "fp64 instruction as one FMA slot (DESIGN.md)" % sm_mhz}
+    roofline.update({"alg_bytes_per_point_rhs_main": per_point, "kernels": kernels, "events_dropped": dropped,
+                     "hbm_peak_gbs": peak, "hbm_peak_source": peak_src})
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):           # dram bytes per launch from the committed ncu --set full capture
         with open(traffic_file) as f:
@@ -354,7 +403,7 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (workspace %.2f GB vs 126 MB)" % (gpu.workspace_bytes / 1e9)
                    if gpu.workspace_bytes > 4 * 126e6 else "workspace %.1f MB is L2-resident; latency point, not a roofline point"
                    % (gpu.workspace_bytes / 1e6),
-                   "weno_activation": {"flagged_nodes": alpha_nodes, "shock_kernel_nodes": alpha_shock}},
+                   "weno_activation": act},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
                 "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e},

@@ -112,15 +112,17 @@ int streams_get_fields(streams_ctx* ctx, double* w_out, int dst_is_device);
 int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_out,
                        int dst_is_device);
 
-/* Diagnostics of the last RHS evaluation, HOST outputs, nullable: number of flagged nodes and
- * number of nodes handled by the shock-capturing kernel (any adjacent interface flagged). */
-int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes);
+/* Diagnostics of the last RHS evaluation, HOST outputs, nullable: number of flagged nodes, number of
+ * nodes next to a flagged interface, and interfaces[3] = flagged interfaces per direction (the paper's
+ * "WENO activation"). */
+int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes,
+                           long long* interfaces);
 
 /* The same counts summed over every sensor evaluation since streams_set_fields (hybrid mode; zeros
- * otherwise), and the number of evaluations: the paper's "WENO activation", which is
- * "not known a priori and may even vary".  HOST outputs, nullable.  Synchronises the stream. */
+ * otherwise), and the number of evaluations: the activation "is not known a priori and may even vary"
+ * (PAPER:497).  HOST outputs, nullable; interfaces_sum has 3 entries.  Synchronises the stream. */
 int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum,
-                                  long long* evaluations);
+                                  long long* interfaces_sum, long long* evaluations);
 
 /* Number of kernels the library has launched on this context since streams_init. */
 long long streams_kernel_launches(const streams_ctx* ctx);
@@ -128,7 +130,8 @@ long long streams_kernel_launches(const streams_ctx* ctx);
 /* Per-kernel device timing, the measurement of BASELINE metric part 2 ("per-kernel % of roofline";
  * the paper's analogue is its per-kernel table).  Kernel classes: */
 enum { STREAMS_K_FILL_PRIM = 0, STREAMS_K_DT = 1, STREAMS_K_SENSOR = 2, STREAMS_K_FLAGS = 3,
-       STREAMS_K_RHS_MAIN = 4, STREAMS_K_RHS_SHOCK = 5, STREAMS_K_MISC = 6, STREAMS_K_COUNT = 7 };
+       STREAMS_K_RHS_MAIN = 4, STREAMS_K_WENO = 5, STREAMS_K_APPLY = 6, STREAMS_K_MISC = 7,
+       STREAMS_K_COUNT = 8 };
 
 /* enable != 0: from now on every launch is bracketed by a CUDA event pair on the context's stream
  * (at most max_records launches between two streams_get_profile calls are recorded, the rest are

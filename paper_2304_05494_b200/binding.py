@@ -20,7 +20,7 @@ EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "str
            "streams_kernel_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name",
            "streams_last_error", "streams_destroy")
-STREAMS_K_COUNT = 7
+STREAMS_K_COUNT = 8
 
 _dp = C.POINTER(C.c_double)
 
@@ -67,8 +67,8 @@ def load_library(path: str = LIB_PATH):
     lib.streams_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
     lib.streams_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
-    lib.streams_get_activation.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
-    lib.streams_get_activation_totals.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 3
+    lib.streams_get_activation.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 3
+    lib.streams_get_activation_totals.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4
     lib.streams_kernel_launches.restype = C.c_longlong
     lib.streams_kernel_launches.argtypes = [C.c_void_p]
     lib.streams_profile.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -186,15 +186,18 @@ class Streams:
         return theta, mask
 
     def get_activation(self):
+        """(flagged nodes, nodes next to a flagged interface, [flagged interfaces x, y, z]) of the last RHS."""
         a, b = C.c_longlong(), C.c_longlong()
-        self._check(self.lib.streams_get_activation(self.h, C.byref(a), C.byref(b)))
-        return a.value, b.value
+        f = (C.c_longlong * 3)()
+        self._check(self.lib.streams_get_activation(self.h, C.byref(a), C.byref(b), f))
+        return a.value, b.value, list(f)
 
     def get_activation_totals(self):
-        """(flagged nodes, shock-kernel nodes, sensor evaluations) summed since set_fields."""
+        """(flagged nodes, shock-list nodes, [interfaces x, y, z], sensor evaluations) summed since set_fields."""
         a, b, n = C.c_longlong(), C.c_longlong(), C.c_longlong()
-        self._check(self.lib.streams_get_activation_totals(self.h, C.byref(a), C.byref(b), C.byref(n)))
-        return a.value, b.value, n.value
+        f = (C.c_longlong * 3)()
+        self._check(self.lib.streams_get_activation_totals(self.h, C.byref(a), C.byref(b), f, C.byref(n)))
+        return a.value, b.value, list(f), n.value
 
     def kernel_launches(self):
         return int(self.lib.streams_kernel_launches(self.h))

@@ -22,8 +22,8 @@ struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
   size_t N;
-  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_list, off_counters, off_R, off_metrics,
-      off_scal, total;
+  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_list, off_ilist, off_dF, off_counters, off_R,
+      off_metrics, off_scal, total;
   int nq;
 };
 
@@ -48,7 +48,8 @@ bool valid_bc(int b) { return b == STREAMS_BC_PERIODIC || b == STREAMS_BC_WALL_I
 const char* plan(const streams_grid* g, const streams_gas* gas, const streams_scheme* sc, Sizes& S) {
   if (!g || !gas || !sc) return "null argument";
   if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid extents must be positive";
-  if ((long long)g->nx * g->ny * g->nz > 2000000000LL) return "grid too large for 32-bit node indices";
+  if (((long long)g->nx + 40) * ((long long)g->ny + 8) * ((long long)g->nz + 8) > 2000000000LL)
+    return "grid too large for 32-bit node indices";
   if (!(g->lx > 0) || !(g->lz > 0)) return "lx, lz must be positive";
   if (!valid_bc(g->bc_x) || !valid_bc(g->bc_y_lo) || !valid_bc(g->bc_y_hi) || !valid_bc(g->bc_z)) return "bad bc code";
   if (g->bc_x == STREAMS_BC_WALL_ISOTHERMAL || g->bc_z == STREAMS_BC_WALL_ISOTHERMAL) return "walls are supported in y only";
@@ -91,7 +92,9 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.off_mask = take(S.fs);
   S.off_nflag = take(hyb ? S.N : 256);
   S.off_list = take(hyb ? S.N * 4 : 256);
-  S.off_counters = take(256);
+  S.off_ilist = take(hyb ? 3 * S.fs * 4 : 256);
+  S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
+  S.off_counters = take(C_COUNT * 4);
   S.off_R = take(5 * S.N * 8);
   S.off_metrics = take(3 * (size_t)g->ny * 8);
   S.off_scal = take(S_COUNT * 8);
@@ -229,13 +232,17 @@ int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   return STREAMS_OK;
 }
 
-// the fused RHS (+ update) of one stage: central/main half, then the shock-capturing half
+// the RHS (+ update) of one stage: fused central/viscous pass over all nodes, then the WENO fluxes of the
+// flagged interfaces and their application
 int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
   const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
-  const int b = timed(ctx, STREAMS_K_RHS_SHOCK, [&] { return launch_rhs_shock(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
-  return (a < 0 || b < 0) ? -1 : a + b;
+  if (a < 0) return -1;
+  if (ctx->scheme.flux_mode == STREAMS_FLUX_CENTRAL) return a;
+  const int b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
+  const int c = timed(ctx, STREAMS_K_APPLY, [&] { return launch_rhs_apply(P, sa, st); });
+  return (b < 0 || c < 0) ? -1 : a + b + c;
 }
 
 }  // namespace
@@ -282,6 +289,8 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
   P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
   P.list = (int*)(ctx->base + S.off_list);
+  for (int d = 0; d < 3; ++d) P.ilist[d] = (int*)(ctx->base + S.off_ilist) + (size_t)d * S.fs;
+  P.dF = (double*)(ctx->base + S.off_dF);
   P.counters = (int*)(ctx->base + S.off_counters);
   P.R = (double*)(ctx->base + S.off_R);
   double* met = (double*)(ctx->base + S.off_metrics);
@@ -332,7 +341,7 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
     CU(cudaMemcpy3DAsync(&p, ctx->stream));
   }
   CU(cudaMemsetAsync(P.scal, 0, S_COUNT * 8, ctx->stream));
-  CU(cudaMemsetAsync(P.counters, 0, 256, ctx->stream));
+  CU(cudaMemsetAsync(P.counters, 0, C_COUNT * 4, ctx->stream));
   if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));   // the host buffer may be reused on return
   ctx->have_fields = true;
   ctx->step_count = 0;
@@ -422,30 +431,35 @@ int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_
   return STREAMS_OK;
 }
 
-int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes) {
+int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long* shock_nodes, long long* interfaces) {
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
-  int h[2] = {0, 0};
+  const DevP& P = ctx->P;
+  int h[C_COUNT] = {0};
   if (ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID) {
-    CU(cudaMemcpyAsync(h, ctx->P.counters, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(h, P.counters, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
   } else if (ctx->scheme.flux_mode == STREAMS_FLUX_WENO) {
-    h[0] = (int)ctx->P.N; h[1] = (int)ctx->P.N;
+    h[C_NSHOCK] = (int)P.N; h[C_NFLAGGED] = (int)P.N;
+    h[C_NIFACE] = (P.nx + 1) * P.ny * P.nz; h[C_NIFACE + 1] = P.nx * (P.ny + 1) * P.nz; h[C_NIFACE + 2] = P.nx * P.ny * (P.nz + 1);
   }
-  if (shock_nodes) *shock_nodes = h[0];
-  if (flagged_nodes) *flagged_nodes = h[1];
+  if (shock_nodes) *shock_nodes = h[C_NSHOCK];
+  if (flagged_nodes) *flagged_nodes = h[C_NFLAGGED];
+  if (interfaces) for (int d = 0; d < 3; ++d) interfaces[d] = h[C_NIFACE + d];
   return STREAMS_OK;
 }
 
-int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum, long long* evaluations) {
+int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum, long long* interfaces_sum,
+                                  long long* evaluations) {
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
-  unsigned long long h[3] = {0, 0, 0};
+  unsigned long long h[6] = {0, 0, 0, 0, 0, 0};
   if (ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID) {
-    CU(cudaMemcpyAsync(h, ctx->P.counters + 4, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(h, ctx->P.counters + C_TOTALS, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
   }
   if (shock_sum) *shock_sum = (long long)h[0];
   if (flagged_sum) *flagged_sum = (long long)h[1];
   if (evaluations) *evaluations = (long long)h[2];
+  if (interfaces_sum) for (int d = 0; d < 3; ++d) interfaces_sum[d] = (long long)h[3 + d];
   return STREAMS_OK;
 }
 
@@ -481,7 +495,7 @@ int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long lon
 }
 
 const char* streams_kernel_name(int kind) {
-  static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "rhs_shock", "misc"};
+  static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "weno", "rhs_apply", "misc"};
   return (kind >= 0 && kind < STREAMS_K_COUNT) ? names[kind] : "";
 }
 

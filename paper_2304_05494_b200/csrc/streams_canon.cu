@@ -103,8 +103,8 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
 // a3: Ducros-type sensor, node mask and dilatation (O2).  One thread per interior node.
 // Canonical order: delta_l = f(+l) - f(-l); acc = a_1 delta_1; acc = acc + a_l delta_l; d = acc * metric;
 // div = (u_x + v_y) + w_z; s = (((div^2 + ox^2) + oy^2) + oz^2) + eps_s; theta = max(-div/sqrt(s), 0).
-// Threads next to a face also write the ghost images of div / mask (periodic wrap, else constant
-// extrapolation; S6).  HBM: 24 B read + 8 B (div) + 1 B (mask) write per node.
+// The face ghosts of div / mask are filled by scalar_ghost_kernel right after.
+// HBM: 24 B read + 8 B (div) + 1 B (mask) write per node.
 // ---------------------------------------------------------------------------------------------
 template <int L>
 __device__ __forceinline__ double ddc(const DevP& P, const double* __restrict__ f, long long n, long long s, double metric) {
@@ -114,27 +114,42 @@ __device__ __forceinline__ double ddc(const DevP& P, const double* __restrict__ 
   return acc * metric;
 }
 
-template <class T>
-__device__ __forceinline__ void write_images(const DevP& P, T* f, T val, int i, int j, int k, long long n) {
+// Face ghosts of the nodal scalars div and mask (S6): periodic wrap, else constant extrapolation of the
+// nearest interior value.  One thread per face-ghost node (edges and corners are never read: every
+// consumer is a star stencil).  Segments of the flat index: x faces, y faces, z faces.
+template <bool MASK>
+__global__ void __launch_bounds__(256) scalar_ghost_kernel(const DevP P) {
   const int g = P.ng;
-  if (P.bc_x == BC_PERIODIC) {
-    if (i < g) f[n + P.nx] = val;
-    if (i >= P.nx - g) f[n - P.nx] = val;
+  const long long nX = 2LL * g * P.ny * P.nz, nY = 2LL * g * P.nx * P.nz, nZ = 2LL * g * P.nx * P.ny;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int i, j, k, is, js, ks;
+  if (t < nX) {
+    const int m = (int)(t % (2 * g));
+    const long long t2 = t / (2 * g);
+    j = js = (int)(t2 % P.ny); k = ks = (int)(t2 / P.ny);
+    i = m < g ? m - g : P.nx + (m - g);
+    is = P.bc_x == BC_PERIODIC ? (i < 0 ? i + P.nx : i - P.nx) : (i < 0 ? 0 : P.nx - 1);
+  } else if ((t -= nX) < nY) {
+    i = is = (int)(t % P.nx);
+    const long long t2 = t / P.nx;
+    const int m = (int)(t2 % (2 * g));
+    k = ks = (int)(t2 / (2 * g));
+    j = m < g ? m - g : P.ny + (m - g);
+    if (j < 0) js = P.bc_y_lo == BC_PERIODIC ? j + P.ny : 0;
+    else js = P.bc_y_hi == BC_PERIODIC ? j - P.ny : P.ny - 1;
+  } else if ((t -= nY) < nZ) {
+    i = is = (int)(t % P.nx);
+    const long long t2 = t / P.nx;
+    j = js = (int)(t2 % P.ny);
+    const int m = (int)(t2 / P.ny);
+    k = m < g ? m - g : P.nz + (m - g);
+    ks = P.bc_z == BC_PERIODIC ? (k < 0 ? k + P.nz : k - P.nz) : (k < 0 ? 0 : P.nz - 1);
   } else {
-    if (i == 0) for (int m = 1; m <= g; ++m) f[n - m] = val;
-    if (i == P.nx - 1) for (int m = 1; m <= g; ++m) f[n + m] = val;
+    return;
   }
-  if (P.bc_y_lo == BC_PERIODIC) { if (j >= P.ny - g) f[n - (long long)P.ny * P.sy] = val; }
-  else if (j == 0) for (int m = 1; m <= g; ++m) f[n - m * P.sy] = val;
-  if (P.bc_y_hi == BC_PERIODIC) { if (j < g) f[n + (long long)P.ny * P.sy] = val; }
-  else if (j == P.ny - 1) for (int m = 1; m <= g; ++m) f[n + m * P.sy] = val;
-  if (P.bc_z == BC_PERIODIC) {
-    if (k < g) f[n + (long long)P.nz * P.sz] = val;
-    if (k >= P.nz - g) f[n - (long long)P.nz * P.sz] = val;
-  } else {
-    if (k == 0) for (int m = 1; m <= g; ++m) f[n - m * P.sz] = val;
-    if (k == P.nz - 1) for (int m = 1; m <= g; ++m) f[n + m * P.sz] = val;
-  }
+  const long long n = pidx(P, i, j, k), ns = pidx(P, is, js, ks);
+  P.div[n] = P.div[ns];
+  if (MASK) P.mask[n] = P.mask[ns];
 }
 
 template <int L, bool MASK, bool THETA>
@@ -153,7 +168,6 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
   const double wx = ddc<L>(P, w, n, 1, P.inv_dx), wy = ddc<L>(P, w, n, P.sy, my), wz = ddc<L>(P, w, n, P.sz, P.inv_dz);
   const double dv = (ux + vy) + wz;
   P.div[n] = dv;
-  write_images<double>(P, P.div, dv, i, j, k, n);
   if (MASK || THETA) {
     const double ox = wy - vz, oy = uz - wx, oz = vx - uy;
     const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
@@ -163,7 +177,6 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
     if (MASK) {
       const unsigned char m = (th > P.thr) ? 1 : 0;
       P.mask[n] = m;
-      write_images<unsigned char>(P, P.mask, m, i, j, k, n);
     }
   }
 }
@@ -171,8 +184,13 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
 // ---------------------------------------------------------------------------------------------
 // Interface flags (O2 / S5): interface n+1/2 along d uses WENO iff any node of its 2r-node
 // stencil {n-r+1..n+r} is flagged.  Per interior node the six adjacent interfaces are packed in a
-// byte (bit 2d: minus side, bit 2d+1: plus side); nodes with any bit set are appended to the
-// shock-node list (warp-aggregated atomic; order is irrelevant, each node is computed independently).
+// byte (bit 2d: minus side, bit 2d+1: plus side).  Three kinds of work lists are built from it:
+//   list      nodes with any bit set (consumed by rhs_apply_kernel),
+//   ilist[d]  flagged interfaces of direction d, each named by the padded index of its left node and
+//             owned by exactly one thread: the node on its left, or - for the interface below the first
+//             node of a pencil - that first node (consumed by weno_kernel).
+// Appends are aggregated per block (one atomic per list per block); the order inside a list is
+// irrelevant, every entry is processed independently and writes its own slot.
 // ---------------------------------------------------------------------------------------------
 template <int R>
 __global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
@@ -181,11 +199,11 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
   const int k = blockIdx.z;
   const bool in = (i < P.nx && j < P.ny);
   unsigned f = 0, own = 0;
-  long long o = 0;
+  long long o = 0, n = 0;
+  const long long st[3] = {1, P.sy, P.sz};
   if (in) {
-    const long long n = pidx(P, i, j, k);
+    n = pidx(P, i, j, k);
     o = iidx(P, i, j, k);
-    const long long st[3] = {1, P.sy, P.sz};
     own = P.mask[n];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
@@ -199,17 +217,42 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
     }
     P.nflag[o] = (unsigned char)f;
   }
-  const unsigned ball = __ballot_sync(0xffffffffu, f != 0);
-  const unsigned ballm = __ballot_sync(0xffffffffu, own != 0);
-  const int lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31;
-  int base = 0;
-  if (lane == 0) {
-    unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + 4);   // totals since set_fields
-    if (ball) { base = atomicAdd(&P.counters[0], __popc(ball)); atomicAdd(&cum[0], (unsigned long long)__popc(ball)); }
-    if (ballm) { atomicAdd(&P.counters[1], __popc(ballm)); atomicAdd(&cum[1], (unsigned long long)__popc(ballm)); }
+  // categories: 0 node list; 1..3 plus-side interface of x, y, z; 4..6 minus-side interface of the first
+  // node of a pencil in x, y, z; 7 flagged nodes (count only)
+  const bool want[8] = {f != 0, (f & 2u) != 0, (f & 8u) != 0, (f & 32u) != 0,
+                        i == 0 && (f & 1u) != 0, j == 0 && (f & 4u) != 0, k == 0 && (f & 16u) != 0, own != 0};
+  __shared__ int s_cnt[8][8];
+  __shared__ int s_base[8];
+  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+  const int lane = tid & 31, wid = tid >> 5;
+  unsigned bal[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    bal[c] = __ballot_sync(0xffffffffu, want[c]);
+    if (lane == 0) s_cnt[c][wid] = __popc(bal[c]);
   }
-  base = __shfl_sync(0xffffffffu, base, 0);
-  if (f != 0) P.list[base + __popc(ball & ((1u << lane) - 1u))] = (int)o;
+  __syncthreads();
+  if (tid < 8) {
+    int tot = 0;
+    for (int w = 0; w < 8; ++w) { const int c = s_cnt[tid][w]; s_cnt[tid][w] = tot; tot += c; }
+    int base = 0;
+    if (tot) {
+      unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS);
+      const int d = (tid - 1) % 3;
+      if (tid == 0) { base = atomicAdd(&P.counters[C_NSHOCK], tot); atomicAdd(&cum[0], (unsigned long long)tot); }
+      else if (tid == 7) { atomicAdd(&P.counters[C_NFLAGGED], tot); atomicAdd(&cum[1], (unsigned long long)tot); }
+      else { base = atomicAdd(&P.counters[C_NIFACE + d], tot); atomicAdd(&cum[3 + d], (unsigned long long)tot); }
+    }
+    s_base[tid] = base;
+  }
+  __syncthreads();
+  const unsigned lt = (1u << lane) - 1u;
+  if (want[0]) P.list[s_base[0] + s_cnt[0][wid] + __popc(bal[0] & lt)] = (int)o;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (want[1 + d]) P.ilist[d][s_base[1 + d] + s_cnt[1 + d][wid] + __popc(bal[1 + d] & lt)] = (int)n;
+    if (want[4 + d]) P.ilist[d][s_base[4 + d] + s_cnt[4 + d][wid] + __popc(bal[4 + d] & lt)] = (int)(n - st[d]);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -278,9 +321,10 @@ __global__ void step_end_kernel(const DevP P) {
 }
 
 __global__ void reset_counters_kernel(const DevP P) {
-  P.counters[0] = 0;
-  P.counters[1] = 0;
-  reinterpret_cast<unsigned long long*>(P.counters + 4)[2] += 1ull;     // sensor evaluations since set_fields
+  P.counters[C_NSHOCK] = 0;
+  P.counters[C_NFLAGGED] = 0;
+  P.counters[C_NIFACE] = 0; P.counters[C_NIFACE + 1] = 0; P.counters[C_NIFACE + 2] = 0;
+  reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[2] += 1ull;   // sensor evaluations since set_fields
 }
 
 // -------------------------------------------------------------------------- launch wrappers
@@ -302,7 +346,11 @@ static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st
   if (theta) sensor_kernel<L, true, true><<<g, b, 0, st>>>(P);
   else if (mask) sensor_kernel<L, true, false><<<g, b, 0, st>>>(P);
   else sensor_kernel<L, false, false><<<g, b, 0, st>>>(P);
-  return 1;
+  const long long ghosts = 2LL * P.ng * ((long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny);
+  dim3 gg((unsigned)((ghosts + 255) / 256));
+  if (mask || theta) scalar_ghost_kernel<true><<<gg, 256, 0, st>>>(P);
+  else scalar_ghost_kernel<false><<<gg, 256, 0, st>>>(P);
+  return 2;
 }
 int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st) {
   switch (L) {

@@ -3,11 +3,13 @@
 // terms (O4) and the low-storage RK3 update (O5), so R is written once and w is updated in place
 // (stencils read the primitive copy q, never w, so no ping-pong buffer is needed).
 //
-//   rhs_main_kernel  : every node, central scheme; in hybrid mode nodes that touch a flagged
-//                      interface are left to
-//   rhs_shock_kernel : the compacted list of such nodes (or every node in full-WENO mode); each of
-//                      the node's six interfaces is WENO (O3) or central according to its flag.
-// Both kernels end in the same finish(): viscous combination, R store, w update.
+//   rhs_main_kernel  : every node, central scheme (in full-WENO mode: viscous terms and update only).
+//   weno_kernel      : one thread per flagged interface of one direction (hybrid: the per-direction lists
+//                      of flags_kernel; full-WENO: every interface): WENO characteristic flux (O3) minus,
+//                      in hybrid mode, the central flux that rhs_main_kernel used there -> dF.
+//   rhs_apply_kernel : nodes next to a flagged interface add -(dF_{n+1/2} - dF_{n-1/2}) metric to R and
+//                      the matching increment to w.
+// Every flagged interface is therefore evaluated exactly once, by a warp whose lanes all do WENO work.
 #include "streams_dev.cuh"
 #include "streams_launch.h"
 
@@ -171,7 +173,7 @@ __device__ __forceinline__ void zero_vacc(VAcc& V) {
 // block-rows in y is swept through all of z before the next slab starts: the 2 ng z-neighbour
 // planes of a slab then stay in L2.
 // ---------------------------------------------------------------------------------------------
-template <int L, int LV, bool VISC, bool HYB, int BX, int BY, int BZ>
+template <int L, int LV, bool VISC, bool CONV, int BX, int BY, int BZ>
 __global__ void __launch_bounds__(BX * BY * BZ) rhs_main_kernel(const DevP P, const StageArgs sa, int nbx, int nby,
                                                                int nbz, int slab) {
   // decode block id -> (bx, by, bz), slab-major
@@ -190,7 +192,6 @@ __global__ void __launch_bounds__(BX * BY * BZ) rhs_main_kernel(const DevP P, co
   const int i = bx * BX + tx, j = (sl * slab + byl) * BY + ty, k = bz * BZ + tz;
   if (i >= P.nx || j >= P.ny || k >= P.nz) return;
   const long long o = iidx(P, i, j, k);
-  if (HYB) { if (P.nflag[o]) return; }
   const long long n = pidx(P, i, j, k);
   double c0[6];
   load_centre(P, n, c0);
@@ -199,9 +200,9 @@ __global__ void __launch_bounds__(BX * BY * BZ) rhs_main_kernel(const DevP P, co
   double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   VAcc V;
   zero_vacc(V);
-  dir_terms<0, L, LV, true, VISC>(P, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
-  dir_terms<1, L, LV, true, VISC>(P, n, P.sy, P.eta_y_c[j], eyv, eyy, c0, T0, r, V);
-  dir_terms<2, L, LV, true, VISC>(P, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
+  dir_terms<0, L, LV, CONV, VISC>(P, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
+  dir_terms<1, L, LV, CONV, VISC>(P, n, P.sy, P.eta_y_c[j], eyv, eyy, c0, T0, r, V);
+  dir_terms<2, L, LV, CONV, VISC>(P, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
   finish<VISC>(P, sa, n, o, c0, mu0, r, V);
 }
 
@@ -394,27 +395,49 @@ __device__ __forceinline__ void weno_flux(const DevP& P, long long n, long long 
   }
 }
 
-// One direction of a shock node: both adjacent interfaces central -> pair-difference form, else
-// interface fluxes one by one.
-template <int D, int L, int LV, int R, bool VISC>
-__device__ __forceinline__ void shock_dir(const DevP& P, unsigned fl, long long n, long long s, double met_c,
-                                          double met_v, double eyy, const double c0[6], double T0, double r[5],
-                                          VAcc& V) {
-  if (fl == 0) {
-    dir_terms<D, L, LV, true, VISC>(P, n, s, met_c, met_v, eyy, c0, T0, r, V);
-    return;
-  }
-  if (VISC) dir_terms<D, L, LV, false, true>(P, n, s, met_c, met_v, eyy, c0, T0, r, V);
-  double fp[5], fm[5];
-  if (fl & 2u) weno_flux<D, R>(P, n, s, fp); else central_flux<D, L>(P, n, s, fp);
-  if (fl & 1u) weno_flux<D, R>(P, n - s, s, fm); else central_flux<D, L>(P, n - s, s, fm);
+// ---------------------------------------------------------------------------------------------
+// weno_kernel: one thread per flagged interface of direction D.  DENSE (full-WENO mode) enumerates every
+// interface of the direction, left node index -1 .. n_D - 1, and stores the WENO flux itself; otherwise
+// the list built by flags_kernel is walked and the difference to the central flux is stored.
+// ---------------------------------------------------------------------------------------------
+template <int D, int L, int R, bool DENSE>
+__global__ void __launch_bounds__(128) weno_kernel(const DevP P) {
+  const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
+  const int e0 = P.nx + (D == 0), e1 = P.ny + (D == 1);
+  const long long count = DENSE ? (long long)e0 * e1 * (P.nz + (D == 2)) : (long long)P.counters[C_NIFACE + D];
+  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += (long long)gridDim.x * blockDim.x) {
+    long long n;
+    if (DENSE) {
+      const int i = (int)(t % e0);
+      const long long t2 = t / e0;
+      const int j = (int)(t2 % e1), k = (int)(t2 / e1);
+      n = pidx(P, i - (D == 0), j - (D == 1), k - (D == 2));
+    } else {
+      n = P.ilist[D][t];
+    }
+    double fw[5];
+    weno_flux<D, R>(P, n, s, fw);
+    if (!DENSE) {
+      double fc[5];
+      central_flux<D, L>(P, n, s, fc);
 #pragma unroll
-  for (int q = 0; q < 5; ++q) r[q] -= (fp[q] - fm[q]) * met_c;
+      for (int q = 0; q < 5; ++q) fw[q] -= fc[q];
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) out[q * P.fs + n] = fw[q];
+  }
 }
 
-template <int L, int LV, int R, bool VISC, bool DENSE>
-__global__ void __launch_bounds__(128) rhs_shock_kernel(const DevP P, const StageArgs sa) {
-  const long long count = DENSE ? P.N : (long long)P.counters[0];
+// ---------------------------------------------------------------------------------------------
+// rhs_apply_kernel: R -= (dF_{n+1/2} - dF_{n-1/2}) metric at the nodes of the shock list (every node in
+// DENSE mode), and the same increment, times dt gamma_l, to w (the RK update of rhs_main_kernel is
+// linear in R).  One thread per node, no two threads touch the same node: deterministic.
+// ---------------------------------------------------------------------------------------------
+template <bool DENSE>
+__global__ void __launch_bounds__(256) rhs_apply_kernel(const DevP P, const StageArgs sa) {
+  const long long count = DENSE ? P.N : (long long)P.counters[C_NSHOCK];
+  const double dtg = sa.update_w ? P.scal[S_DT] * sa.gam : 0.0;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += (long long)gridDim.x * blockDim.x) {
     const long long o = DENSE ? t : (long long)P.list[t];
     const unsigned fl = DENSE ? 0x3fu : (unsigned)P.nflag[o];
@@ -422,17 +445,32 @@ __global__ void __launch_bounds__(128) rhs_shock_kernel(const DevP P, const Stag
     const long long t2 = o / P.nx;
     const int j = (int)(t2 % P.ny), k = (int)(t2 / P.ny);
     const long long n = pidx(P, i, j, k);
-    double c0[6];
-    load_centre(P, n, c0);
-    double T0 = 0.0, mu0 = 0.0, eyv = 0.0, eyy = 0.0;
-    if (VISC) { T0 = P.q[Q_T * P.fs + n]; mu0 = P.q[Q_MU * P.fs + n]; eyv = P.eta_y_v[j]; eyy = P.eta_yy_v[j]; }
-    double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    VAcc V;
-    zero_vacc(V);
-    shock_dir<0, L, LV, R, VISC>(P, fl & 3u, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
-    shock_dir<1, L, LV, R, VISC>(P, (fl >> 2) & 3u, n, P.sy, P.eta_y_c[j], eyv, eyy, c0, T0, r, V);
-    shock_dir<2, L, LV, R, VISC>(P, (fl >> 4) & 3u, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
-    finish<VISC>(P, sa, n, o, c0, mu0, r, V);
+    const long long st[3] = {1, P.sy, P.sz};
+    const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+    double dr[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const unsigned b = (fl >> (2 * d)) & 3u;
+      if (b == 0) continue;
+      const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) {
+        const double fp = (b & 2u) ? f[q * P.fs] : 0.0;
+        const double fm = (b & 1u) ? f[q * P.fs - st[d]] : 0.0;
+        dr[q] -= (fp - fm) * met[d];
+      }
+    }
+    if (sa.update_w) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) {
+        double* wp = P.w + q * P.fs + n;
+        *wp = *wp + dtg * dr[q];
+      }
+    }
+    if (sa.write_r) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) sa.r_out[q * P.N + o] += dr[q];
+    }
   }
 }
 
@@ -441,39 +479,46 @@ constexpr int MBX = 32, MBY = 4, MBZ = 4;
 
 template <int L, int LV, int R>
 static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
-  if (P.flux_mode == FLUX_WENO) return 0;
   const bool visc = P.visc_law != VISC_NONE;
+  const bool conv = P.flux_mode != FLUX_WENO;
   const int nbx = (P.nx + MBX - 1) / MBX, nby = (P.ny + MBY - 1) / MBY, nbz = (P.nz + MBZ - 1) / MBZ;
   int slab = 8;                                  // 8 block rows = 32 grid rows per slab
   if (slab > nby) slab = nby;
   const int nslab = (nby + slab - 1) / slab;
   const long long nblocks = (long long)nslab * nbx * slab * nbz;
   dim3 b(MBX * MBY * MBZ), g((unsigned)nblocks);
-  const bool hyb = P.flux_mode == FLUX_HYBRID;
-  if (visc && hyb) rhs_main_kernel<L, LV, true, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  if (visc && conv) rhs_main_kernel<L, LV, true, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
   else if (visc) rhs_main_kernel<L, LV, true, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
-  else if (hyb) rhs_main_kernel<L, LV, false, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
+  else if (conv) rhs_main_kernel<L, LV, false, true, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
   else rhs_main_kernel<L, LV, false, false, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab);
   return 1;
 }
 
-template <int L, int LV, int R>
-static int launch_shock_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
-  const bool visc = P.visc_law != VISC_NONE;
+template <int L, int R>
+static int launch_weno_T(const DevP& P, cudaStream_t st) {
+  if (P.flux_mode == FLUX_CENTRAL) return 0;
+  dim3 b(128);
   if (P.flux_mode == FLUX_HYBRID) {
-    dim3 b(128), g(148 * 8);
-    if (visc) rhs_shock_kernel<L, LV, R, true, false><<<g, b, 0, st>>>(P, sa);
-    else rhs_shock_kernel<L, LV, R, false, false><<<g, b, 0, st>>>(P, sa);
-    return 1;
+    dim3 g(148 * 8);
+    weno_kernel<0, L, R, false><<<g, b, 0, st>>>(P);
+    weno_kernel<1, L, R, false><<<g, b, 0, st>>>(P);
+    weno_kernel<2, L, R, false><<<g, b, 0, st>>>(P);
+  } else {
+    const long long a = (long long)P.nx * P.ny * P.nz;
+    auto blocks = [&](long long extra) { return dim3((unsigned)((a + extra + 127) / 128)); };
+    weno_kernel<0, L, R, true><<<blocks((long long)P.ny * P.nz), b, 0, st>>>(P);
+    weno_kernel<1, L, R, true><<<blocks((long long)P.nx * P.nz), b, 0, st>>>(P);
+    weno_kernel<2, L, R, true><<<blocks((long long)P.nx * P.ny), b, 0, st>>>(P);
   }
-  if (P.flux_mode == FLUX_WENO) {
-    const long long nb = (P.N + 127) / 128;
-    dim3 b(128), g((unsigned)nb);
-    if (visc) rhs_shock_kernel<L, LV, R, true, true><<<g, b, 0, st>>>(P, sa);
-    else rhs_shock_kernel<L, LV, R, false, true><<<g, b, 0, st>>>(P, sa);
-    return 1;
-  }
-  return 0;
+  return 3;
+}
+
+static int launch_apply_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+  if (P.flux_mode == FLUX_CENTRAL) return 0;
+  dim3 b(256);
+  if (P.flux_mode == FLUX_HYBRID) rhs_apply_kernel<false><<<dim3(148 * 8), b, 0, st>>>(P, sa);
+  else rhs_apply_kernel<true><<<dim3((unsigned)((P.N + 255) / 256)), b, 0, st>>>(P, sa);
+  return 1;
 }
 
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
@@ -486,9 +531,10 @@ int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cu
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
   return launch_main_T<3, 3, 3>(P, sa, st);
 }
-int launch_rhs_shock(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
+int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
-  return launch_shock_T<3, 3, 3>(P, sa, st);
+  return launch_weno_T<3, 3>(P, st);
 }
+int launch_rhs_apply(const DevP& P, const StageArgs& sa, cudaStream_t st) { return launch_apply_T(P, sa, st); }
 
 }  // namespace streams

@@ -44,8 +44,10 @@ def check_case(S, case, nsteps, tol_rhs=TOL_RHS, tol_step=TOL_STEP, expect_activ
         frac = float(mk_o.mean())
         if expect_activation is not None:
             assert expect_activation[0] <= frac <= expect_activation[1], frac
-        flagged, shock = gpu.get_activation()
+        flagged, shock, ifaces = gpu.get_activation()
         assert flagged == int(mk_o.sum())
+        # every flagged interface is on exactly one work list (oracle: nd + 1 interfaces per pencil)
+        assert ifaces == [int(ora.interface_flags(d).sum()) for d in range(3)]
     # nsteps RK3 steps
     dt_g, t_g = gpu.step(nsteps)
     dt_o, t_o = ora.step(nsteps)
