@@ -22,7 +22,7 @@ struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
   size_t N;
-  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_list, off_ilist, off_dF, off_counters, off_R,
+  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_dF, off_counters, off_R,
       off_metrics, off_scal, total;
   int nq;
 };
@@ -90,9 +90,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.off_div = take(S.fs * 8);
   S.off_theta = take(S.N * 8);
   S.off_mask = take(S.fs);
-  S.off_nflag = take(hyb ? S.N : 256);
-  S.off_list = take(hyb ? S.N * 4 : 256);
-  S.off_ilist = take(hyb ? 3 * S.fs * 4 : 256);
+  S.off_nflag = take(hyb ? S.fs : 256);
   S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
   S.off_counters = take(C_COUNT * 4);
   S.off_R = take(5 * S.N * 8);
@@ -232,17 +230,16 @@ int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   return STREAMS_OK;
 }
 
-// the RHS (+ update) of one stage: fused central/viscous pass over all nodes, then the WENO fluxes of the
-// flagged interfaces and their application
+// the RHS (+ update) of one stage: the WENO flux corrections of the flagged interfaces first (they read the
+// primitives only), then the fused central / viscous / correction / update pass over all nodes
 int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
+  int b = 0;
+  if (ctx->scheme.flux_mode != STREAMS_FLUX_CENTRAL)
+    b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
   const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
-  if (a < 0) return -1;
-  if (ctx->scheme.flux_mode == STREAMS_FLUX_CENTRAL) return a;
-  const int b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
-  const int c = timed(ctx, STREAMS_K_APPLY, [&] { return launch_rhs_apply(P, sa, st); });
-  return (b < 0 || c < 0) ? -1 : a + b + c;
+  return (a < 0 || b < 0) ? -1 : a + b;
 }
 
 }  // namespace
@@ -288,8 +285,6 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.theta = (double*)(ctx->base + S.off_theta);
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
   P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
-  P.list = (int*)(ctx->base + S.off_list);
-  for (int d = 0; d < 3; ++d) P.ilist[d] = (int*)(ctx->base + S.off_ilist) + (size_t)d * S.fs;
   P.dF = (double*)(ctx->base + S.off_dF);
   P.counters = (int*)(ctx->base + S.off_counters);
   P.R = (double*)(ctx->base + S.off_R);

@@ -183,75 +183,94 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
 
 // ---------------------------------------------------------------------------------------------
 // Interface flags (O2 / S5): interface n+1/2 along d uses WENO iff any node of its 2r-node
-// stencil {n-r+1..n+r} is flagged.  Per interior node the six adjacent interfaces are packed in a
-// byte (bit 2d: minus side, bit 2d+1: plus side).  Three kinds of work lists are built from it:
-//   list      nodes with any bit set (consumed by rhs_apply_kernel),
-//   ilist[d]  flagged interfaces of direction d, each named by the padded index of its left node and
-//             owned by exactly one thread: the node on its left, or - for the interface below the first
-//             node of a pencil - that first node (consumed by weno_kernel).
-// Appends are aggregated per block (one atomic per list per block); the order inside a list is
-// irrelevant, every entry is processed independently and writes its own slot.
+// stencil {n-r+1..n+r} is flagged.  Per interior node the six adjacent interfaces are packed in a byte
+// (bit 2d: minus side, bit 2d+1: plus side), stored at the node's padded index.
+// One thread handles 8 consecutive x nodes as one 64-bit word of 0/1 mask bytes: the y / z windows are
+// ORs of 64-bit loads, the x window is an OR of byte-shifted words (SWAR), so the whole kernel is ~15
+// 8-byte loads per 8 nodes and no per-node atomics.  It also counts, per evaluation, flagged nodes,
+// nodes next to a flagged interface and flagged interfaces per direction (the paper's "WENO
+// activation"): warp-shuffle sums, one atomic per counter per block.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long ldw(const unsigned char* p) {
+  return *reinterpret_cast<const unsigned long long*>(p);
+}
+// bytes of `cur` shifted so that byte b holds the mask of node b + m (|m| < 8); prev / next are the
+// neighbouring words along x
+__device__ __forceinline__ unsigned long long xshift(unsigned long long prev, unsigned long long cur,
+                                                     unsigned long long next, int m) {
+  if (m == 0) return cur;
+  if (m > 0) return (cur >> (8 * m)) | (next << (64 - 8 * m));
+  return (cur << (-8 * m)) | (prev >> (64 + 8 * m));
+}
+
 template <int R>
-__global__ void __launch_bounds__(256) flags_kernel(const DevP P) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  const bool in = (i < P.nx && j < P.ny);
-  unsigned f = 0, own = 0;
-  long long o = 0, n = 0;
-  const long long st[3] = {1, P.sy, P.sz};
-  if (in) {
-    n = pidx(P, i, j, k);
-    o = iidx(P, i, j, k);
-    own = P.mask[n];
+__global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long nwords = (long long)nwx * P.ny * P.nz;
+  int cnt[5] = {0, 0, 0, 0, 0};      // flagged nodes, shock nodes, interfaces x, y, z
+  if (t < nwords) {
+    const int iw = (int)(t % nwx);
+    const long long t2 = t / nwx;
+    const int j = (int)(t2 % P.ny), k = (int)(t2 / P.ny);
+    const int i0 = iw * 8;
+    const long long n0 = pidx(P, i0, j, k);
+    const unsigned char* m = P.mask + n0;
+    const int nvalid = min(8, P.nx - i0);
+    const unsigned long long valid = nvalid == 8 ? ~0ull : ((1ull << (8 * nvalid)) - 1ull);
+    const unsigned long long cur = ldw(m), prev = ldw(m - 8);
+    const unsigned long long next = (i0 + 8 < P.nx + P.ng) ? ldw(m + 8) : 0ull;
+    unsigned long long lo[3], hi[3];
+    {
+      unsigned long long mid = cur;
+#pragma unroll
+      for (int q = 1; q <= R - 1; ++q) mid |= xshift(prev, cur, next, q) | xshift(prev, cur, next, -q);
+      lo[0] = mid | xshift(prev, cur, next, -R);
+      hi[0] = mid | xshift(prev, cur, next, R);
+    }
+    const long long st[3] = {1, P.sy, P.sz};
+#pragma unroll
+    for (int d = 1; d < 3; ++d) {
+      unsigned long long mid = cur;
+#pragma unroll
+      for (int q = 1; q <= R - 1; ++q) mid |= ldw(m + q * st[d]) | ldw(m - q * st[d]);
+      lo[d] = mid | ldw(m - R * st[d]);
+      hi[d] = mid | ldw(m + R * st[d]);
+    }
+    unsigned long long nf = 0ull, any = 0ull;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      unsigned mid = 0;
-#pragma unroll
-      for (int m = -R + 1; m <= R - 1; ++m) mid |= P.mask[n + m * st[d]];
-      const unsigned lo = mid | P.mask[n - R * st[d]];
-      const unsigned hi = mid | P.mask[n + R * st[d]];
-      f |= (lo ? 1u : 0u) << (2 * d);
-      f |= (hi ? 1u : 0u) << (2 * d + 1);
+      lo[d] &= valid & 0x0101010101010101ull;
+      hi[d] &= valid & 0x0101010101010101ull;
+      nf |= (lo[d] << (2 * d)) | (hi[d] << (2 * d + 1));
+      any |= lo[d] | hi[d];
     }
-    P.nflag[o] = (unsigned char)f;
+    *reinterpret_cast<unsigned long long*>(P.nflag + n0) = nf;
+    cnt[0] = __popcll(cur & valid & 0x0101010101010101ull);
+    cnt[1] = __popcll(any);
+    // every interface is counted by its left node; the one below the first node of a pencil by that node
+    cnt[2] = __popcll(hi[0]) + (i0 == 0 ? (int)(lo[0] & 1ull) : 0);
+    cnt[3] = __popcll(hi[1]) + (j == 0 ? __popcll(lo[1]) : 0);
+    cnt[4] = __popcll(hi[2]) + (k == 0 ? __popcll(lo[2]) : 0);
   }
-  // categories: 0 node list; 1..3 plus-side interface of x, y, z; 4..6 minus-side interface of the first
-  // node of a pencil in x, y, z; 7 flagged nodes (count only)
-  const bool want[8] = {f != 0, (f & 2u) != 0, (f & 8u) != 0, (f & 32u) != 0,
-                        i == 0 && (f & 1u) != 0, j == 0 && (f & 4u) != 0, k == 0 && (f & 16u) != 0, own != 0};
-  __shared__ int s_cnt[8][8];
-  __shared__ int s_base[8];
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-  const int lane = tid & 31, wid = tid >> 5;
-  unsigned bal[8];
+  __shared__ int s_cnt[5];
+  if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+  __syncthreads();
 #pragma unroll
-  for (int c = 0; c < 8; ++c) {
-    bal[c] = __ballot_sync(0xffffffffu, want[c]);
-    if (lane == 0) s_cnt[c][wid] = __popc(bal[c]);
+  for (int c = 0; c < 5; ++c) {
+    int v = cnt[c];
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(&s_cnt[c], v);
   }
   __syncthreads();
-  if (tid < 8) {
-    int tot = 0;
-    for (int w = 0; w < 8; ++w) { const int c = s_cnt[tid][w]; s_cnt[tid][w] = tot; tot += c; }
-    int base = 0;
-    if (tot) {
-      unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS);
-      const int d = (tid - 1) % 3;
-      if (tid == 0) { base = atomicAdd(&P.counters[C_NSHOCK], tot); atomicAdd(&cum[0], (unsigned long long)tot); }
-      else if (tid == 7) { atomicAdd(&P.counters[C_NFLAGGED], tot); atomicAdd(&cum[1], (unsigned long long)tot); }
-      else { base = atomicAdd(&P.counters[C_NIFACE + d], tot); atomicAdd(&cum[3 + d], (unsigned long long)tot); }
-    }
-    s_base[tid] = base;
-  }
-  __syncthreads();
-  const unsigned lt = (1u << lane) - 1u;
-  if (want[0]) P.list[s_base[0] + s_cnt[0][wid] + __popc(bal[0] & lt)] = (int)o;
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    if (want[1 + d]) P.ilist[d][s_base[1 + d] + s_cnt[1 + d][wid] + __popc(bal[1 + d] & lt)] = (int)n;
-    if (want[4 + d]) P.ilist[d][s_base[4 + d] + s_cnt[4 + d][wid] + __popc(bal[4 + d] & lt)] = (int)(n - st[d]);
+  if (threadIdx.x < 5 && s_cnt[threadIdx.x]) {
+    const int c = threadIdx.x, v = s_cnt[c];
+    unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS);
+    // counters: C_NFLAGGED, C_NSHOCK, C_NIFACE + d; totals: [0] shock, [1] flagged, [3 + d] interfaces
+    const int slot = c == 0 ? C_NFLAGGED : (c == 1 ? C_NSHOCK : C_NIFACE + (c - 2));
+    const int cslot = c == 0 ? 1 : (c == 1 ? 0 : 3 + (c - 2));
+    atomicAdd(&P.counters[slot], v);
+    atomicAdd(&cum[cslot], (unsigned long long)v);
   }
 }
 
@@ -362,13 +381,15 @@ int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st) 
 }
 
 int launch_flags(const DevP& P, int r, cudaStream_t st) {
-  dim3 b(64, 4), g = grid2d(P, b);
+  const int nwx = (P.nx + 7) / 8;
+  const long long nwords = (long long)nwx * P.ny * P.nz;
+  dim3 b(256), g((unsigned)((nwords + 255) / 256));
   reset_counters_kernel<<<1, 1, 0, st>>>(P);
   switch (r) {
-    case 1: flags_kernel<1><<<g, b, 0, st>>>(P); break;
-    case 2: flags_kernel<2><<<g, b, 0, st>>>(P); break;
-    case 3: flags_kernel<3><<<g, b, 0, st>>>(P); break;
-    default: flags_kernel<4><<<g, b, 0, st>>>(P); break;
+    case 1: flags_kernel<1><<<g, b, 0, st>>>(P, nwx); break;
+    case 2: flags_kernel<2><<<g, b, 0, st>>>(P, nwx); break;
+    case 3: flags_kernel<3><<<g, b, 0, st>>>(P, nwx); break;
+    default: flags_kernel<4><<<g, b, 0, st>>>(P, nwx); break;
   }
   return 2;
 }

@@ -20,12 +20,11 @@ int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st);
 int launch_flags(const DevP& P, int r, cudaStream_t st);
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);
 int launch_step_end(const DevP& P, cudaStream_t st);
-// The fused RHS + update (all nodes), the per-interface WENO fluxes and their application; each returns the
-// number of launches (0 when the flux mode does not need it) or < 0 if the (L, Lv, r) combination is not
-// instantiated.
-int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
+// The per-interface WENO flux corrections (run first) and the fused RHS + update over all nodes; each
+// returns the number of launches (0 when the flux mode does not need it) or < 0 if the (L, Lv, r)
+// combination is not instantiated.
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st);
-int launch_rhs_apply(const DevP& P, const StageArgs& sa, cudaStream_t st);
+int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law);
 
 }  // namespace streams
