@@ -304,6 +304,15 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.t_wall_lo = grid->t_wall_lo; P.t_wall_hi = grid->t_wall_hi;
   P.bc_x = grid->bc_x; P.bc_y_lo = grid->bc_y_lo; P.bc_y_hi = grid->bc_y_hi; P.bc_z = grid->bc_z;
   P.visc_law = gas->visc_law; P.flux_mode = scheme->flux_mode;
+  {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+      delete ctx;
+      return fail(nullptr, STREAMS_ECUDA, "cannot query the device");
+    }
+    P.nsm = nsm;
+  }
 
   std::vector<double> eyc, eyv, eyyv;
   build_metrics(ctx, grid->y_nodes, eyc, eyv, eyyv);

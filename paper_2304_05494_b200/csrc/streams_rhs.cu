@@ -18,213 +18,388 @@ namespace streams {
 struct VAcc {          // velocity / temperature / viscosity / dilatation derivatives at a node
   double g[3][3];      // g[a][b] = d u_a / d x_b
   double gT[3], gmu[3], gdiv[3];
-  double lap[3], lapT;
+  double lap[3], lapT; // sum over directions of the second-derivative stencils, centre term applied at the end
 };
 
 template <int D>
 __device__ __forceinline__ double pick(double a, double b, double c) { return D == 0 ? a : (D == 1 ? b : c); }
 
+// fields of the marching kernel, in the order of DevP::q (F_DIV is DevP::div)
+enum { F_U = 0, F_V = 1, F_W = 2, F_H = 3, F_P = 4, F_RHO = 5, F_T = 6, F_MU = 7, F_DIV = 8 };
+
+__device__ __forceinline__ const double* field_ptr(const DevP& P, int f) { return f < 8 ? P.q + f * P.fs : P.div; }
+
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+}
+// copies 8 bytes when `take`, writes zeros (and reads nothing) otherwise
+__device__ __forceinline__ void cp_async8_zfill(void* smem_dst, const void* gsrc, bool take) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const unsigned n = take ? 8u : 0u;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(s), "l"(gsrc), "r"(n) : "memory");
+}
+// a load the compiler may not sink to its first use
+__device__ __forceinline__ unsigned ld_u8_now(const unsigned char* p) {
+  unsigned v;
+  asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// per-direction stencil coefficients with the metric folded in
+struct DirCoef {
+  double kc[3];        // convective: a_l / 4            (mass flux pairs; the metric multiplies the sums)
+  double ap[3];        // pressure:   a_l
+  double met_c;        // convective metric
+  double av[3];        // viscous first derivative:  a_l * metric
+  double bv[3];        // viscous second derivative: b_l * metric^2
+};
+
 // ---------------------------------------------------------------------------------------------
-// One direction at one node.  Convective part in pair-difference form: with
-//   Pq(a,b) = (rho_a+rho_b)(ud_a+ud_b)(phi_a+phi_b)  the flux difference telescopes to
-//   f_{n+1/2} - f_{n-1/2} = 1/4 sum_l a_l [P(n, n+l) - P(n-l, n)]   (+ sum_l a_l (p_{n+l} - p_{n-l}))
-// which is the same sum as the oracle's interface-flux form (O1) in another order.
-// Viscous part: first derivatives of u, v, w, T, mu, div and second derivatives of u, v, w, T.
-// c0 = (rho, u, v, w, H, p) at the node.
+// One direction at one node; G(f, o) returns field f at offset o (-3..3) along the direction.
+// Convective part (O1) in pair-difference form: with m(a,b) = (a_l/4)(rho_a+rho_b)(ud_a+ud_b),
+//   f_{n+1/2} - f_{n-1/2} = sum_l [ m(n,n+l)(phi_n+phi_{n+l}) - m(n-l,n)(phi_{n-l}+phi_n) ]
+//                         = phi_n S0 + sum_l [ m(n,n+l) phi_{n+l} - m(n-l,n) phi_{n-l} ],  S0 = sum_l [m(n,n+l) - m(n-l,n)]
+// (the same sum as the oracle's interface-flux form, regrouped), plus sum_l a_l (p_{n+l} - p_{n-l}) on the
+// D-momentum.  Viscous part (O4): first derivatives of u, v, w, T, mu, div; second-derivative sums
+// sum_l b_l (f_{+l} + f_{-l}) of u, v, w, T (the centre term -2 f_0 sum b_l is applied once by the caller).
+// c0 = (u, v, w, H, p, rho) at the node, alr[l] = kc[l] * rho_0.
 // ---------------------------------------------------------------------------------------------
-template <int D, int L, int LV, bool CONV, bool VISC>
-__device__ __forceinline__ void dir_terms(const DevP& P, long long n, long long s, double met_c, double met_v,
-                                          double eyy, const double c0[6], double T0, double r[5], VAcc& V) {
-  const double* __restrict__ RHO = P.q + Q_RHO * P.fs + n;
-  const double* __restrict__ U = P.q + Q_U * P.fs + n;
-  const double* __restrict__ Vv = P.q + Q_V * P.fs + n;
-  const double* __restrict__ W = P.q + Q_W * P.fs + n;
-  const double* __restrict__ Hh = P.q + Q_H * P.fs + n;
-  const double* __restrict__ Pp = P.q + Q_P * P.fs + n;
-  const double* __restrict__ Tt = P.q + Q_T * P.fs + n;
-  const double* __restrict__ Mu = P.q + Q_MU * P.fs + n;
-  const double* __restrict__ Dv = P.div + n;
+template <int D, int L, int LV, bool CONV, bool VISC, class G>
+__device__ __forceinline__ void dir_terms(const G& g, const DirCoef& c, const double c0[6], const double alr[3],
+                                          double eyr, double r[5], VAcc& V) {
   constexpr int LC = CONV ? L : 0;
   constexpr int LVV = VISC ? LV : 0;
   constexpr int LM = LC > LVV ? LC : LVV;
-  double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, SP = 0.0;
+  double S0 = 0.0, S[4] = {0.0, 0.0, 0.0, 0.0}, SP = 0.0;
   double d1[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // u v w T mu div
   double d2[4] = {0.0, 0.0, 0.0, 0.0};             // u v w T
-  const double ud0 = pick<D>(c0[1], c0[2], c0[3]);
+  const double ud0 = pick<D>(c0[0], c0[1], c0[2]);
 #pragma unroll
   for (int l = 1; l <= LM; ++l) {
-    const long long off = l * s;
-    const double ub = U[off], ua = U[-off];
-    const double vb = Vv[off], va = Vv[-off];
-    const double wb = W[off], wa = W[-off];
-    if (l <= LC) {
-      const double rb = RHO[off], ra = RHO[-off];
-      const double hb = Hh[off], ha = Hh[-off];
-      const double pb = Pp[off], pa = Pp[-off];
-      const double mb = (c0[0] + rb) * (ud0 + pick<D>(ub, vb, wb));
-      const double ma = (ra + c0[0]) * (pick<D>(ua, va, wa) + ud0);
-      const double al = P.a1[l - 1];
-      S[0] += al * (mb - ma);
-      S[1] += al * (mb * (c0[1] + ub) - ma * (ua + c0[1]));
-      S[2] += al * (mb * (c0[2] + vb) - ma * (va + c0[2]));
-      S[3] += al * (mb * (c0[3] + wb) - ma * (wa + c0[3]));
-      S[4] += al * (mb * (c0[4] + hb) - ma * (ha + c0[4]));
-      SP += al * (pb - pa);
+    const double ub = g(F_U, l), ua = g(F_U, -l);
+    const double vb = g(F_V, l), va = g(F_V, -l);
+    const double wb = g(F_W, l), wa = g(F_W, -l);
+    if constexpr (CONV) if (l <= LC) {
+      const double rb = g(F_RHO, l), ra = g(F_RHO, -l);
+      const double hb = g(F_H, l), ha = g(F_H, -l);
+      const double pb = g(F_P, l), pa = g(F_P, -l);
+      const double mb = fma(c.kc[l - 1], rb, alr[l - 1]) * (ud0 + pick<D>(ub, vb, wb));
+      const double ma = fma(c.kc[l - 1], ra, alr[l - 1]) * (pick<D>(ua, va, wa) + ud0);
+      S0 += mb - ma;
+      S[0] = fma(mb, ub, S[0]); S[0] = fma(-ma, ua, S[0]);
+      S[1] = fma(mb, vb, S[1]); S[1] = fma(-ma, va, S[1]);
+      S[2] = fma(mb, wb, S[2]); S[2] = fma(-ma, wa, S[2]);
+      S[3] = fma(mb, hb, S[3]); S[3] = fma(-ma, ha, S[3]);
+      SP = fma(c.ap[l - 1], pb - pa, SP);
     }
-    if (l <= LVV) {
-      const double tb = Tt[off], ta = Tt[-off];
-      const double a = P.a1v[l - 1], b = P.b2v[l - 1];
-      d1[0] += a * (ub - ua);  d2[0] += b * ((ub - 2.0 * c0[1]) + ua);
-      d1[1] += a * (vb - va);  d2[1] += b * ((vb - 2.0 * c0[2]) + va);
-      d1[2] += a * (wb - wa);  d2[2] += b * ((wb - 2.0 * c0[3]) + wa);
-      d1[3] += a * (tb - ta);  d2[3] += b * ((tb - 2.0 * T0) + ta);
-      d1[4] += a * (Mu[off] - Mu[-off]);
-      d1[5] += a * (Dv[off] - Dv[-off]);
+    if constexpr (VISC) if (l <= LVV) {
+      const double tb = g(F_T, l), ta = g(F_T, -l);
+      const double a = c.av[l - 1], b = c.bv[l - 1];
+      d1[0] = fma(a, ub - ua, d1[0]);  d2[0] = fma(b, ub + ua, d2[0]);
+      d1[1] = fma(a, vb - va, d1[1]);  d2[1] = fma(b, vb + va, d2[1]);
+      d1[2] = fma(a, wb - wa, d1[2]);  d2[2] = fma(b, wb + wa, d2[2]);
+      d1[3] = fma(a, tb - ta, d1[3]);  d2[3] = fma(b, tb + ta, d2[3]);
+      d1[4] = fma(a, g(F_MU, l) - g(F_MU, -l), d1[4]);
+      d1[5] = fma(a, g(F_DIV, l) - g(F_DIV, -l), d1[5]);
     }
   }
   if (CONV) {
-    r[0] -= met_c * (0.5 * S[0]);
-    r[1] -= met_c * (0.25 * S[1]);
-    r[2] -= met_c * (0.25 * S[2]);
-    r[3] -= met_c * (0.25 * S[3]);
-    r[4] -= met_c * (0.25 * S[4]);
-    r[1 + D] -= met_c * SP;
+    r[0] = fma(-2.0 * c.met_c, S0, r[0]);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) r[1 + q] = fma(-c.met_c, fma(c0[q], S0, S[q]), r[1 + q]);
+    r[1 + D] = fma(-c.met_c, SP, r[1 + D]);
   }
   if (VISC) {
-    const double m2 = met_v * met_v;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-      V.g[a][D] = d1[a] * met_v;
-      double sec = d2[a] * m2;
-      if (D == 1) sec += eyy * d1[a];
-      V.lap[a] += sec;
+      V.g[a][D] = d1[a];
+      V.lap[a] += (D == 1) ? fma(eyr, d1[a], d2[a]) : d2[a];
     }
-    V.gT[D] = d1[3] * met_v;
-    double secT = d2[3] * m2;
-    if (D == 1) secT += eyy * d1[3];
-    V.lapT += secT;
-    V.gmu[D] = d1[4] * met_v;
-    V.gdiv[D] = d1[5] * met_v;
+    V.gT[D] = d1[3];
+    V.lapT += (D == 1) ? fma(eyr, d1[3], d2[3]) : d2[3];
+    V.gmu[D] = d1[4];
+    V.gdiv[D] = d1[5];
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Viscous combination (O4), R store and RK update (O5) for one node.
+// Viscous combination (O4) for one node; c0 = (u, v, w, ...).
 // ---------------------------------------------------------------------------------------------
-template <bool VISC, bool WENO, bool DENSE>
-__device__ __forceinline__ void finish(const DevP& P, const StageArgs& sa, long long n, long long o, double met_y,
-                                       const double c0[6], double mu0, double r[5], const VAcc& V) {
-  if (VISC) {
-    const double dv = (V.g[0][0] + V.g[1][1]) + V.g[2][2];
-    double vm[3];
+__device__ __forceinline__ void viscous_combine(const DevP& P, const double c0[6], double mu0, double r[5], const VAcc& V) {
+  const double dv = (V.g[0][0] + V.g[1][1]) + V.g[2][2];
+  const double s01 = V.g[0][1] + V.g[1][0], s02 = V.g[0][2] + V.g[2][0], s12 = V.g[1][2] + V.g[2][1];
+  const double s[3][3] = {{2.0 * V.g[0][0], s01, s02}, {s01, 2.0 * V.g[1][1], s12}, {s02, s12, 2.0 * V.g[2][2]}};
+  const double tdv = (2.0 / 3.0) * dv;
+  double vm[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      double cross = 0.0;
-#pragma unroll
-      for (int b = 0; b < 3; ++b) cross += V.gmu[b] * (V.g[a][b] + V.g[b][a]);
-      vm[a] = mu0 * V.lap[a] + cross - (2.0 / 3.0) * V.gmu[a] * dv + mu0 * V.gdiv[a] * (1.0 / 3.0);
-    }
-    const double s01 = V.g[0][1] + V.g[1][0], s02 = V.g[0][2] + V.g[2][0], s12 = V.g[1][2] + V.g[2][1];
-    const double phi = mu0 * (2.0 * (V.g[0][0] * V.g[0][0] + V.g[1][1] * V.g[1][1] + V.g[2][2] * V.g[2][2]) +
-                              s01 * s01 + s02 * s02 + s12 * s12 - (2.0 / 3.0) * dv * dv);
-    const double cond = P.kfac * (mu0 * V.lapT + (V.gmu[0] * V.gT[0] + V.gmu[1] * V.gT[1] + V.gmu[2] * V.gT[2]));
-    r[1] += vm[0];
-    r[2] += vm[1];
-    r[3] += vm[2];
-    r[4] += (c0[1] * vm[0] + c0[2] * vm[1] + c0[3] * vm[2]) + phi + cond;
+  for (int a = 0; a < 3; ++a) {
+    double cross = V.gmu[0] * s[a][0];
+    cross = fma(V.gmu[1], s[a][1], cross);
+    cross = fma(V.gmu[2], s[a][2], cross);
+    cross = fma(-V.gmu[a], tdv, cross);
+    vm[a] = fma(mu0, fma(V.gdiv[a], 1.0 / 3.0, V.lap[a]), cross);
   }
-  if (WENO) {
-    // flux corrections of the flagged interfaces around this node (written by weno_kernel)
-    const unsigned fl = DENSE ? 0x3fu : (unsigned)P.nflag[n];
-    if (fl) {
-      const long long st[3] = {1, P.sy, P.sz};
-      const double met[3] = {P.inv_dx, met_y, P.inv_dz};
+  double ph = V.g[0][0] * V.g[0][0];
+  ph = fma(V.g[1][1], V.g[1][1], ph);
+  ph = fma(V.g[2][2], V.g[2][2], ph);
+  ph = ph + ph;
+  ph = fma(s01, s01, ph);
+  ph = fma(s02, s02, ph);
+  ph = fma(s12, s12, ph);
+  ph = fma(-tdv, dv, ph);
+  double cond = mu0 * V.lapT;
+  cond = fma(V.gmu[0], V.gT[0], cond);
+  cond = fma(V.gmu[1], V.gT[1], cond);
+  cond = fma(V.gmu[2], V.gT[2], cond);
+  r[1] += vm[0];
+  r[2] += vm[1];
+  r[3] += vm[2];
+  double e = fma(mu0, ph, P.kfac * cond);
+  e = fma(c0[0], vm[0], e);
+  e = fma(c0[1], vm[1], e);
+  e = fma(c0[2], vm[2], e);
+  r[4] += e;
+}
+
+// ---------------------------------------------------------------------------------------------
+// rhs_march_kernel (a4-a8 in one pass).  A block owns a 32 x TY tile of (x, y) and marches through a chunk
+// of z planes (2.5-D blocking):
+//   - z neighbours: every thread keeps the 7-plane column (k-3 .. k+3) of its node for all fields in
+//     registers; plane k+4 is fetched one iteration ahead (plain coalesced loads, consumed at the ring shift);
+//   - x / y neighbours: the centre plane of every field sits in shared memory with its 3-wide halo
+//     (interior written from the registers, halo copied with cp.async one iteration ahead, two buffers, one
+//     barrier per plane); all stencil offsets are compile-time immediates;
+//   - RK operands (previous-stage R, w) are staged with cp.async at the start of the iteration and consumed
+//     at its end, so no global-memory latency is exposed in the loop.
+// Threads of a ragged tile beyond the interior load (clamped) ghost nodes, so the tile's shared-memory
+// plane is correct wherever an interior thread reads it; they do not store.
+// ---------------------------------------------------------------------------------------------
+constexpr int MTX = 32;
+
+template <int TY>
+struct MarchGeom {
+  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (3 used), rows stay 16 B aligned
+  static constexpr int ROWS = TY + 6;
+  static constexpr int PLANE = ROW * ROWS;       // doubles per field per buffer
+  static constexpr int NT = MTX * TY;
+  static constexpr int NH = 6 * TY + 6 * MTX;    // halo nodes of a plane (corners are never read)
+  static constexpr int HE = (NH + NT - 1) / NT;  // halo nodes per thread
+};
+
+template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
+__global__ void __launch_bounds__(MTX * TY, (TY >= 8 ? 1 : 2))
+rhs_march_kernel(const DevP P, const StageArgs sa, int nbx, int nby, int kz) {
+  using G = MarchGeom<TY>;
+  constexpr int NF = VISC ? 9 : 6;
+  constexpr int NG = 3;
+  static_assert(L <= NG && LV <= NG, "ring depth");
+  extern __shared__ double smem[];
+  double* buf = smem;                              // [2][NF][PLANE]  centre planes with halo
+  double* epi = buf + 2 * NF * G::PLANE;           // [10][NT]         previous-stage R, w of this plane
+  double* nxs = epi + 10 * G::NT;                  // [NF][NT]         plane k+4 of this thread's column
+  double* dfs = nxs + NF * G::NT;                  // [30][NT]         flux corrections around this node (WENO)
+
+  const int tid = threadIdx.x;
+  const int tx = tid & 31, ty = tid >> 5;
+  int bid = blockIdx.x;
+  const int bx = bid % nbx; bid /= nbx;
+  const int by = bid % nby;
+  const int bc = bid / nby;
+  const int i0 = bx * MTX, j0 = by * TY;
+  const int kb = bc * kz, ke = min(P.nz, kb + kz);
+  if (kb >= ke) return;
+  const int i = i0 + tx, j = j0 + ty;
+  const bool active = i < P.nx && j < P.ny;
+  const int ic = min(i, P.nx + P.ng - 1), jc = min(j, P.ny + P.ng - 1);
+  const long long ncol = pidx(P, ic, jc, 0);       // this thread's column at k = 0
+  const long long ocol = (long long)j * P.nx + i;  // interior index at k = 0 (active threads only)
+  const int s0 = (ty + 3) * G::ROW + tx + 4;       // this node in a shared-memory plane
+
+  // halo nodes handled by this thread: offset in a padded plane, offset in a shared-memory plane
+  int hsrc[G::HE], hdst[G::HE];
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        const unsigned b = (fl >> (2 * d)) & 3u;
-        if (b == 0) continue;
-        const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+  for (int h = 0; h < G::HE; ++h) {
+    const int e = tid + h * G::NT;
+    int xo, yo;
+    if (e < 6 * TY) { const int rr = e / 6, c = e % 6; yo = rr; xo = c < 3 ? c - 3 : MTX + c - 3; }
+    else { const int e2 = e - 6 * TY, hr = e2 / MTX; xo = e2 % MTX; yo = hr < 3 ? hr - 3 : TY + hr - 3; }
+    const int ih = min(i0 + xo, P.nx + P.ng - 1), jh = min(j0 + yo, P.ny + P.ng - 1);
+    hsrc[h] = e < G::NH ? (int)((long long)(jh + P.ng) * P.sy + ih + P.ox) : -1;
+    hdst[h] = (yo + 3) * G::ROW + 4 + xo;
+  }
+
+  // y metrics of this row (constant along the march)
+  DirCoef cx, cy, cz;
+  const double eyc = P.eta_y_c[min(j, P.ny - 1)];
+  double eyv = 0.0, eyr = 0.0;
+  if (VISC) { eyv = P.eta_y_v[min(j, P.ny - 1)]; eyr = P.eta_yy_v[min(j, P.ny - 1)] / eyv; }
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const double fp = (b & 2u) ? f[q * P.fs] : 0.0;
-          const double fm = (b & 1u) ? f[q * P.fs - st[d]] : 0.0;
-          r[q] -= (fp - fm) * met[d];
+  for (int l = 0; l < 3; ++l) {
+    cx.kc[l] = cy.kc[l] = cz.kc[l] = 0.25 * P.a1[l];
+    cx.ap[l] = cy.ap[l] = cz.ap[l] = P.a1[l];
+    cx.av[l] = P.a1v[l] * P.inv_dx; cx.bv[l] = P.b2v[l] * (P.inv_dx * P.inv_dx);
+    cy.av[l] = P.a1v[l] * eyv;      cy.bv[l] = P.b2v[l] * (eyv * eyv);
+    cz.av[l] = P.a1v[l] * P.inv_dz; cz.bv[l] = P.b2v[l] * (P.inv_dz * P.inv_dz);
+  }
+  cx.met_c = P.inv_dx; cy.met_c = eyc; cz.met_c = P.inv_dz;
+  const double sb2 = -2.0 * (((cx.bv[0] + cx.bv[1]) + cx.bv[2]) + ((cy.bv[0] + cy.bv[1]) + cy.bv[2]) +
+                             ((cz.bv[0] + cz.bv[1]) + cz.bv[2]));
+  const double dt = sa.update_w ? P.scal[S_DT] : 0.0;
+
+  // ---- prologue: ring = planes kb-3 .. kb+3, halo of plane kb
+  double zr[NF][2 * NG + 1];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    const double* __restrict__ fp = field_ptr(P, f) + ncol + (long long)(kb - NG) * P.sz;
+#pragma unroll
+    for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
+  }
+  {
+    const long long pl = (long long)(kb + P.ng) * P.sz;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const double* __restrict__ fp = field_ptr(P, f) + pl;
+#pragma unroll
+      for (int h = 0; h < G::HE; ++h)
+        if (hsrc[h] >= 0) cp_async8(buf + f * G::PLANE + hdst[h], fp + hsrc[h]);
+    }
+    cp_async_commit();
+  }
+
+  for (int k = kb; k < ke; ++k) {
+    const int b = (k - kb) & 1;
+    double* __restrict__ sm = buf + b * NF * G::PLANE;
+    // (A) centre plane -> shared memory; halo of plane k has been in flight for one iteration
+#pragma unroll
+    for (int f = 0; f < NF; ++f) sm[f * G::PLANE + s0] = zr[f][NG];
+    cp_async_wait<0>();
+    __syncthreads();
+    // (B) start what the next iteration and this iteration's epilogue need
+    const long long n = ncol + (long long)k * P.sz;
+    const long long o = ocol + (long long)k * P.ny * P.nx;
+    unsigned fl = 0;
+    if (WENO) {
+      fl = CONV ? (active ? ld_u8_now(P.nflag + n) : 0u) : 0x3fu;
+    }
+    if (active) {
+      if (sa.read_prev) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) cp_async8(epi + q * G::NT + tid, P.R + q * P.N + o);
+      }
+      if (sa.update_w) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) cp_async8(epi + (5 + q) * G::NT + tid, P.w + q * P.fs + n);
+      }
+    }
+    {
+      // plane k+4 (clamped to the last ghost plane: the value is unused when it is beyond)
+      const int kn = min(k + NG + 1, P.nz + P.ng - 1);
+      const long long nn = ncol + (long long)kn * P.sz;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async8(nxs + f * G::NT + tid, field_ptr(P, f) + nn);
+    }
+    cp_async_commit();
+    if (k + 1 < ke) {
+      double* __restrict__ smn = buf + (b ^ 1) * NF * G::PLANE;
+      const long long pl = (long long)(k + 1 + P.ng) * P.sz;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const double* __restrict__ fp = field_ptr(P, f) + pl;
+#pragma unroll
+        for (int h = 0; h < G::HE; ++h)
+          if (hsrc[h] >= 0) cp_async8(smn + f * G::PLANE + hdst[h], fp + hsrc[h]);
+      }
+    }
+    cp_async_commit();
+    // flux corrections of the flagged interfaces around the nodes of this warp (third group: waited with
+    // the first at the epilogue; zero-filled where an interface is not flagged)
+    bool any_fl = false;
+    if (WENO) {
+      any_fl = __any_sync(0xffffffffu, fl != 0);
+      if (any_fl) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+          const long long sd = d == 0 ? 1 : (d == 1 ? P.sy : P.sz);
+          const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 0) * G::NT + tid, f + q * P.fs, (fl >> (2 * d + 1)) & 1u);
+            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 1) * G::NT + tid, f + q * P.fs - sd, (fl >> (2 * d)) & 1u);
+          }
         }
       }
     }
-  }
-  if (sa.update_w) {
-    const double dt = P.scal[S_DT];
+    cp_async_commit();
+
+    // (C) the right-hand side of this node
+    double c0[6];
 #pragma unroll
-    for (int q = 0; q < 5; ++q) {
-      double inc = sa.gam * r[q];
-      if (sa.read_prev) inc += sa.rhk * P.R[q * P.N + o];
-      double* wp = P.w + q * P.fs + n;
-      *wp = *wp + dt * inc;
+    for (int q = 0; q < 6; ++q) c0[q] = zr[q][NG];
+    double alr[3];
+#pragma unroll
+    for (int l = 0; l < 3; ++l) alr[l] = cx.kc[l] * c0[F_RHO];
+    double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    VAcc V;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { V.lap[a] = 0.0; }
+    V.lapT = 0.0;
+    {
+      const double* __restrict__ sc = sm + s0;
+      auto gx = [&](int f, int o2) { return sc[f * G::PLANE + o2]; };
+      dir_terms<0, L, LV, CONV, VISC>(gx, cx, c0, alr, 0.0, r, V);
+      auto gy = [&](int f, int o2) { return sc[f * G::PLANE + o2 * G::ROW]; };
+      dir_terms<1, L, LV, CONV, VISC>(gy, cy, c0, alr, eyr, r, V);
+      auto gz = [&](int f, int o2) { return zr[f][NG + o2]; };
+      dir_terms<2, L, LV, CONV, VISC>(gz, cz, c0, alr, 0.0, r, V);
+    }
+    if (VISC) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) V.lap[a] = fma(sb2, c0[a], V.lap[a]);
+      V.lapT = fma(sb2, zr[VISC ? F_T : 0][NG], V.lapT);
+      viscous_combine(P, c0, zr[VISC ? F_MU : 0][NG], r, V);
+    }
+
+    // (D) flux corrections of flagged interfaces, RK update, stores
+    cp_async_wait<0>();
+    if (active) {
+      if (WENO && any_fl) {
+        const double met[3] = {P.inv_dx, eyc, P.inv_dz};
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            const double fp = dfs[((d * 5 + q) * 2 + 0) * G::NT + tid];
+            const double fm = dfs[((d * 5 + q) * 2 + 1) * G::NT + tid];
+            r[q] = fma(-met[d], fp - fm, r[q]);
+          }
+        }
+      }
+      if (sa.update_w) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          double inc = sa.gam * r[q];
+          if (sa.read_prev) inc = fma(sa.rhk, epi[q * G::NT + tid], inc);
+          P.w[q * P.fs + n] = fma(dt, inc, epi[(5 + q) * G::NT + tid]);
+        }
+      }
+      if (sa.write_r) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sa.r_out[q * P.N + o] = r[q];
+      }
+    }
+
+    // (E) shift the ring
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+#pragma unroll
+      for (int m = 0; m < 2 * NG; ++m) zr[f][m] = zr[f][m + 1];
+      zr[f][2 * NG] = nxs[f * G::NT + tid];
     }
   }
-  if (sa.write_r) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) sa.r_out[q * P.N + o] = r[q];
-  }
-}
-
-__device__ __forceinline__ void load_centre(const DevP& P, long long n, double c0[6]) {
-  c0[0] = P.q[Q_RHO * P.fs + n];
-  c0[1] = P.q[Q_U * P.fs + n];
-  c0[2] = P.q[Q_V * P.fs + n];
-  c0[3] = P.q[Q_W * P.fs + n];
-  c0[4] = P.q[Q_H * P.fs + n];
-  c0[5] = P.q[Q_P * P.fs + n];
-}
-
-__device__ __forceinline__ void zero_vacc(VAcc& V) {
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    V.lap[a] = 0.0; V.gT[a] = 0.0; V.gmu[a] = 0.0; V.gdiv[a] = 0.0;
-#pragma unroll
-    for (int b = 0; b < 3; ++b) V.g[a][b] = 0.0;
-  }
-  V.lapT = 0.0;
-}
-
-// ---------------------------------------------------------------------------------------------
-// rhs_main_kernel: BX x BY x BZ nodes per block.  Blocks are numbered so that a slab of `slab`
-// block-rows in y is swept through all of z before the next slab starts: the 2 ng z-neighbour
-// planes of a slab then stay in L2.
-// ---------------------------------------------------------------------------------------------
-template <int L, int LV, bool VISC, bool CONV, bool WENO, int BX, int BY, int BZ>
-__global__ void __launch_bounds__(BX * BY * BZ) rhs_main_kernel(const DevP P, const StageArgs sa, int nbx, int nby,
-                                                               int nbz, int slab) {
-  // decode block id -> (bx, by, bz), slab-major
-  long long bid = blockIdx.x;
-  const long long per_slab = (long long)nbx * slab * nbz;
-  const int sl = (int)(bid / per_slab);
-  const int rows = min(slab, nby - sl * slab);
-  bid -= (long long)sl * per_slab;
-  // inside a slab: x fastest, then y (rows of this slab), then z
-  const int bx = (int)(bid % nbx);
-  const long long t = bid / nbx;
-  const int byl = (int)(t % rows);
-  const int bz = (int)(t / rows);
-  if (bz >= nbz) return;
-  const int tx = threadIdx.x % BX, ty = (threadIdx.x / BX) % BY, tz = threadIdx.x / (BX * BY);
-  const int i = bx * BX + tx, j = (sl * slab + byl) * BY + ty, k = bz * BZ + tz;
-  if (i >= P.nx || j >= P.ny || k >= P.nz) return;
-  const long long o = iidx(P, i, j, k);
-  const long long n = pidx(P, i, j, k);
-  double c0[6];
-  load_centre(P, n, c0);
-  double T0 = 0.0, mu0 = 0.0, eyv = 0.0, eyy = 0.0;
-  if (VISC) { T0 = P.q[Q_T * P.fs + n]; mu0 = P.q[Q_MU * P.fs + n]; eyv = P.eta_y_v[j]; eyy = P.eta_yy_v[j]; }
-  double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  VAcc V;
-  zero_vacc(V);
-  dir_terms<0, L, LV, CONV, VISC>(P, n, 1, P.inv_dx, P.inv_dx, 0.0, c0, T0, r, V);
-  const double eyc = P.eta_y_c[j];
-  dir_terms<1, L, LV, CONV, VISC>(P, n, P.sy, eyc, eyv, eyy, c0, T0, r, V);
-  dir_terms<2, L, LV, CONV, VISC>(P, n, P.sz, P.inv_dz, P.inv_dz, 0.0, c0, T0, r, V);
-  finish<VISC, WENO, !CONV>(P, sa, n, o, eyc, c0, mu0, r, V);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -518,20 +693,51 @@ __global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_kernel(const DevP
 }
 
 // -------------------------------------------------------------------------- launch
-constexpr int MBX = 32, MBY = 4, MBZ = 4;
+// z chunks per tile: enough blocks to fill every SM slot in whole waves, long enough that the ring fill
+// (6 planes of loads, no arithmetic) stays a small part of a chunk.
+static int pick_chunks(int tiles, int nz, int slots) {
+  int best_c = 1;
+  double best = 1e300;
+  for (int c = 1; c <= (nz + 3) / 4; ++c) {
+    const int kz = (nz + c - 1) / c, ce = (nz + kz - 1) / kz;
+    const long long waves = ((long long)tiles * ce + slots - 1) / slots;
+    const double cost = (double)waves * (kz + 1.0);
+    if (cost < best - 1e-9) { best = cost; best_c = ce; }
+  }
+  return best_c;
+}
+
+#ifndef STREAMS_MARCH_TY
+#define STREAMS_MARCH_TY 8
+#endif
+
+template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
+static int launch_march(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+  using G = MarchGeom<TY>;
+  constexpr int NF = VISC ? 9 : 6;
+  const size_t smem = (size_t)(2 * NF * G::PLANE + (10 + NF + (WENO ? 30 : 0)) * G::NT) * sizeof(double);
+  auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    attr_set = true;
+  }
+  const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
+  const int tiles = nbx * nby;
+  const int slots = P.nsm * (TY >= 8 ? 1 : 2);
+  const int chunks = pick_chunks(tiles, P.nz, slots);
+  const int kz = (P.nz + chunks - 1) / chunks;
+  kern<<<(unsigned)(tiles * chunks), G::NT, smem, st>>>(P, sa, nbx, nby, kz);
+  return 1;
+}
 
 template <int L, int LV, int R>
 static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
   const bool visc = P.visc_law != VISC_NONE;
   const bool conv = P.flux_mode != FLUX_WENO;
   const bool weno = P.flux_mode != FLUX_CENTRAL;
-  const int nbx = (P.nx + MBX - 1) / MBX, nby = (P.ny + MBY - 1) / MBY, nbz = (P.nz + MBZ - 1) / MBZ;
-  int slab = 8;                                  // 8 block rows = 32 grid rows per slab
-  if (slab > nby) slab = nby;
-  const int nslab = (nby + slab - 1) / slab;
-  const long long nblocks = (long long)nslab * nbx * slab * nbz;
-  dim3 b(MBX * MBY * MBZ), g((unsigned)nblocks);
-#define STREAMS_MAIN(V, C, W) rhs_main_kernel<L, LV, V, C, W, MBX, MBY, MBZ><<<g, b, 0, st>>>(P, sa, nbx, nby, nbz, slab)
+  constexpr int TY = STREAMS_MARCH_TY;
+#define STREAMS_MAIN(V, C, W) return launch_march<L, LV, V, C, W, TY>(P, sa, st)
   if (visc && conv && weno) STREAMS_MAIN(true, true, true);
   else if (visc && conv) STREAMS_MAIN(true, true, false);
   else if (visc) STREAMS_MAIN(true, false, true);
@@ -539,7 +745,6 @@ static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
   else if (conv) STREAMS_MAIN(false, true, false);
   else STREAMS_MAIN(false, false, true);
 #undef STREAMS_MAIN
-  return 1;
 }
 
 template <int L, int R>
