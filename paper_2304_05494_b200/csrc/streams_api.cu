@@ -87,13 +87,13 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   S.off_w = take(5 * S.fs * 8);
   S.off_q = take((size_t)S.nq * S.fs * 8);
-  S.off_div = take(S.fs * 8);
+  S.off_div = S.off_q + (size_t)Q_DIV * S.fs * 8;
   S.off_theta = take(S.N * 8);
   S.off_mask = take(S.fs);
   S.off_nflag = take(hyb ? S.fs : 256);
   S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
   S.off_counters = take(C_COUNT * 4);
-  S.off_R = take(5 * S.N * 8);
+  S.off_R = take(5 * S.fs * 8);
   S.off_metrics = take(3 * (size_t)g->ny * 8);
   S.off_scal = take(S_COUNT * 8);
   S.total = off;
@@ -108,6 +108,7 @@ struct streams_ctx {
   streams_scheme scheme;
   Sizes S;
   DevP P;
+  MarchMaps maps;
   cudaStream_t stream;
   char* base;
   bool have_fields;
@@ -238,7 +239,7 @@ int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   int b = 0;
   if (ctx->scheme.flux_mode != STREAMS_FLUX_CENTRAL)
     b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
-  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
+  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
   return (a < 0 || b < 0) ? -1 : a + b;
 }
 
@@ -294,6 +295,14 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.inv_dx = (double)grid->nx / grid->lx;
   P.inv_dz = (double)grid->nz / grid->lz;
   fd1(S.L, P.a1); fd1(S.Lv, P.a1v); fd2(S.Lv, P.b2v);
+  P.sbv = 0.0;
+  for (int l = 0; l < 4; ++l) {
+    P.kc[l] = 0.25 * P.a1[l];
+    P.avx[l] = P.a1v[l] * P.inv_dx; P.bvx[l] = P.b2v[l] * (P.inv_dx * P.inv_dx);
+    P.avz[l] = P.a1v[l] * P.inv_dz; P.bvz[l] = P.b2v[l] * (P.inv_dz * P.inv_dz);
+    P.sbv += P.b2v[l];
+  }
+  P.sb2xz = -2.0 * P.sbv * (P.inv_dx * P.inv_dx + P.inv_dz * P.inv_dz);
   P.gamma = gas->gamma; P.gm1 = gas->gamma - 1.0; P.rgas = gas->rgas; P.prandtl = gas->prandtl;
   P.kfac = (gas->gamma * gas->rgas / (gas->gamma - 1.0)) / gas->prandtl;
   P.mu_ref = gas->mu_ref; P.t_ref = gas->t_ref; P.suth_s = gas->suth_s_over_tref; P.pow_exp = gas->pow_exp;
@@ -312,6 +321,10 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
       return fail(nullptr, STREAMS_ECUDA, "cannot query the device");
     }
     P.nsm = nsm;
+  }
+  if (make_march_maps(P, &ctx->maps) != 0) {
+    delete ctx;
+    return fail(nullptr, STREAMS_ECUDA, "cannot build the TMA descriptors (cuTensorMapEncodeTiled)");
   }
 
   std::vector<double> eyc, eyv, eyyv;
@@ -377,7 +390,7 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   enqueue_prepare(ctx, false, false);
   StageArgs sa;
   sa.gam = 0.0; sa.rhk = 0.0; sa.update_w = 0; sa.read_prev = 0; sa.write_r = 1;
-  sa.r_out = rhs_out_dev ? rhs_out_dev : ctx->P.R;
+  sa.r_dense = rhs_out_dev;
   if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
   CU(cudaGetLastError());
   return STREAMS_OK;
@@ -396,7 +409,7 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
       enqueue_prepare(ctx, want_dt && l == 0, false);
       StageArgs sa;
       sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
-      sa.r_out = ctx->P.R;
+      sa.r_dense = nullptr;
       if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
     }
     timed(ctx, STREAMS_K_MISC, [&] { return launch_step_end(ctx->P, ctx->stream); });

@@ -1,6 +1,7 @@
 // Host-side launch wrappers implemented by the kernel translation units.
 // Each returns the number of kernels it launched.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include "streams_dev.cuh"
 
@@ -11,9 +12,15 @@ struct StageArgs {
   double gam, rhk;      // w += dt (gam R + rhk R_prev)            (O5)
   int update_w;         // 0: RHS only (streams_rhs)
   int read_prev;        // stage uses the previous-stage RHS
-  int write_r;          // keep R for the next stage
-  double* r_out;        // where R goes when write_r (interior [5][N])
+  int write_r;          // keep R (padded layout, DevP::R) for the next stage
+  double* r_dense;      // if not null: also write R here, interior [5][N] (streams_rhs output)
 };
+
+// TMA descriptors of the fused RHS kernel (built once per context by make_march_maps):
+// centre planes with halo and ring planes of the primitives, RK operands w and R.
+struct MarchMaps { CUtensorMap centre, ring, w, r; };
+// Returns 0, or a negative code: -1 driver entry point missing, -2 encode failed.
+int make_march_maps(const DevP& P, MarchMaps* maps);
 
 int launch_fill_prim(const DevP& P, cudaStream_t st);
 int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st);
@@ -24,7 +31,7 @@ int launch_step_end(const DevP& P, cudaStream_t st);
 // returns the number of launches (0 when the flux mode does not need it) or < 0 if the (L, Lv, r)
 // combination is not instantiated.
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st);
-int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
+int launch_rhs_main(const DevP& P, const MarchMaps& maps, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law);
 
 }  // namespace streams

@@ -15,68 +15,111 @@
 
 namespace streams {
 
-struct VAcc {          // velocity / temperature / viscosity / dilatation derivatives at a node
-  double g[3][3];      // g[a][b] = d u_a / d x_b
-  double gT[3], gmu[3], gdiv[3];
-  double lap[3], lapT; // sum over directions of the second-derivative stencils, centre term applied at the end
-};
-
 template <int D>
 __device__ __forceinline__ double pick(double a, double b, double c) { return D == 0 ? a : (D == 1 ? b : c); }
 
-// fields of the marching kernel, in the order of DevP::q (F_DIV is DevP::div)
-enum { F_U = 0, F_V = 1, F_W = 2, F_H = 3, F_P = 4, F_RHO = 5, F_T = 6, F_MU = 7, F_DIV = 8 };
+// fields of the marching kernel = the first nine slots of DevP::q
+enum { F_U = Q_U, F_V = Q_V, F_W = Q_W, F_H = Q_H, F_P = Q_P, F_RHO = Q_RHO, F_T = Q_T, F_MU = Q_MU, F_DIV = Q_DIV };
 
-__device__ __forceinline__ const double* field_ptr(const DevP& P, int f) { return f < 8 ? P.q + f * P.fs : P.div; }
+// ------------------------------------------------------------------ async-copy / mbarrier / TMA primitives
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
-}
 // copies 8 bytes when `take`, writes zeros (and reads nothing) otherwise
 __device__ __forceinline__ void cp_async8_zfill(void* smem_dst, const void* gsrc, bool take) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
   const unsigned n = take ? 8u : 0u;
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(s), "l"(gsrc), "r"(n) : "memory");
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(n) : "memory");
 }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // a load the compiler may not sink to its first use
 __device__ __forceinline__ unsigned ld_u8_now(const unsigned char* p) {
   unsigned v;
   asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// one box of a 4-D tensor (x, y, z, field) into shared memory, completion counted on `bar`
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1,
+                                            int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::
+          "r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
 
-// per-direction stencil coefficients with the metric folded in
-struct DirCoef {
-  double kc[3];        // convective: a_l / 4            (mass flux pairs; the metric multiplies the sums)
-  double ap[3];        // pressure:   a_l
-  double met_c;        // convective metric
-  double av[3];        // viscous first derivative:  a_l * metric
-  double bv[3];        // viscous second derivative: b_l * metric^2
+// ------------------------------------------------------------------ arithmetic of one node
+// Stencil coefficients of direction D.  x and z: the uniform metric is folded in on the host (DevP::avx ...);
+// y: raw coefficients, the row's metrics are applied to the sums.
+template <int D> __device__ __forceinline__ double coef_a(const DevP& P, int l) { return D == 0 ? P.avx[l] : (D == 1 ? P.a1v[l] : P.avz[l]); }
+template <int D> __device__ __forceinline__ double coef_b(const DevP& P, int l) { return D == 0 ? P.bvx[l] : (D == 1 ? P.b2v[l] : P.bvz[l]); }
+
+struct YMet { double eyc, eyv, eyv2, eyy; };   // d eta/dy (central order, viscous order), its square, d2 eta/dy2
+
+// Viscous accumulators of a node (O4), folded as the derivatives arrive so that few values stay live:
+//   vm_a  = mu (lap u_a + (d_a div)/3) + sum_b d_b mu (d_b u_a + d_a u_b) - 2/3 d_a mu div u
+//   Phi   = mu [2 sum_a (d_a u_a)^2 + sum_{a<b} (d_b u_a + d_a u_b)^2 - 2/3 (div u)^2]
+//   cond  = (cp/Pr) (mu lap T + grad mu . grad T)
+struct Visc {
+  double gmu[3];
+  double vm[3];          // cross terms sum_b d_b mu (d_b u_a + d_a u_b)
+  double lap[3];         // second-derivative sums of u_a + (d_a div)/3 (centre term applied at the end)
+  double dv, ph, cond;
+  double k10, k20, k21;  // d_x v, d_x w, d_y w kept for the symmetric strain terms
 };
 
-// ---------------------------------------------------------------------------------------------
-// One direction at one node; G(f, o) returns field f at offset o (-3..3) along the direction.
-// Convective part (O1) in pair-difference form: with m(a,b) = (a_l/4)(rho_a+rho_b)(ud_a+ud_b),
+// grad mu, grad T, lap T, grad div along D; G(f, o) = field f at offset o along D.
+template <int D, int LV, class G>
+__device__ __forceinline__ void scalar_terms(const DevP& P, const G& g, const YMet& ym, double gT[3], double& lapT, Visc& V) {
+  double dm = 0.0, dd = 0.0, dT = 0.0, sT = 0.0;
+#pragma unroll
+  for (int l = 1; l <= LV; ++l) {
+    const double a = coef_a<D>(P, l - 1), b = coef_b<D>(P, l - 1);
+    const double tb = g(F_T, l), ta = g(F_T, -l);
+    dm = fma(a, g(F_MU, l) - g(F_MU, -l), dm);
+    dd = fma(a, g(F_DIV, l) - g(F_DIV, -l), dd);
+    dT = fma(a, tb - ta, dT);
+    sT = fma(b, tb + ta, sT);
+  }
+  if (D == 1) {
+    sT = fma(ym.eyy, dT, ym.eyv2 * sT);
+    dm *= ym.eyv; dd *= ym.eyv; dT *= ym.eyv;
+  }
+  V.gmu[D] = dm;
+  V.lap[D] = dd * (1.0 / 3.0);
+  gT[D] = dT;
+  lapT += sT;
+}
+
+// Convective terms (O1) and the velocity derivatives along D.
+// Convective part in pair-difference form: with m(a,b) = (a_l/4)(rho_a+rho_b)(ud_a+ud_b),
 //   f_{n+1/2} - f_{n-1/2} = sum_l [ m(n,n+l)(phi_n+phi_{n+l}) - m(n-l,n)(phi_{n-l}+phi_n) ]
 //                         = phi_n S0 + sum_l [ m(n,n+l) phi_{n+l} - m(n-l,n) phi_{n-l} ],  S0 = sum_l [m(n,n+l) - m(n-l,n)]
-// (the same sum as the oracle's interface-flux form, regrouped), plus sum_l a_l (p_{n+l} - p_{n-l}) on the
-// D-momentum.  Viscous part (O4): first derivatives of u, v, w, T, mu, div; second-derivative sums
-// sum_l b_l (f_{+l} + f_{-l}) of u, v, w, T (the centre term -2 f_0 sum b_l is applied once by the caller).
-// c0 = (u, v, w, H, p, rho) at the node, alr[l] = kc[l] * rho_0.
-// ---------------------------------------------------------------------------------------------
+// (the oracle's interface-flux sum, regrouped), plus sum_l a_l (p_{n+l} - p_{n-l}) on the D-momentum.
+// c0 = (u, v, w, H, p, rho) at the node, alr[l] = (a_l/4) rho_0.
 template <int D, int L, int LV, bool CONV, bool VISC, class G>
-__device__ __forceinline__ void dir_terms(const G& g, const DirCoef& c, const double c0[6], const double alr[3],
-                                          double eyr, double r[5], VAcc& V) {
+__device__ __forceinline__ void dir_terms(const DevP& P, const G& g, const YMet& ym, const double c0[6],
+                                          const double alr[3], double r[5], Visc& V) {
   constexpr int LC = CONV ? L : 0;
   constexpr int LVV = VISC ? LV : 0;
   constexpr int LM = LC > LVV ? LC : LVV;
   double S0 = 0.0, S[4] = {0.0, 0.0, 0.0, 0.0}, SP = 0.0;
-  double d1[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // u v w T mu div
-  double d2[4] = {0.0, 0.0, 0.0, 0.0};             // u v w T
+  double d1[3] = {0.0, 0.0, 0.0}, d2[3] = {0.0, 0.0, 0.0};
   const double ud0 = pick<D>(c0[0], c0[1], c0[2]);
 #pragma unroll
   for (int l = 1; l <= LM; ++l) {
@@ -87,81 +130,66 @@ __device__ __forceinline__ void dir_terms(const G& g, const DirCoef& c, const do
       const double rb = g(F_RHO, l), ra = g(F_RHO, -l);
       const double hb = g(F_H, l), ha = g(F_H, -l);
       const double pb = g(F_P, l), pa = g(F_P, -l);
-      const double mb = fma(c.kc[l - 1], rb, alr[l - 1]) * (ud0 + pick<D>(ub, vb, wb));
-      const double ma = fma(c.kc[l - 1], ra, alr[l - 1]) * (pick<D>(ua, va, wa) + ud0);
+      const double mb = fma(P.kc[l - 1], rb, alr[l - 1]) * (ud0 + pick<D>(ub, vb, wb));
+      const double ma = fma(P.kc[l - 1], ra, alr[l - 1]) * (pick<D>(ua, va, wa) + ud0);
       S0 += mb - ma;
       S[0] = fma(mb, ub, S[0]); S[0] = fma(-ma, ua, S[0]);
       S[1] = fma(mb, vb, S[1]); S[1] = fma(-ma, va, S[1]);
       S[2] = fma(mb, wb, S[2]); S[2] = fma(-ma, wa, S[2]);
       S[3] = fma(mb, hb, S[3]); S[3] = fma(-ma, ha, S[3]);
-      SP = fma(c.ap[l - 1], pb - pa, SP);
+      SP = fma(P.a1[l - 1], pb - pa, SP);
     }
     if constexpr (VISC) if (l <= LVV) {
-      const double tb = g(F_T, l), ta = g(F_T, -l);
-      const double a = c.av[l - 1], b = c.bv[l - 1];
+      const double a = coef_a<D>(P, l - 1), b = coef_b<D>(P, l - 1);
       d1[0] = fma(a, ub - ua, d1[0]);  d2[0] = fma(b, ub + ua, d2[0]);
       d1[1] = fma(a, vb - va, d1[1]);  d2[1] = fma(b, vb + va, d2[1]);
       d1[2] = fma(a, wb - wa, d1[2]);  d2[2] = fma(b, wb + wa, d2[2]);
-      d1[3] = fma(a, tb - ta, d1[3]);  d2[3] = fma(b, tb + ta, d2[3]);
-      d1[4] = fma(a, g(F_MU, l) - g(F_MU, -l), d1[4]);
-      d1[5] = fma(a, g(F_DIV, l) - g(F_DIV, -l), d1[5]);
     }
   }
   if (CONV) {
-    r[0] = fma(-2.0 * c.met_c, S0, r[0]);
+    const double met = D == 0 ? P.inv_dx : (D == 1 ? ym.eyc : P.inv_dz);
+    r[0] = fma(-2.0 * met, S0, r[0]);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) r[1 + q] = fma(-c.met_c, fma(c0[q], S0, S[q]), r[1 + q]);
-    r[1 + D] = fma(-c.met_c, SP, r[1 + D]);
+    for (int q = 0; q < 4; ++q) r[1 + q] = fma(-met, fma(c0[q], S0, S[q]), r[1 + q]);
+    r[1 + D] = fma(-met, SP, r[1 + D]);
   }
   if (VISC) {
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-      V.g[a][D] = d1[a];
-      V.lap[a] += (D == 1) ? fma(eyr, d1[a], d2[a]) : d2[a];
+      if (D == 1) {
+        d2[a] = fma(ym.eyy, d1[a], ym.eyv2 * d2[a]);
+        d1[a] *= ym.eyv;
+      }
+      V.lap[a] += d2[a];
+      V.vm[a] = fma(V.gmu[D], d1[a], V.vm[a]);          // d_D mu d_D u_a
     }
-    V.gT[D] = d1[3];
-    V.lapT += (D == 1) ? fma(eyr, d1[3], d2[3]) : d2[3];
-    V.gmu[D] = d1[4];
-    V.gdiv[D] = d1[5];
+    double t = V.gmu[0] * d1[0];                          // sum_a d_a mu d_D u_a -> vm_D
+    t = fma(V.gmu[1], d1[1], t);
+    t = fma(V.gmu[2], d1[2], t);
+    V.vm[D] += t;
+    V.dv += d1[D];
+    V.ph = fma(d1[D], d1[D], V.ph);                       // doubled at the end
+    if (D == 0) { V.k10 = d1[1]; V.k20 = d1[2]; }
+    if (D == 1) { const double s01 = d1[0] + V.k10; V.k10 = s01 * s01; V.k21 = d1[2]; }
+    if (D == 2) {
+      const double s02 = d1[0] + V.k20, s12 = d1[1] + V.k21;
+      V.k20 = fma(s02, s02, V.k10);
+      V.k20 = fma(s12, s12, V.k20);                       // sum of the squared off-diagonal strains
+    }
   }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Viscous combination (O4) for one node; c0 = (u, v, w, ...).
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void viscous_combine(const DevP& P, const double c0[6], double mu0, double r[5], const VAcc& V) {
-  const double dv = (V.g[0][0] + V.g[1][1]) + V.g[2][2];
-  const double s01 = V.g[0][1] + V.g[1][0], s02 = V.g[0][2] + V.g[2][0], s12 = V.g[1][2] + V.g[2][1];
-  const double s[3][3] = {{2.0 * V.g[0][0], s01, s02}, {s01, 2.0 * V.g[1][1], s12}, {s02, s12, 2.0 * V.g[2][2]}};
-  const double tdv = (2.0 / 3.0) * dv;
-  double vm[3];
+// closes the viscous terms of a node: c0 = (u, v, w, ...), T0, mu0 at the node, sb2 = -2 sum_d sum_l b_l metric_d^2
+__device__ __forceinline__ void viscous_close(const DevP& P, const double c0[6], double mu0, double sb2, double r[5], Visc& V) {
+  const double tdv = (2.0 / 3.0) * V.dv;
+  double e = fma(mu0, fma(-tdv, V.dv, fma(2.0, V.ph, V.k20)), P.kfac * V.cond);
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    double cross = V.gmu[0] * s[a][0];
-    cross = fma(V.gmu[1], s[a][1], cross);
-    cross = fma(V.gmu[2], s[a][2], cross);
-    cross = fma(-V.gmu[a], tdv, cross);
-    vm[a] = fma(mu0, fma(V.gdiv[a], 1.0 / 3.0, V.lap[a]), cross);
+    const double lap = fma(sb2, c0[a], V.lap[a]);
+    const double vm = fma(mu0, lap, fma(-V.gmu[a], tdv, V.vm[a]));
+    r[1 + a] += vm;
+    e = fma(c0[a], vm, e);
   }
-  double ph = V.g[0][0] * V.g[0][0];
-  ph = fma(V.g[1][1], V.g[1][1], ph);
-  ph = fma(V.g[2][2], V.g[2][2], ph);
-  ph = ph + ph;
-  ph = fma(s01, s01, ph);
-  ph = fma(s02, s02, ph);
-  ph = fma(s12, s12, ph);
-  ph = fma(-tdv, dv, ph);
-  double cond = mu0 * V.lapT;
-  cond = fma(V.gmu[0], V.gT[0], cond);
-  cond = fma(V.gmu[1], V.gT[1], cond);
-  cond = fma(V.gmu[2], V.gT[2], cond);
-  r[1] += vm[0];
-  r[2] += vm[1];
-  r[3] += vm[2];
-  double e = fma(mu0, ph, P.kfac * cond);
-  e = fma(c0[0], vm[0], e);
-  e = fma(c0[1], vm[1], e);
-  e = fma(c0[2], vm[2], e);
   r[4] += e;
 }
 
@@ -169,39 +197,57 @@ __device__ __forceinline__ void viscous_combine(const DevP& P, const double c0[6
 // rhs_march_kernel (a4-a8 in one pass).  A block owns a 32 x TY tile of (x, y) and marches through a chunk
 // of z planes (2.5-D blocking):
 //   - z neighbours: every thread keeps the 7-plane column (k-3 .. k+3) of its node for all fields in
-//     registers; plane k+4 is fetched one iteration ahead (plain coalesced loads, consumed at the ring shift);
-//   - x / y neighbours: the centre plane of every field sits in shared memory with its 3-wide halo
-//     (interior written from the registers, halo copied with cp.async one iteration ahead, two buffers, one
-//     barrier per plane); all stencil offsets are compile-time immediates;
-//   - RK operands (previous-stage R, w) are staged with cp.async at the start of the iteration and consumed
-//     at its end, so no global-memory latency is exposed in the loop.
-// Threads of a ragged tile beyond the interior load (clamped) ghost nodes, so the tile's shared-memory
-// plane is correct wherever an interior thread reads it; they do not store.
+//     registers; plane k+4 arrives by TMA in a shared-memory slot and enters the ring at the shift;
+//   - x / y neighbours: the centre plane of all fields with its 3-wide halo is ONE 4-D TMA box
+//     (x, y, z, field) = (40, TY+6, 1, 9) into one of two shared-memory buffers, issued two planes ahead;
+//     every stencil offset is a compile-time immediate;
+//   - RK operands (w, previous-stage R) of the plane arrive by TMA one plane ahead;
+//   - flux corrections of flagged interfaces (hybrid / WENO): cp.async with zero fill, by the warps that
+//     have a flagged node only.
+// One thread issues the TMA copies after a split barrier (bar.arrive by the other warps, bar.sync by
+// its warp), so no warp but that one waits for the slowest.  Completion is tracked by mbarriers.
 // ---------------------------------------------------------------------------------------------
 constexpr int MTX = 32;
 
 template <int TY>
 struct MarchGeom {
-  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (3 used), rows stay 16 B aligned
+  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (3 used), rows stay 32 B aligned
   static constexpr int ROWS = TY + 6;
   static constexpr int PLANE = ROW * ROWS;       // doubles per field per buffer
   static constexpr int NT = MTX * TY;
-  static constexpr int NH = 6 * TY + 6 * MTX;    // halo nodes of a plane (corners are never read)
-  static constexpr int HE = (NH + NT - 1) / NT;  // halo nodes per thread
+};
+
+template <int TY, bool VISC, bool WENO>
+struct MarchSmem {
+  using G = MarchGeom<TY>;
+  static constexpr int NF = VISC ? 9 : 6;
+  static constexpr size_t BUF = (size_t)NF * G::PLANE * 8;     // one centre-plane buffer
+  static constexpr size_t RING = (size_t)NF * G::NT * 8;       // one ring-plane slot
+  static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[5]
+  static constexpr size_t DFS = WENO ? (size_t)30 * G::NT * 8 : 0;
+  static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + 2 * RING, OFF_DFS = OFF_EPI + 2 * EPI,
+                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 64;
+  static_assert(BUF % 128 == 0 && RING % 128 == 0 && EPI % 128 == 0, "TMA destinations are 128-byte aligned");
 };
 
 template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
-__global__ void __launch_bounds__(MTX * TY, (TY >= 8 ? 1 : 2))
-rhs_march_kernel(const DevP P, const StageArgs sa, int nbx, int nby, int kz) {
+__global__ void __launch_bounds__(MTX * TY, 1)
+rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
+                 const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r, const DevP P,
+                 const StageArgs sa, int nbx, int nby, int kz) {
   using G = MarchGeom<TY>;
-  constexpr int NF = VISC ? 9 : 6;
+  using SM = MarchSmem<TY, VISC, WENO>;
+  constexpr int NF = SM::NF;
   constexpr int NG = 3;
   static_assert(L <= NG && LV <= NG, "ring depth");
-  extern __shared__ double smem[];
-  double* buf = smem;                              // [2][NF][PLANE]  centre planes with halo
-  double* epi = buf + 2 * NF * G::PLANE;           // [10][NT]         previous-stage R, w of this plane
-  double* nxs = epi + 10 * G::NT;                  // [NF][NT]         plane k+4 of this thread's column
-  double* dfs = nxs + NF * G::NT;                  // [30][NT]         flux corrections around this node (WENO)
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][NF][PLANE]
+  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][NF][NT]
+  double* const epi = reinterpret_cast<double*>(smem_raw + SM::OFF_EPI);    // [2][10][NT]
+  double* const dfs = reinterpret_cast<double*>(smem_raw + SM::OFF_DFS);    // [30][NT]
+  unsigned long long* const bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
+  unsigned long long* const full_c = bars;        // [2] centre plane landed
+  unsigned long long* const full_e = bars + 2;    // [2] ring plane + RK operands landed
 
   const int tid = threadIdx.x;
   const int tx = tid & 31, ty = tid >> 5;
@@ -215,189 +261,174 @@ rhs_march_kernel(const DevP P, const StageArgs sa, int nbx, int nby, int kz) {
   const int i = i0 + tx, j = j0 + ty;
   const bool active = i < P.nx && j < P.ny;
   const int ic = min(i, P.nx + P.ng - 1), jc = min(j, P.ny + P.ng - 1);
-  const long long ncol = pidx(P, ic, jc, 0);       // this thread's column at k = 0
-  const long long ocol = (long long)j * P.nx + i;  // interior index at k = 0 (active threads only)
-  const int s0 = (ty + 3) * G::ROW + tx + 4;       // this node in a shared-memory plane
+  const int isz = (int)P.sz;
+  const int ncol = (int)pidx(P, ic, jc, 0);            // this thread's column at k = 0 (padded index < 2^31)
+  const int s0 = (ty + 3) * G::ROW + tx + 4;           // this node in a shared-memory plane
 
-  // halo nodes handled by this thread: offset in a padded plane, offset in a shared-memory plane
-  int hsrc[G::HE], hdst[G::HE];
-#pragma unroll
-  for (int h = 0; h < G::HE; ++h) {
-    const int e = tid + h * G::NT;
-    int xo, yo;
-    if (e < 6 * TY) { const int rr = e / 6, c = e % 6; yo = rr; xo = c < 3 ? c - 3 : MTX + c - 3; }
-    else { const int e2 = e - 6 * TY, hr = e2 / MTX; xo = e2 % MTX; yo = hr < 3 ? hr - 3 : TY + hr - 3; }
-    const int ih = min(i0 + xo, P.nx + P.ng - 1), jh = min(j0 + yo, P.ny + P.ng - 1);
-    hsrc[h] = e < G::NH ? (int)((long long)(jh + P.ng) * P.sy + ih + P.ox) : -1;
-    hdst[h] = (yo + 3) * G::ROW + 4 + xo;
+  const unsigned bytes_c = (unsigned)SM::BUF;
+  const unsigned bytes_e = (unsigned)SM::RING + (sa.update_w ? 5u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
+  const int cx0 = i0 + P.ox, cy0 = j0 + P.ng;          // tile origin in padded coordinates
+
+  auto issue_centre = [&](int k, int b) {              // thread 0 only
+    mbar_expect_tx(&full_c[b], bytes_c);
+    tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - 3, k + P.ng, 0);
+  };
+  auto issue_ring_epi = [&](int k, int b) {            // ring plane k+4 and the RK operands of plane k into slot b
+    mbar_expect_tx(&full_e[b], bytes_e);
+    tma_load_4d(ring + (size_t)b * NF * G::NT, &tm_ring, &full_e[b], cx0, cy0, k + NG + 1 + P.ng, 0);
+    if (sa.read_prev) tma_load_4d(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + P.ng, 0);
+    if (sa.update_w) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + P.ng, 0);
+  };
+
+  if (tid == 0) {
+    mbar_init(&full_c[0], 1); mbar_init(&full_c[1], 1);
+    mbar_init(&full_e[0], 1); mbar_init(&full_e[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    issue_centre(kb, 0);
+    if (kb + 1 < ke) issue_centre(kb + 1, 1);
+    issue_ring_epi(kb, 0);
   }
 
-  // y metrics of this row (constant along the march)
-  DirCoef cx, cy, cz;
-  const double eyc = P.eta_y_c[min(j, P.ny - 1)];
-  double eyv = 0.0, eyr = 0.0;
-  if (VISC) { eyv = P.eta_y_v[min(j, P.ny - 1)]; eyr = P.eta_yy_v[min(j, P.ny - 1)] / eyv; }
-#pragma unroll
-  for (int l = 0; l < 3; ++l) {
-    cx.kc[l] = cy.kc[l] = cz.kc[l] = 0.25 * P.a1[l];
-    cx.ap[l] = cy.ap[l] = cz.ap[l] = P.a1[l];
-    cx.av[l] = P.a1v[l] * P.inv_dx; cx.bv[l] = P.b2v[l] * (P.inv_dx * P.inv_dx);
-    cy.av[l] = P.a1v[l] * eyv;      cy.bv[l] = P.b2v[l] * (eyv * eyv);
-    cz.av[l] = P.a1v[l] * P.inv_dz; cz.bv[l] = P.b2v[l] * (P.inv_dz * P.inv_dz);
+  // metrics of this row (constant along the march)
+  YMet ym;
+  ym.eyc = P.eta_y_c[min(j, P.ny - 1)];
+  ym.eyv = ym.eyv2 = ym.eyy = 0.0;
+  if (VISC) {
+    ym.eyv = P.eta_y_v[min(j, P.ny - 1)];
+    ym.eyv2 = ym.eyv * ym.eyv;
+    ym.eyy = P.eta_yy_v[min(j, P.ny - 1)];
   }
-  cx.met_c = P.inv_dx; cy.met_c = eyc; cz.met_c = P.inv_dz;
-  const double sb2 = -2.0 * (((cx.bv[0] + cx.bv[1]) + cx.bv[2]) + ((cy.bv[0] + cy.bv[1]) + cy.bv[2]) +
-                             ((cz.bv[0] + cz.bv[1]) + cz.bv[2]));
+  const double sb2 = fma(-2.0 * P.sbv, ym.eyv2, P.sb2xz);
   const double dt = sa.update_w ? P.scal[S_DT] : 0.0;
 
-  // ---- prologue: ring = planes kb-3 .. kb+3, halo of plane kb
+  // ring = planes kb-3 .. kb+3 of this thread's column
   double zr[NF][2 * NG + 1];
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
-    const double* __restrict__ fp = field_ptr(P, f) + ncol + (long long)(kb - NG) * P.sz;
+    const double* __restrict__ fp = P.q + (long long)f * P.fs + ncol + (long long)(kb - NG) * P.sz;
 #pragma unroll
     for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
   }
-  {
-    const long long pl = (long long)(kb + P.ng) * P.sz;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      const double* __restrict__ fp = field_ptr(P, f) + pl;
-#pragma unroll
-      for (int h = 0; h < G::HE; ++h)
-        if (hsrc[h] >= 0) cp_async8(buf + f * G::PLANE + hdst[h], fp + hsrc[h]);
-    }
-    cp_async_commit();
-  }
+  unsigned fl_next = 0;
+  if (WENO && CONV && active) fl_next = ld_u8_now(P.nflag + ncol + (long long)kb * P.sz);
 
   for (int k = kb; k < ke; ++k) {
-    const int b = (k - kb) & 1;
-    double* __restrict__ sm = buf + b * NF * G::PLANE;
-    // (A) centre plane -> shared memory; halo of plane k has been in flight for one iteration
-#pragma unroll
-    for (int f = 0; f < NF; ++f) sm[f * G::PLANE + s0] = zr[f][NG];
-    cp_async_wait<0>();
-    __syncthreads();
-    // (B) start what the next iteration and this iteration's epilogue need
-    const long long n = ncol + (long long)k * P.sz;
-    const long long o = ocol + (long long)k * P.ny * P.nx;
+    const int it = k - kb, b = it & 1;
+    const unsigned par = (unsigned)(it >> 1) & 1u;
+    const int n = ncol + k * isz;
+    // flags of this plane (prefetched), of the next one, and this plane's flux corrections
     unsigned fl = 0;
-    if (WENO) {
-      fl = CONV ? (active ? ld_u8_now(P.nflag + n) : 0u) : 0x3fu;
-    }
-    if (active) {
-      if (sa.read_prev) {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) cp_async8(epi + q * G::NT + tid, P.R + q * P.N + o);
-      }
-      if (sa.update_w) {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) cp_async8(epi + (5 + q) * G::NT + tid, P.w + q * P.fs + n);
-      }
-    }
-    {
-      // plane k+4 (clamped to the last ghost plane: the value is unused when it is beyond)
-      const int kn = min(k + NG + 1, P.nz + P.ng - 1);
-      const long long nn = ncol + (long long)kn * P.sz;
-#pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async8(nxs + f * G::NT + tid, field_ptr(P, f) + nn);
-    }
-    cp_async_commit();
-    if (k + 1 < ke) {
-      double* __restrict__ smn = buf + (b ^ 1) * NF * G::PLANE;
-      const long long pl = (long long)(k + 1 + P.ng) * P.sz;
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        const double* __restrict__ fp = field_ptr(P, f) + pl;
-#pragma unroll
-        for (int h = 0; h < G::HE; ++h)
-          if (hsrc[h] >= 0) cp_async8(smn + f * G::PLANE + hdst[h], fp + hsrc[h]);
-      }
-    }
-    cp_async_commit();
-    // flux corrections of the flagged interfaces around the nodes of this warp (third group: waited with
-    // the first at the epilogue; zero-filled where an interface is not flagged)
     bool any_fl = false;
     if (WENO) {
+      fl = CONV ? fl_next : (active ? 0x3fu : 0u);
+      if (CONV && active && k + 1 < ke) fl_next = ld_u8_now(P.nflag + n + isz);
       any_fl = __any_sync(0xffffffffu, fl != 0);
       if (any_fl) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-          const long long sd = d == 0 ? 1 : (d == 1 ? P.sy : P.sz);
+          const int sd = d == 0 ? 1 : (d == 1 ? (int)P.sy : isz);
           const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 0) * G::NT + tid, f + q * P.fs, (fl >> (2 * d + 1)) & 1u);
-            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 1) * G::NT + tid, f + q * P.fs - sd, (fl >> (2 * d)) & 1u);
+            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 0) * G::NT + tid, f + (long long)q * P.fs, (fl >> (2 * d + 1)) & 1u);
+            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 1) * G::NT + tid, f + (long long)q * P.fs - sd, (fl >> (2 * d)) & 1u);
           }
         }
       }
     }
-    cp_async_commit();
 
     // (C) the right-hand side of this node
+    mbar_wait(&full_c[b], par);
+    const double* __restrict__ sc = buf + (size_t)b * NF * G::PLANE + s0;
+    auto gx = [&](int f, int o2) { return sc[f * G::PLANE + o2]; };
+    auto gy = [&](int f, int o2) { return sc[f * G::PLANE + o2 * G::ROW]; };
+    auto gz = [&](int f, int o2) { return zr[f][NG + o2]; };
     double c0[6];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c0[q] = zr[q][NG];
     double alr[3];
 #pragma unroll
-    for (int l = 0; l < 3; ++l) alr[l] = cx.kc[l] * c0[F_RHO];
+    for (int l = 0; l < 3; ++l) alr[l] = P.kc[l] * c0[F_RHO];
     double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    VAcc V;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { V.lap[a] = 0.0; }
-    V.lapT = 0.0;
-    {
-      const double* __restrict__ sc = sm + s0;
-      auto gx = [&](int f, int o2) { return sc[f * G::PLANE + o2]; };
-      dir_terms<0, L, LV, CONV, VISC>(gx, cx, c0, alr, 0.0, r, V);
-      auto gy = [&](int f, int o2) { return sc[f * G::PLANE + o2 * G::ROW]; };
-      dir_terms<1, L, LV, CONV, VISC>(gy, cy, c0, alr, eyr, r, V);
-      auto gz = [&](int f, int o2) { return zr[f][NG + o2]; };
-      dir_terms<2, L, LV, CONV, VISC>(gz, cz, c0, alr, 0.0, r, V);
-    }
+    Visc V;
     if (VISC) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) V.lap[a] = fma(sb2, c0[a], V.lap[a]);
-      V.lapT = fma(sb2, zr[VISC ? F_T : 0][NG], V.lapT);
-      viscous_combine(P, c0, zr[VISC ? F_MU : 0][NG], r, V);
+      double gT[3], lapT = 0.0;
+      scalar_terms<0, LV>(P, gx, ym, gT, lapT, V);
+      scalar_terms<1, LV>(P, gy, ym, gT, lapT, V);
+      scalar_terms<2, LV>(P, gz, ym, gT, lapT, V);
+      const double mu0 = zr[VISC ? F_MU : 0][NG];
+      double cond = mu0 * fma(sb2, zr[VISC ? F_T : 0][NG], lapT);
+      cond = fma(V.gmu[0], gT[0], cond);
+      cond = fma(V.gmu[1], gT[1], cond);
+      V.cond = fma(V.gmu[2], gT[2], cond);
+      V.vm[0] = V.vm[1] = V.vm[2] = 0.0;
+      V.dv = 0.0; V.ph = 0.0;
+    }
+    dir_terms<0, L, LV, CONV, VISC>(P, gx, ym, c0, alr, r, V);
+    dir_terms<1, L, LV, CONV, VISC>(P, gy, ym, c0, alr, r, V);
+    dir_terms<2, L, LV, CONV, VISC>(P, gz, ym, c0, alr, r, V);
+    if (VISC) viscous_close(P, c0, zr[VISC ? F_MU : 0][NG], sb2, r, V);
+
+    // every warp is done with buf[b], ring[b^1], epi[b^1]: the issuing thread refills them
+    // (two alternating barrier ids: a warp may run one iteration ahead of the slowest)
+    if (tid >> 5) {
+      if (b) asm volatile("bar.arrive 2, %0;" ::"n"(G::NT) : "memory");
+      else asm volatile("bar.arrive 1, %0;" ::"n"(G::NT) : "memory");
+    } else {
+      if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
+      else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
+      if (tid == 0) {
+        if (k + 2 < ke) issue_centre(k + 2, b);
+        if (k + 1 < ke) issue_ring_epi(k + 1, b ^ 1);
+      }
     }
 
     // (D) flux corrections of flagged interfaces, RK update, stores
-    cp_async_wait<0>();
-    if (active) {
-      if (WENO && any_fl) {
-        const double met[3] = {P.inv_dx, eyc, P.inv_dz};
+    mbar_wait(&full_e[b], par);
+    const double* __restrict__ ep = epi + (size_t)b * 10 * G::NT + tid;
+    if (WENO && any_fl) {
+      cp_async_wait_all();
+      const double met[3] = {P.inv_dx, ym.eyc, P.inv_dz};
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
+      for (int d = 0; d < 3; ++d) {
 #pragma unroll
-          for (int q = 0; q < 5; ++q) {
-            const double fp = dfs[((d * 5 + q) * 2 + 0) * G::NT + tid];
-            const double fm = dfs[((d * 5 + q) * 2 + 1) * G::NT + tid];
-            r[q] = fma(-met[d], fp - fm, r[q]);
-          }
+        for (int q = 0; q < 5; ++q) {
+          const double fp = dfs[((d * 5 + q) * 2 + 0) * G::NT + tid];
+          const double fm = dfs[((d * 5 + q) * 2 + 1) * G::NT + tid];
+          r[q] = fma(-met[d], fp - fm, r[q]);
         }
       }
+    }
+    if (active) {
       if (sa.update_w) {
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           double inc = sa.gam * r[q];
-          if (sa.read_prev) inc = fma(sa.rhk, epi[q * G::NT + tid], inc);
-          P.w[q * P.fs + n] = fma(dt, inc, epi[(5 + q) * G::NT + tid]);
+          if (sa.read_prev) inc = fma(sa.rhk, ep[q * G::NT], inc);
+          P.w[(long long)q * P.fs + n] = fma(dt, inc, ep[(5 + q) * G::NT]);
         }
       }
       if (sa.write_r) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) sa.r_out[q * P.N + o] = r[q];
+        for (int q = 0; q < 5; ++q) P.R[(long long)q * P.fs + n] = r[q];
+      }
+      if (sa.r_dense) {
+        const long long o = ((long long)k * P.ny + j) * P.nx + i;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sa.r_dense[q * P.N + o] = r[q];
       }
     }
 
     // (E) shift the ring
+    const double* __restrict__ rn = ring + (size_t)b * NF * G::NT + tid;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
 #pragma unroll
       for (int m = 0; m < 2 * NG; ++m) zr[f][m] = zr[f][m + 1];
-      zr[f][2 * NG] = nxs[f * G::NT + tid];
+      zr[f][2 * NG] = rn[f * G::NT];
     }
   }
 }
@@ -712,32 +743,30 @@ static int pick_chunks(int tiles, int nz, int slots) {
 #endif
 
 template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
-static int launch_march(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st) {
   using G = MarchGeom<TY>;
-  constexpr int NF = VISC ? 9 : 6;
-  const size_t smem = (size_t)(2 * NF * G::PLANE + (10 + NF + (WENO ? 30 : 0)) * G::NT) * sizeof(double);
+  using SM = MarchSmem<TY, VISC, WENO>;
   auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY>;
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
     attr_set = true;
   }
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int tiles = nbx * nby;
-  const int slots = P.nsm * (TY >= 8 ? 1 : 2);
-  const int chunks = pick_chunks(tiles, P.nz, slots);
+  const int chunks = pick_chunks(tiles, P.nz, P.nsm);
   const int kz = (P.nz + chunks - 1) / chunks;
-  kern<<<(unsigned)(tiles * chunks), G::NT, smem, st>>>(P, sa, nbx, nby, kz);
+  kern<<<(unsigned)(tiles * chunks), G::NT, SM::TOTAL, st>>>(mp.centre, mp.ring, mp.w, mp.r, P, sa, nbx, nby, kz);
   return 1;
 }
 
 template <int L, int LV, int R>
-static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
+static int launch_main_T(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st) {
   const bool visc = P.visc_law != VISC_NONE;
   const bool conv = P.flux_mode != FLUX_WENO;
   const bool weno = P.flux_mode != FLUX_CENTRAL;
   constexpr int TY = STREAMS_MARCH_TY;
-#define STREAMS_MAIN(V, C, W) return launch_march<L, LV, V, C, W, TY>(P, sa, st)
+#define STREAMS_MAIN(V, C, W) return launch_march<L, LV, V, C, W, TY>(P, mp, sa, st)
   if (visc && conv && weno) STREAMS_MAIN(true, true, true);
   else if (visc && conv) STREAMS_MAIN(true, true, false);
   else if (visc) STREAMS_MAIN(true, false, true);
@@ -745,6 +774,36 @@ static int launch_main_T(const DevP& P, const StageArgs& sa, cudaStream_t st) {
   else if (conv) STREAMS_MAIN(false, true, false);
   else STREAMS_MAIN(false, false, true);
 #undef STREAMS_MAIN
+}
+
+// TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point: libstreams does not link
+// libcuda).  All four tensors are 4-D (x, y, z, field) views of padded fields: the primitives + dilatation
+// (DevP::q, NF fields), w and R (5 fields each).
+int make_march_maps(const DevP& P, MarchMaps* maps) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return -1;
+  const encode_fn encode = (encode_fn)fn;
+  constexpr int TY = STREAMS_MARCH_TY;
+  const cuuint32_t nf = P.visc_law != VISC_NONE ? 9 : 6;
+  const cuuint64_t strides[3] = {(cuuint64_t)P.px * 8, (cuuint64_t)P.sz * 8, (cuuint64_t)P.fs * 8};
+  const cuuint32_t ones[4] = {1, 1, 1, 1};
+  auto make = [&](CUtensorMap* m, void* base, cuuint64_t nfields, cuuint32_t bx, cuuint32_t by, cuuint32_t bf) {
+    const cuuint64_t dims[4] = {(cuuint64_t)P.px, (cuuint64_t)P.py, (cuuint64_t)P.pz, nfields};
+    const cuuint32_t box[4] = {bx, by, 1, bf};
+    return encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  };
+  if (make(&maps->centre, P.q, nf, MarchGeom<TY>::ROW, MarchGeom<TY>::ROWS, nf) != CUDA_SUCCESS) return -2;
+  if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
+  if (make(&maps->w, P.w, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
+  if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
+  return 0;
 }
 
 template <int L, int R>
@@ -765,9 +824,9 @@ bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
   return L == 3 && lv == 3 && rr == 3;
 }
 
-int launch_rhs_main(const DevP& P, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
+int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
-  return launch_main_T<3, 3, 3>(P, sa, st);
+  return launch_main_T<3, 3, 3>(P, mp, sa, st);
 }
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
