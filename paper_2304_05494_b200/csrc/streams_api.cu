@@ -221,7 +221,8 @@ cudaError_t prof_drain(streams_ctx* ctx) {
 int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
-  timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, st); });
+  const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0);
+  timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
   if (want_dt) timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, st); });
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;

@@ -21,11 +21,16 @@ __device__ __forceinline__ double viscosity(const DevP& P, double T) {
   return P.mu_ref * pow(t, P.pow_exp);
 }
 
-template <bool VISC, bool STORE_C>
+// With DT the same pass takes the time-step rate of every interior node (a9, O5 / S13): max over
+// directions of (|u_d| + c) m_d, nu m_d^2, gamma nu m_d^2 / Pr, reduced by warp shuffles on the bit patterns
+// (rates are non-negative, so unsigned order = numeric order, and a NaN wins and is detected) and one
+// atomicMax per block.
+template <bool VISC, bool STORE_C, bool DT>
 __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
-  if (i < -P.ng || i >= P.nx + P.ng) return;
+  double rmax = 0.0;
+  if (i >= -P.ng && i < P.nx + P.ng) {
   int is = i, js = j, ks = k;
   bool fsx = false, fsy = false, fsz = false;
   double t_wall = 0.0;
@@ -91,12 +96,48 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
   P.q[Q_H * P.fs + n] = (s[4] + pp) / rho;
   P.q[Q_P * P.fs + n] = pp;
   P.q[Q_RHO * P.fs + n] = rho;
+  double mu = 0.0;
   if (VISC) {
     const double TT = pp / (rho * P.rgas);
+    mu = viscosity(P, TT);
     P.q[Q_T * P.fs + n] = TT;
-    P.q[Q_MU * P.fs + n] = viscosity(P, TT);
+    P.q[Q_MU * P.fs + n] = mu;
   }
-  if (STORE_C) P.q[Q_C * P.fs + n] = sqrt(P.gamma * pp / rho);
+  double cc = 0.0;
+  if (STORE_C || DT) cc = sqrt(P.gamma * pp / rho);
+  if (STORE_C) P.q[Q_C * P.fs + n] = cc;
+  if (DT && !ghost) {
+    const double md[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+    const double vel[3] = {uu, vv, wv};
+    double nu = 0.0;
+    if (VISC) nu = mu / rho;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      rmax = fmax(rmax, (fabs(vel[d]) + cc) * md[d]);
+      if (VISC) {
+        rmax = fmax(rmax, nu * (md[d] * md[d]));
+        rmax = fmax(rmax, (P.gamma * nu / P.prandtl) * (md[d] * md[d]));
+      }
+    }
+    if (!(rmax == rmax) || !(cc == cc)) rmax = __longlong_as_double(0x7ff8000000000000LL);
+  }
+  }
+  if (DT) {
+    unsigned long long bits = (unsigned long long)__double_as_longlong(rmax);
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+      const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
+      bits = o > bits ? o : bits;
+    }
+    __shared__ unsigned long long sm[4];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = bits;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+      for (int wq = 1; wq < 4; ++wq) bits = sm[wq] > bits ? sm[wq] : bits;
+      if (bits) atomicMax(reinterpret_cast<unsigned long long*>(P.scal + S_RATE), bits);
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -274,58 +315,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   }
 }
 
-// ---------------------------------------------------------------------------------------------
-// a9: time-step reduction (O5 / S13): max over interior nodes and directions of
-// (|u_d| + c) m_d, nu m_d^2, gamma nu m_d^2 / Pr.  Warp-shuffle max on the bit patterns (rates are
-// non-negative, so unsigned order = numeric order, and a NaN wins and is detected), one atomicMax
-// per block.  HBM: ~56 B read per node.
-// ---------------------------------------------------------------------------------------------
-template <bool VISC>
-__global__ void __launch_bounds__(256) dt_kernel(const DevP P) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  double rmax = 0.0;
-  if (i < P.nx && j < P.ny) {
-    const long long n = pidx(P, i, j, k);
-    const double rho = P.q[Q_RHO * P.fs + n];
-    const double pp = P.q[Q_P * P.fs + n];
-    const double c = sqrt(P.gamma * pp / rho);
-    const double md[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
-    const double vel[3] = {P.q[Q_U * P.fs + n], P.q[Q_V * P.fs + n], P.q[Q_W * P.fs + n]};
-    double nu = 0.0;
-    if (VISC) nu = P.q[Q_MU * P.fs + n] / rho;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      rmax = fmax(rmax, (fabs(vel[d]) + c) * md[d]);
-      if (VISC) {
-        rmax = fmax(rmax, nu * (md[d] * md[d]));
-        rmax = fmax(rmax, (P.gamma * nu / P.prandtl) * (md[d] * md[d]));
-      }
-    }
-    if (!(rmax == rmax) || !(c == c)) rmax = __longlong_as_double(0x7ff8000000000000LL);
-  }
-  unsigned long long bits = (unsigned long long)__double_as_longlong(rmax);
-#pragma unroll
-  for (int s = 16; s > 0; s >>= 1) {
-    const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
-    bits = o > bits ? o : bits;
-  }
-  __shared__ unsigned long long sm[8];
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-  if ((tid & 31) == 0) sm[tid >> 5] = bits;
-  __syncthreads();
-  if (tid < 32) {
-    bits = tid < (int)((blockDim.x * blockDim.y + 31) >> 5) ? sm[tid] : 0ull;
-#pragma unroll
-    for (int s = 4; s > 0; s >>= 1) {
-      const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
-      bits = o > bits ? o : bits;
-    }
-    if (tid == 0) atomicMax(reinterpret_cast<unsigned long long*>(P.scal + S_RATE), bits);
-  }
-}
-
+// a9, second half: dt = CFL / (the rate fill_prim_kernel<.., DT> reduced), or the fixed step.
 __global__ void dt_finalize_kernel(const DevP P, double dt_fixed) {
   const double rate = P.scal[S_RATE];
   const double dt = dt_fixed > 0.0 ? dt_fixed : P.cfl / rate;
@@ -349,13 +339,19 @@ __global__ void reset_counters_kernel(const DevP P) {
 // -------------------------------------------------------------------------- launch wrappers
 static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }
 
-int launch_fill_prim(const DevP& P, cudaStream_t st) {
+int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st) {
   dim3 b(128), g((P.px + 127) / 128, P.py, P.pz);
   const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
-  if (visc && sc) fill_prim_kernel<true, true><<<g, b, 0, st>>>(P);
-  else if (visc) fill_prim_kernel<true, false><<<g, b, 0, st>>>(P);
-  else if (sc) fill_prim_kernel<false, true><<<g, b, 0, st>>>(P);
-  else fill_prim_kernel<false, false><<<g, b, 0, st>>>(P);
+#define STREAMS_FILL(V, C)                                            \
+  do {                                                                \
+    if (with_dt) fill_prim_kernel<V, C, true><<<g, b, 0, st>>>(P);    \
+    else fill_prim_kernel<V, C, false><<<g, b, 0, st>>>(P);           \
+  } while (0)
+  if (visc && sc) STREAMS_FILL(true, true);
+  else if (visc) STREAMS_FILL(true, false);
+  else if (sc) STREAMS_FILL(false, true);
+  else STREAMS_FILL(false, false);
+#undef STREAMS_FILL
   return 1;
 }
 
@@ -395,15 +391,8 @@ int launch_flags(const DevP& P, int r, cudaStream_t st) {
 }
 
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st) {
-  int n = 0;
-  if (!(dt_fixed > 0.0)) {
-    dim3 b(64, 4), g = grid2d(P, b);
-    if (P.visc_law != VISC_NONE) dt_kernel<true><<<g, b, 0, st>>>(P);
-    else dt_kernel<false><<<g, b, 0, st>>>(P);
-    ++n;
-  }
   dt_finalize_kernel<<<1, 1, 0, st>>>(P, dt_fixed);
-  return n + 1;
+  return 1;
 }
 
 int launch_step_end(const DevP& P, cudaStream_t st) {

@@ -22,7 +22,7 @@ struct MarchMaps { CUtensorMap centre, ring, w, r; };
 // Returns 0, or a negative code: -1 driver entry point missing, -2 encode failed.
 int make_march_maps(const DevP& P, MarchMaps* maps);
 
-int launch_fill_prim(const DevP& P, cudaStream_t st);
+int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st);   // with_dt: also reduce the time-step rate (a9)
 int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st);
 int launch_flags(const DevP& P, int r, cudaStream_t st);
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);
