@@ -1,5 +1,6 @@
 // C ABI of libstreams (include/streams.h): context, workspace carving, y metrics, and the host
 // driver that sequences the kernels of one RK3 step.  No compute happens on the host.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -21,8 +22,8 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
-  size_t N;
-  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_dF, off_counters, off_R,
+  size_t N, lcap;
+  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_ilist, off_dF, off_counters, off_R,
       off_metrics, off_scal, total;
   int nq;
 };
@@ -91,6 +92,11 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.off_theta = take(S.N * 8);
   S.off_mask = take(S.fs);
   S.off_nflag = take(hyb ? S.fs : 256);
+  {
+    const size_t face = std::max(std::max((size_t)g->ny * g->nz, (size_t)g->nx * g->nz), (size_t)g->nx * g->ny);
+    S.lcap = align_up(S.N + face, 64);
+    S.off_ilist = take(hyb ? 3 * S.lcap * 4 : 256);
+  }
   S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
   S.off_counters = take(C_COUNT * 4);
   S.off_R = take(5 * S.fs * 8);
@@ -287,6 +293,8 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.theta = (double*)(ctx->base + S.off_theta);
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
   P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
+  P.ilist = (int*)(ctx->base + S.off_ilist);
+  P.lcap = (long long)S.lcap;
   P.dF = (double*)(ctx->base + S.off_dF);
   P.counters = (int*)(ctx->base + S.off_counters);
   P.R = (double*)(ctx->base + S.off_R);

@@ -249,6 +249,8 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nwords = (long long)nwx * P.ny * P.nz;
   int cnt[5] = {0, 0, 0, 0, 0};      // flagged nodes, shock nodes, interfaces x, y, z
+  unsigned long long hiw[3] = {0ull, 0ull, 0ull}, first[3] = {0ull, 0ull, 0ull};   // flagged interfaces named by their
+  int n0w = 0;                                                                    // left node: plus sides, pencil starts
   if (t < nwords) {
     const int iw = (int)(t % nwx);
     const long long t2 = t / nwx;
@@ -289,29 +291,72 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
     cnt[0] = __popcll(cur & valid & 0x0101010101010101ull);
     cnt[1] = __popcll(any);
     // every interface is counted by its left node; the one below the first node of a pencil by that node
-    cnt[2] = __popcll(hi[0]) + (i0 == 0 ? (int)(lo[0] & 1ull) : 0);
-    cnt[3] = __popcll(hi[1]) + (j == 0 ? __popcll(lo[1]) : 0);
-    cnt[4] = __popcll(hi[2]) + (k == 0 ? __popcll(lo[2]) : 0);
+    n0w = (int)n0;
+    first[0] = i0 == 0 ? (lo[0] & 1ull) : 0ull;
+    first[1] = j == 0 ? lo[1] : 0ull;
+    first[2] = k == 0 ? lo[2] : 0ull;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      hiw[d] = hi[d];
+      cnt[2 + d] = __popcll(hi[d]) + __popcll(first[d]);
+    }
   }
-  __shared__ int s_cnt[5];
-  if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+  // counters 0, 1: warp-shuffle sums, one atomic per block
+  __shared__ int s_cnt[2];
+  __shared__ int s_wsum[3][8], s_base[3];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
   __syncthreads();
 #pragma unroll
-  for (int c = 0; c < 5; ++c) {
+  for (int c = 0; c < 2; ++c) {
     int v = cnt[c];
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
-    if ((threadIdx.x & 31) == 0 && v) atomicAdd(&s_cnt[c], v);
+    if (lane == 0 && v) atomicAdd(&s_cnt[c], v);
+  }
+  // flagged interfaces: exclusive scan over the block, one atomic per direction per block reserves the
+  // block's range of the direction's work list (DevP::ilist), every thread writes its own entries
+  int off[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int v = cnt[2 + d];
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+      const int t2 = __shfl_up_sync(0xffffffffu, v, s);
+      if (lane >= s) v += t2;
+    }
+    if (lane == 31) s_wsum[d][wid] = v;
+    off[d] = v - cnt[2 + d];
   }
   __syncthreads();
-  if (threadIdx.x < 5 && s_cnt[threadIdx.x]) {
-    const int c = threadIdx.x, v = s_cnt[c];
-    unsigned long long* cum = reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS);
-    // counters: C_NFLAGGED, C_NSHOCK, C_NIFACE + d; totals: [0] shock, [1] flagged, [3 + d] interfaces
-    const int slot = c == 0 ? C_NFLAGGED : (c == 1 ? C_NSHOCK : C_NIFACE + (c - 2));
-    const int cslot = c == 0 ? 1 : (c == 1 ? 0 : 3 + (c - 2));
-    atomicAdd(&P.counters[slot], v);
-    atomicAdd(&cum[cslot], (unsigned long long)v);
+  if (threadIdx.x < 3) {
+    const int d = threadIdx.x;
+    int run = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { const int t2 = s_wsum[d][w]; s_wsum[d][w] = run; run += t2; }
+    int base = 0;
+    if (run) {
+      base = atomicAdd(&P.counters[C_NIFACE + d], run);
+      atomicAdd(&reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[3 + d], (unsigned long long)run);
+    }
+    s_base[d] = base;
+  } else if (threadIdx.x >= 32 && threadIdx.x < 34 && s_cnt[threadIdx.x - 32]) {
+    // counters: C_NFLAGGED, C_NSHOCK; totals: [0] shock, [1] flagged
+    const int c = threadIdx.x - 32, v = s_cnt[c];
+    atomicAdd(&P.counters[c == 0 ? C_NFLAGGED : C_NSHOCK], v);
+    atomicAdd(&reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[c == 0 ? 1 : 0], (unsigned long long)v);
+  }
+  __syncthreads();
+  if (t < nwords) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      if (cnt[2 + d] == 0) continue;
+      int* __restrict__ Lst = P.ilist + (long long)d * P.lcap + s_base[d] + s_wsum[d][wid] + off[d];
+      unsigned long long wl = first[d], wh = hiw[d];
+      const int nl = n0w - (int)(d == 0 ? 1 : (d == 1 ? P.sy : P.sz));
+      while (wl) { *Lst++ = nl + ((__ffsll((long long)wl) - 1) >> 3); wl &= wl - 1; }
+      while (wh) { *Lst++ = n0w + ((__ffsll((long long)wh) - 1) >> 3); wh &= wh - 1; }
+    }
   }
 }
 

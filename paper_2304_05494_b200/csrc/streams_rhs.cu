@@ -723,6 +723,37 @@ __global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_kernel(const DevP
   else weno_block<2, L, R, DENSE>(P, b - nb0 - nb1, s_list, &s_count, s_st);
 }
 
+// ---------------------------------------------------------------------------------------------
+// weno_list_kernel (hybrid mode): the flagged interfaces of each direction were compacted into global work
+// lists by flags_kernel (DevP::ilist, counts in DevP::counters), so every warp here is full of WENO work
+// whatever the activation pattern.  Persistent blocks walk groups of WTH consecutive list entries
+// (consecutive entries are mostly consecutive nodes: coalesced stencil loads), directions one after the other.
+// ---------------------------------------------------------------------------------------------
+template <int D, int L, int R>
+__device__ __forceinline__ void weno_list_item(const DevP& P, int e, int count, double* s_st) {
+  if (e >= count) return;
+  const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
+  const long long n = P.ilist[(long long)D * P.lcap + e];
+  double fw[5], fc[5];
+  weno_flux<D, R>(P, n, s, fw, s_st + threadIdx.x);
+  central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);
+  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q] - fc[q];
+}
+
+template <int L, int R>
+__global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_list_kernel(const DevP P) {
+  __shared__ double s_st[6 * 2 * R * WTH];
+  const int c0 = P.counters[C_NIFACE], c1 = P.counters[C_NIFACE + 1], c2 = P.counters[C_NIFACE + 2];
+  const int g0 = (c0 + WTH - 1) / WTH, g1 = (c1 + WTH - 1) / WTH, g2 = (c2 + WTH - 1) / WTH;
+  for (int g = blockIdx.x; g < g0 + g1 + g2; g += gridDim.x) {
+    if (g < g0) weno_list_item<0, L, R>(P, g * WTH + threadIdx.x, c0, s_st);
+    else if (g < g0 + g1) weno_list_item<1, L, R>(P, (g - g0) * WTH + threadIdx.x, c1, s_st);
+    else weno_list_item<2, L, R>(P, (g - g0 - g1) * WTH + threadIdx.x, c2, s_st);
+  }
+}
+
 // -------------------------------------------------------------------------- launch
 // z chunks per tile: enough blocks to fill every SM slot in whole waves, long enough that the ring fill
 // (6 planes of loads, no arithmetic) stays a small part of a chunk.
@@ -813,7 +844,7 @@ static int launch_weno_T(const DevP& P, cudaStream_t st) {
   auto blocks = [&](long long extra) { return (int)((a + extra + WCH - 1) / WCH); };
   const int nb0 = blocks((long long)P.ny * P.nz), nb1 = blocks((long long)P.nx * P.nz), nb2 = blocks((long long)P.nx * P.ny);
   dim3 b(WTH), g((unsigned)(nb0 + nb1 + nb2));
-  if (P.flux_mode == FLUX_HYBRID) weno_kernel<L, R, false><<<g, b, 0, st>>>(P, nb0, nb1);
+  if (P.flux_mode == FLUX_HYBRID) weno_list_kernel<L, R><<<P.nsm * STREAMS_WENO_MINB, b, 0, st>>>(P);
   else weno_kernel<L, R, true><<<g, b, 0, st>>>(P, nb0, nb1);
   return 1;
 }
