@@ -131,8 +131,8 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # fp64 instructions per unit of work (thread-level DFMA + DADD + DMUL of the straight-line SASS of each
 # kernel, `cuobjdump -sass`, orders 6/5/6)
-FP64_INST = {"rhs_main_cv": 631, "rhs_main_c": 310, "rhs_main_v": 335, "rhs_main_0": 17,
-             "weno_hybrid": 1422, "weno_dense": 1320, "fill_prim": 289, "sensor": 144, "rhs_apply": 111, "dt": 90}
+FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 30,
+             "weno_hybrid": 1085, "weno_dense": 975, "fill_prim": 270, "fill_prim_dt": 32, "sensor": 135}
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
 
 
@@ -153,26 +153,26 @@ def work_model(case, act):
     n_sh = act["shock"] * N if hyb else (N if weno else 0)
     B, I = {}, {}
     B["fill_prim"] = Np * (40 + 8 * nprim) + (Np - N) * 40     # read w, write primitives, write ghost w
-    I["fill_prim"] = Np * FP64_INST["fill_prim"]
+    I["fill_prim"] = Np * FP64_INST["fill_prim"] + N * FP64_INST["fill_prim_dt"] / 3.0   # dt rate: first stage only
     B["sensor"] = N * (24 + 8 + (1 if hyb else 0))             # read u v w, write div [mask]
     I["sensor"] = N * FP64_INST["sensor"]
-    B["flags"] = N * (1 + 1) + n_sh * 4 + n_if * 4             # read mask, write flags byte, append to lists
+    B["flags"] = N * (1 + 1) + n_if * 4                        # read mask, write flags byte, append to the work lists
     I["flags"] = 0
     # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
     # read R_prev (stages 2, 3), write R (stages 1, 2)
+    # (+ hybrid / WENO: the flag byte of every node and the 5 flux corrections of every flagged interface)
     per_point = (48 if conv else 0) + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40
-    B["rhs_main"] = N * per_point
-    I["rhs_main"] = N * FP64_INST["rhs_main_" + (("c" if conv else "") + ("v" if visc else "") or "0")]
+    B["rhs_main"] = N * per_point + (N * 1 if hyb else 0) + n_if * 40
+    I["rhs_main"] = (N * FP64_INST["rhs_main_" + (("c" if conv else "") + ("v" if visc else "") or "0")]
+                     + n_sh * FP64_INST["rhs_corr"])
     # WENO: per flagged interface one new stencil node of 7 fields (runs of flagged interfaces share the
     # rest), a list entry, 5 flux values out
     B["weno"] = n_if * (56 + 4 + 40)                           # per timed group: the x, y and z launches of a stage
     I["weno"] = n_if * FP64_INST["weno_hybrid" if hyb else "weno_dense"]
-    # apply: flags byte + list entry, 2 x 5 flux values per direction (shared with the neighbour: 5),
-    # read-modify-write of w and (2 stages of 3) R
-    B["rhs_apply"] = n_sh * (1 + 4 + 3 * 40 + 80 + (2.0 / 3.0) * 80)
-    I["rhs_apply"] = n_sh * FP64_INST["rhs_apply"]
-    B["dt"] = N * (40 + (8 if visc else 0))                    # rho p u v w [mu]
-    I["dt"] = N * FP64_INST["dt"]
+    B["rhs_apply"] = 0                                         # (class kept for the ABI's kernel table; not launched)
+    I["rhs_apply"] = 0
+    B["dt"] = 0                                                # the rate is reduced inside fill_prim; this class is
+    I["dt"] = 0                                                # the one-thread finalize (dt = CFL / rate)
     B["misc"] = 0
     I["misc"] = 0
     return B, I, per_point

@@ -5,6 +5,7 @@
 // mask is then bit-identical to any IEEE evaluation of the same formulas on the same state.
 #include "streams_dev.cuh"
 #include "streams_launch.h"
+#include "streams_tma.cuh"
 
 namespace streams {
 
@@ -223,6 +224,135 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// sensor_march_kernel: the same sensor (identical operations in identical order, so identical bits) as a
+// z-marching kernel like rhs_march_kernel (streams_rhs.cu): a block owns a 32 x TY tile and a chunk of z
+// planes; the centre plane of (u, v, w) with its halo is one 4-D TMA box per plane (two buffers, issued two
+// planes ahead), the z neighbours live in a 7-plane register ring fed by a second TMA box per plane.
+// HBM: 24 B read + 8 B (div) + 1 B (mask) write per node; every stencil offset is an immediate.
+// ---------------------------------------------------------------------------------------------
+template <int TY>
+struct SensorSmem {
+  using G = MarchGeom<TY>;
+  static constexpr size_t BUF = (size_t)3 * G::PLANE * 8, RING = (size_t)3 * G::NT * 8;
+  static constexpr size_t OFF_RING = 2 * BUF, OFF_BAR = OFF_RING + 2 * RING, TOTAL = OFF_BAR + 64;
+  static_assert(BUF % 128 == 0 && RING % 128 == 0, "TMA destinations are 128-byte aligned");
+};
+
+// acc = a_1 d_1; acc = acc + a_l d_l; derivative = acc * metric (canonical order), G(o) = value at offset o
+template <int L, class G>
+__device__ __forceinline__ double ddc_g(const DevP& P, const G& g, double metric) {
+  double acc = P.a1[0] * (g(1) - g(-1));
+#pragma unroll
+  for (int l = 2; l <= L; ++l) acc = acc + P.a1[l - 1] * (g(l) - g(-l));
+  return acc * metric;
+}
+
+template <bool MASK, bool THETA, int TY>
+__global__ void __launch_bounds__(MTX * TY, 3)
+sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring, const DevP P,
+                    int nbx, int nby, int kz) {
+  using G = MarchGeom<TY>;
+  using SM = SensorSmem<TY>;
+  constexpr int L = 3, NG = 3;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][3][PLANE]
+  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][3][NT]
+  unsigned long long* const full_c = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
+  unsigned long long* const full_r = full_c + 2;
+
+  const int tid = threadIdx.x;
+  const int tx = tid & 31, ty = tid >> 5;
+  int bid = blockIdx.x;
+  const int bx = bid % nbx; bid /= nbx;
+  const int by = bid % nby;
+  const int bc = bid / nby;
+  const int i0 = bx * MTX, j0 = by * TY;
+  const int kb = bc * kz, ke = min(P.nz, kb + kz);
+  if (kb >= ke) return;
+  const int i = i0 + tx, j = j0 + ty;
+  const bool active = i < P.nx && j < P.ny;
+  const int ic = min(i, P.nx + P.ng - 1), jc = min(j, P.ny + P.ng - 1);
+  const int isz = (int)P.sz;
+  const int ncol = (int)pidx(P, ic, jc, 0);
+  const int s0 = (ty + 3) * G::ROW + tx + 4;
+  const int cx0 = i0 + P.ox, cy0 = j0 + P.ng;
+
+  auto issue_centre = [&](int k, int b) {
+    mbar_expect_tx(&full_c[b], (unsigned)SM::BUF);
+    tma_load_4d(buf + (size_t)b * 3 * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - 3, k + P.ng, 0);
+  };
+  auto issue_ring = [&](int k, int b) {              // ring plane k+4 into slot b
+    mbar_expect_tx(&full_r[b], (unsigned)SM::RING);
+    tma_load_4d(ring + (size_t)b * 3 * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + 1 + P.ng, 0);
+  };
+  if (tid == 0) {
+    mbar_init(&full_c[0], 1); mbar_init(&full_c[1], 1);
+    mbar_init(&full_r[0], 1); mbar_init(&full_r[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    issue_centre(kb, 0);
+    if (kb + 1 < ke) issue_centre(kb + 1, 1);
+    issue_ring(kb, 0);
+  }
+  const double my = P.eta_y_c[min(j, P.ny - 1)];
+  double zr[3][2 * NG + 1];
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    const double* __restrict__ fp = P.q + (long long)f * P.fs + ncol + (long long)(kb - NG) * P.sz;
+#pragma unroll
+    for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
+  }
+
+  for (int k = kb; k < ke; ++k) {
+    const int it = k - kb, b = it & 1;
+    const unsigned par = (unsigned)(it >> 1) & 1u;
+    mbar_wait(&full_c[b], par);
+    const double* __restrict__ sc = buf + (size_t)b * 3 * G::PLANE + s0;
+    double gx[3], gy[3], gz[3];
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+      gx[f] = ddc_g<L>(P, [&](int o) { return sc[f * G::PLANE + o]; }, P.inv_dx);
+      gy[f] = ddc_g<L>(P, [&](int o) { return sc[f * G::PLANE + o * G::ROW]; }, my);
+      gz[f] = ddc_g<L>(P, [&](int o) { return zr[f][NG + o]; }, P.inv_dz);
+    }
+    if (tid >> 5) {
+      if (b) asm volatile("bar.arrive 2, %0;" ::"n"(G::NT) : "memory");
+      else asm volatile("bar.arrive 1, %0;" ::"n"(G::NT) : "memory");
+    } else {
+      if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
+      else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
+      if (tid == 0) {
+        if (k + 2 < ke) issue_centre(k + 2, b);
+        if (k + 1 < ke) issue_ring(k + 1, b ^ 1);
+      }
+    }
+    const double dv = (gx[0] + gy[1]) + gz[2];
+    if (active) {
+      const long long n = ncol + (long long)k * isz;
+      P.div[n] = dv;
+      if (MASK || THETA) {
+        const double ox = gy[2] - gz[1], oy = gz[0] - gx[2], oz = gx[1] - gy[0];
+        const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
+        double th = -dv / sqrt(s);
+        if (!(th > 0.0)) th = 0.0;
+        if (THETA) P.theta[iidx(P, i, j, k)] = th;
+        if (MASK) P.mask[n] = (th > P.thr) ? 1 : 0;
+      }
+    }
+    mbar_wait(&full_r[b], par);
+    const double* __restrict__ rn = ring + (size_t)b * 3 * G::NT + tid;
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+#pragma unroll
+      for (int m = 0; m < 2 * NG; ++m) zr[f][m] = zr[f][m + 1];
+      zr[f][2 * NG] = rn[f * G::NT];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Interface flags (O2 / S5): interface n+1/2 along d uses WENO iff any node of its 2r-node
 // stencil {n-r+1..n+r} is flagged.  Per interior node the six adjacent interfaces are packed in a byte
 // (bit 2d: minus side, bit 2d+1: plus side), stored at the node's padded index.
@@ -412,7 +542,33 @@ static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st
   else scalar_ghost_kernel<false><<<gg, 256, 0, st>>>(P);
   return 2;
 }
-int launch_sensor(const DevP& P, int L, bool mask, bool theta, cudaStream_t st) {
+template <bool MASK, bool THETA>
+static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t st) {
+  constexpr int TY = STREAMS_MARCH_TY;
+  using SM = SensorSmem<TY>;
+  auto kern = sensor_march_kernel<MASK, THETA, TY>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
+    attr_set = true;
+  }
+  const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
+  const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * 3);
+  const int kz = (P.nz + chunks - 1) / chunks;
+  kern<<<(unsigned)(nbx * nby * chunks), MTX * TY, SM::TOTAL, st>>>(mp.s_centre, mp.s_ring, P, nbx, nby, kz);
+  const long long ghosts = 2LL * P.ng * ((long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny);
+  dim3 gg((unsigned)((ghosts + 255) / 256));
+  if (MASK) scalar_ghost_kernel<true><<<gg, 256, 0, st>>>(P);
+  else scalar_ghost_kernel<false><<<gg, 256, 0, st>>>(P);
+  return 2;
+}
+
+int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool theta, cudaStream_t st) {
+  if (L == 3 && P.ng == 3) {
+    if (theta) return launch_sensor_march<true, true>(P, mp, st);
+    if (mask) return launch_sensor_march<true, false>(P, mp, st);
+    return launch_sensor_march<false, false>(P, mp, st);
+  }
   switch (L) {
     case 1: return launch_sensor_L<1>(P, mask, theta, st);
     case 2: return launch_sensor_L<2>(P, mask, theta, st);

@@ -1,0 +1,79 @@
+// TMA / mbarrier / cp.async primitives and the tile geometry shared by the z-marching kernels
+// (rhs_march_kernel in streams_rhs.cu, sensor_march_kernel in streams_canon.cu).  sm_100a only.
+#pragma once
+#include <cuda.h>
+#include "streams_dev.cuh"
+
+#ifndef STREAMS_MARCH_TY
+#define STREAMS_MARCH_TY 8
+#endif
+
+namespace streams {
+
+// ------------------------------------------------------------------ async-copy / mbarrier / TMA primitives
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// copies 8 bytes when `take`, writes zeros (and reads nothing) otherwise
+__device__ __forceinline__ void cp_async8_zfill(void* smem_dst, const void* gsrc, bool take) {
+  const unsigned n = take ? 8u : 0u;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// a load the compiler may not sink to its first use
+__device__ __forceinline__ unsigned ld_u8_now(const unsigned char* p) {
+  unsigned v;
+  asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// one box of a 4-D tensor (x, y, z, field) into shared memory, completion counted on `bar`
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1,
+                                            int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::
+          "r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
+
+constexpr int MTX = 32;
+
+template <int TY>
+struct MarchGeom {
+  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (3 used), rows stay 32 B aligned
+  static constexpr int ROWS = TY + 6;
+  static constexpr int PLANE = ROW * ROWS;       // doubles per field per buffer
+  static constexpr int NT = MTX * TY;
+};
+
+// z chunks per tile: enough blocks to fill every SM slot in whole waves, long enough that the ring fill
+// (6 planes of loads, no arithmetic) stays a small part of a chunk.
+static inline int pick_chunks(int tiles, int nz, int slots) {
+  int best_c = 1;
+  double best = 1e300;
+  for (int c = 1; c <= (nz + 3) / 4; ++c) {
+    const int kz = (nz + c - 1) / c, ce = (nz + kz - 1) / kz;
+    const long long waves = ((long long)tiles * ce + slots - 1) / slots;
+    const double cost = (double)waves * (kz + 1.0);
+    if (cost < best - 1e-9) { best = cost; best_c = ce; }
+  }
+  return best_c;
+}
+
+}  // namespace streams
