@@ -324,8 +324,8 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
       if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
       else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
       if (tid == 0) {
+        if (k + 1 < ke) issue_ring(k + 1, b ^ 1);       // needed first
         if (k + 2 < ke) issue_centre(k + 2, b);
-        if (k + 1 < ke) issue_ring(k + 1, b ^ 1);
       }
     }
     const double dv = (gx[0] + gy[1]) + gz[2];

@@ -180,7 +180,10 @@ struct MarchSmem {
 };
 
 template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
-__global__ void __launch_bounds__(MTX * TY, 1)
+#ifndef STREAMS_MARCH_MINB
+#define STREAMS_MARCH_MINB 1
+#endif
+__global__ void __launch_bounds__(MTX * TY, STREAMS_MARCH_MINB)
 rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
                  const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r, const DevP P,
                  const StageArgs sa, int nbx, int nby, int kz) {
@@ -330,8 +333,8 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
       else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
       if (tid == 0) {
+        if (k + 1 < ke) issue_ring_epi(k + 1, b ^ 1);   // needed one plane from now: ahead of the larger centre box
         if (k + 2 < ke) issue_centre(k + 2, b);
-        if (k + 1 < ke) issue_ring_epi(k + 1, b ^ 1);
       }
     }
 
@@ -453,153 +456,166 @@ __device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// WENO characteristic flux at interface n+1/2 along D (O3).  Characteristic projections are formed
-// from primitives: l.W = rho (l0 + l1 u + l2 v + l3 w + l4 H) - l4 p and
-// l.F = u_D (l.W) + p (l_{1+D} + l4 u_D), since F = u_D W + p (0, e_D, u_D); for the two shear fields
-// (l = (-vbar_t, e_t, 0)) this collapses to l.W = rho (v_t - vbar_t), l.F = u_D (l.W).
-// One characteristic field at a time (5 x 2 reconstructions).  The 2R-node stencil of (rho, u, v, w, H, p)
-// lives in a per-thread column of shared memory (st[(f * 2R + m) * WTH], conflict-free), not in registers:
-// the kernel then fits 4 blocks of 128 threads per SM instead of 2.
+// WENO characteristic flux at interface n+1/2 along D (O3), and the central flux (O1) it replaces.
+// Characteristic projections are formed from primitives: with W the conserved state and
+// F = u_D W + p (0, e_D, u_D), l.W = rho (l0 + l1 u + l2 v + l3 w + l4 H) - l4 p and
+// l.F = u_D (l.W) + p (l_{1+D} + l4 u_D).  With b1 = (gamma-1)/c^2, b2 = b1 q^2/2 and the 1/2 of the
+// Lax-Friedrichs splitting folded into l, the three non-shear rows share per node
+//   A  = [rho (b2 - b1 vbar.v + b1 H) - b1 p] / 4        B  = rho (un - u_D) / (4 c)
+//   FA = u_D A + b1 p (u_D - un) / 4                     FB = u_D B - p / (4 c)
+// as  u-c: (l.W, l.F) = (A + B, FA + FB);  u+c: (A - B, FA - FB);  entropy: (rho/2 - 2A, rho u_D/2 - 2FA);
+// the two shear rows (l = (-vbar_t, e_t, 0)) collapse to l.W = rho (v_t - vbar_t)/2, l.F = u_D (l.W).
+// The 2R-node stencil of (rho, u, v, w, H, p) lives in a per-thread column of shared memory
+// (st[(f * 2R + m) * WTH], conflict-free) so that the kernel fits 4 blocks of 128 threads per SM; every node is
+// read once per pass (central pairs, shared rows, entropy row, shear rows): ~120 loads per interface.
 // ---------------------------------------------------------------------------------------------
 constexpr int WTH = 128;       // threads per block of weno_kernel
 constexpr int WCH = 2048;      // interface slots per block
 
-template <int D, int R>
-__device__ __forceinline__ void weno_flux(const DevP& P, long long n, long long s, double f[5], double* __restrict__ st) {
-  constexpr int NS = 2 * R;
-  enum { F_RHO = 0, F_U = 1, F_V = 2, F_W = 3, F_H = 4, F_P = 5 };
 #define ST(fld, m) (((volatile double*)st)[((fld) * NS + (m)) * WTH])
-  double lam_m = 0.0, lam_0 = 0.0, lam_p = 0.0;
+enum { SF_RHO = 0, SF_U = 1, SF_V = 2, SF_W = 3, SF_H = 4, SF_P = 5 };
+
+// Central interface flux (O1) from the shared-memory stencil (needs L <= R): the flux that rhs_march_kernel's
+// pair-difference form implies at this interface.  f = 1/4 sum_l a_l sum_{m<l} (rho_a+rho_b)(ud_a+ud_b)(phi_a+phi_b),
+// pairs (a, b) = (n-m, n-m+l).  The L left nodes stay in registers, the right nodes stream past them.
+template <int D, int L, int R>
+__device__ __forceinline__ void central_flux_st(const DevP& P, double f[5], const double* st) {
+  static_assert(L <= R, "the central stencil must fit in the WENO stencil");
+  constexpr int NS = 2 * R;
+  double lf[L][6];                                 // left nodes n, n-1, .., n-L+1: rho, u, v, w, H, p
+#pragma unroll
+  for (int m = 0; m < L; ++m) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) lf[m][q] = ST(q, R - 1 - m);
+  }
+  double fs[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ps = 0.0;
+#pragma unroll
+  for (int j = 0; j < L; ++j) {                    // right node n+1+j pairs with left node n-m at distance l = j+1+m
+    double rt[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) rt[q] = ST(q, R + j);
+#pragma unroll
+    for (int m = 0; m + j < L; ++m) {
+      const double al = P.a1[j + m];
+      const double ru = (al * (lf[m][SF_RHO] + rt[SF_RHO])) * (lf[m][SF_U + D] + rt[SF_U + D]);
+      fs[0] += ru;
+#pragma unroll
+      for (int q = 1; q < 5; ++q) fs[q] = fma(ru, lf[m][q] + rt[q], fs[q]);
+      ps = fma(al, lf[m][SF_P] + rt[SF_P], ps);
+    }
+  }
+  f[0] = 0.5 * fs[0];
+#pragma unroll
+  for (int q = 1; q < 5; ++q) f[q] = 0.25 * fs[q];
+  f[1 + D] += ps;
+}
+
+// Fills the stencil column of interface n+1/2 (left node index n, stride s along D) and returns the local
+// Lax-Friedrichs speeds max |u_D - c|, |u_D|, |u_D + c| over its 2R nodes.
+template <int D, int R>
+__device__ __forceinline__ void weno_stencil(const DevP& P, long long n, long long s, double* __restrict__ st, double lam[3]) {
+  constexpr int NS = 2 * R;
+  lam[0] = lam[1] = lam[2] = 0.0;
 #pragma unroll
   for (int m = 0; m < NS; ++m) {
     const long long a = n + (long long)(m - R + 1) * s;
     const double u = P.q[Q_U * P.fs + a], v = P.q[Q_V * P.fs + a], w = P.q[Q_W * P.fs + a];
     const double c = P.q[Q_C * P.fs + a];
-    ST(F_RHO, m) = P.q[Q_RHO * P.fs + a];
-    ST(F_U, m) = u;
-    ST(F_V, m) = v;
-    ST(F_W, m) = w;
-    ST(F_H, m) = P.q[Q_H * P.fs + a];
-    ST(F_P, m) = P.q[Q_P * P.fs + a];
+    ST(SF_RHO, m) = P.q[Q_RHO * P.fs + a];
+    ST(SF_U, m) = u;
+    ST(SF_V, m) = v;
+    ST(SF_W, m) = w;
+    ST(SF_H, m) = P.q[Q_H * P.fs + a];
+    ST(SF_P, m) = P.q[Q_P * P.fs + a];
     const double ud = D == 0 ? u : (D == 1 ? v : w);
-    lam_m = fmax(lam_m, fabs(ud - c));
-    lam_0 = fmax(lam_0, fabs(ud));
-    lam_p = fmax(lam_p, fabs(ud + c));
+    lam[0] = fmax(lam[0], fabs(ud - c));
+    lam[1] = fmax(lam[1], fabs(ud));
+    lam[2] = fmax(lam[2], fabs(ud + c));
   }
+}
+
+template <int D, int R>
+__device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], double f[5], const double* __restrict__ st) {
+  constexpr int NS = 2 * R;
   // Roe average of nodes n (slot R-1) and n+1 (slot R)
-  const double rw = sqrt(ST(F_RHO, R) * rcp_pos(ST(F_RHO, R - 1)));
+  const double rw = sqrt(ST(SF_RHO, R) * rcp_pos(ST(SF_RHO, R - 1)));
   const double iden = rcp_pos(1.0 + rw);
   double vb[3];
 #pragma unroll
-  for (int a = 0; a < 3; ++a) vb[a] = (ST(F_U + a, R - 1) + rw * ST(F_U + a, R)) * iden;
-  const double Hb = (ST(F_H, R - 1) + rw * ST(F_H, R)) * iden;
+  for (int a = 0; a < 3; ++a) vb[a] = (ST(SF_U + a, R - 1) + rw * ST(SF_U + a, R)) * iden;
+  const double Hb = (ST(SF_H, R - 1) + rw * ST(SF_H, R)) * iden;
   const double qq = 0.5 * (vb[0] * vb[0] + vb[1] * vb[1] + vb[2] * vb[2]);
-  const double c2 = P.gm1 * (Hb - qq);
-  const double cb = sqrt(c2);
+  const double cb = sqrt(P.gm1 * (Hb - qq));
   const double ic = rcp_pos(cb);
-  const double b1 = P.gm1 * (ic * ic), b2 = qq * b1;
   const double un = vb[D];
+  const double k1 = 0.25 * (P.gm1 * (ic * ic)), k2 = qq * k1, ki = 0.25 * ic;
   constexpr int T1 = (D == 0) ? 1 : 0;
   constexpr int T2 = (D == 2) ? 1 : 2;
-#pragma unroll
-  for (int q = 0; q < 5; ++q) f[q] = 0.0;
-  // One characteristic field after the other.  The stencil is read through volatile shared-memory loads so
-  // that the compiler cannot hoist all 36 values of every field into registers (it then needs > 200).
-#pragma unroll
-  for (int sc = 0; sc < 5; ++sc) {
-    double gp[NS], gm[NS];
-    double rv[5];                                   // right eigenvector of this field
-    if (sc == 2 || sc == 3) {
-      const int t = (sc == 2) ? T1 : T2;
-      const double vbt = t == 0 ? vb[0] : (t == 1 ? vb[1] : vb[2]);
-      const volatile double* stt = st + (F_U + t) * NS * WTH;
-#pragma unroll
-      for (int m = 0; m < NS; ++m) {
-        const double lw = (0.5 * ST(F_RHO, m)) * (stt[m * WTH] - vbt);   // (l.W) / 2
-        const double lf = ST(F_U + D, m) * lw;                           // (l.F) / 2
-        gp[m] = fma(lam_0, lw, lf);
-        gm[NS - 1 - m] = fma(-lam_0, lw, lf);        // mirrored: gm[0] is node n+R
-      }
-      rv[0] = 0.0;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) rv[1 + a] = (a == t) ? 1.0 : 0.0;
-      rv[4] = vbt;
-    } else {
-      double l0, lv[3], l4, lam;
-      if (sc == 1) {
-        l0 = 0.5 * (1.0 - b2);                      // the 1/2 of the flux splitting is folded into l
-#pragma unroll
-        for (int a = 0; a < 3; ++a) lv[a] = 0.5 * (b1 * vb[a]);
-        l4 = -0.5 * b1;
-        lam = lam_0;
-        rv[0] = 1.0;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) rv[1 + a] = vb[a];
-        rv[4] = qq;
-      } else {
-        const double sg = (sc == 0) ? 1.0 : -1.0;
-        l0 = 0.25 * (b2 + sg * un * ic);
-#pragma unroll
-        for (int a = 0; a < 3; ++a) lv[a] = 0.25 * (-b1 * vb[a] - (a == D ? sg * ic : 0.0));
-        l4 = 0.25 * b1;
-        lam = (sc == 0) ? lam_m : lam_p;
-        rv[0] = 1.0;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) rv[1 + a] = vb[a] - (a == D ? sg * cb : 0.0);
-        rv[4] = Hb - sg * un * cb;
-      }
-#pragma unroll
-      for (int m = 0; m < NS; ++m) {
-        const double um = ST(F_U, m), vm = ST(F_V, m), wm = ST(F_W, m), pm = ST(F_P, m);
-        const double ud = D == 0 ? um : (D == 1 ? vm : wm);
-        const double lw = ST(F_RHO, m) * (l0 + lv[0] * um + lv[1] * vm + lv[2] * wm + l4 * ST(F_H, m)) - l4 * pm;
-        const double lf = ud * lw + pm * (lv[D] + l4 * ud);
-        gp[m] = fma(lam, lw, lf);
-        gm[NS - 1 - m] = fma(-lam, lw, lf);
-      }
-    }
-    const double gh = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
-#pragma unroll
-    for (int q = 0; q < 5; ++q) f[q] += gh * rv[q];
-  }
-#undef ST
-}
+  double gp[NS], gm[NS];
 
-// Central interface flux (O1) from the same shared-memory stencil (needs L <= R): the flux that
-// rhs_main_kernel's pair-difference form implies at this interface, subtracted in hybrid mode.
-template <int D, int L, int R>
-__device__ __forceinline__ void central_flux_st(const DevP& P, double f[5], const double* st) {
-  static_assert(L <= R, "the central stencil must fit in the WENO stencil");
-  constexpr int NS = 2 * R;
-  enum { F_RHO = 0, F_U = 1, F_V = 2, F_W = 3, F_H = 4, F_P = 5 };
-#define ST(fld, m) (((const volatile double*)st)[((fld) * NS + (m)) * WTH])
-  double fs[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ps = 0.0;
+  // shared rows of the two acoustic fields and the entropy field, one pass over the nodes
+  double A[NS], B[NS], FA[NS], FB[NS];
 #pragma unroll
-  for (int l = 1; l <= L; ++l) {
-    double in[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, pin = 0.0;
-#pragma unroll
-    for (int m = 0; m < l; ++m) {
-      const int a = R - 1 - m, b = a + l;          // slots of nodes n - m and n - m + l
-      const double ua = ST(F_U, a), va = ST(F_V, a), wa = ST(F_W, a);
-      const double ub = ST(F_U, b), vb = ST(F_V, b), wb = ST(F_W, b);
-      const double uda = D == 0 ? ua : (D == 1 ? va : wa), udb = D == 0 ? ub : (D == 1 ? vb : wb);
-      const double ru = (ST(F_RHO, a) + ST(F_RHO, b)) * (uda + udb);
-      in[0] += ru * 2.0;
-      in[1] += ru * (ua + ub);
-      in[2] += ru * (va + vb);
-      in[3] += ru * (wa + wb);
-      in[4] += ru * (ST(F_H, a) + ST(F_H, b));
-      pin += ST(F_P, a) + ST(F_P, b);
-    }
-#pragma unroll
-    for (int q = 0; q < 5; ++q) fs[q] += P.a1[l - 1] * in[q];
-    ps += P.a1[l - 1] * pin;
+  for (int m = 0; m < NS; ++m) {
+    const double rho = ST(SF_RHO, m), um = ST(SF_U, m), vm = ST(SF_V, m), wm = ST(SF_W, m), hm = ST(SF_H, m), pm = ST(SF_P, m);
+    const double ud = D == 0 ? um : (D == 1 ? vm : wm);
+    const double dot = fma(vb[2], wm, fma(vb[1], vm, vb[0] * um));
+    const double kp = k1 * pm, du = ud - un;
+    A[m] = fma(rho, fma(k1, hm - dot, k2), -kp);
+    B[m] = -((rho * ki) * du);
+    FA[m] = fma(ud, A[m], kp * du);
+    FB[m] = fma(ud, B[m], -(ki * pm));
   }
+  // u - c
 #pragma unroll
-  for (int q = 0; q < 5; ++q) f[q] = 0.25 * fs[q];
-  f[1 + D] += ps;
-#undef ST
+  for (int m = 0; m < NS; ++m) {
+    const double lw = A[m] + B[m], lf = FA[m] + FB[m];
+    gp[m] = fma(lam[0], lw, lf);
+    gm[NS - 1 - m] = fma(-lam[0], lw, lf);          // mirrored: gm[0] is node n+R
+  }
+  const double g0 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  // u + c
+#pragma unroll
+  for (int m = 0; m < NS; ++m) {
+    const double lw = A[m] - B[m], lf = FA[m] - FB[m];
+    gp[m] = fma(lam[2], lw, lf);
+    gm[NS - 1 - m] = fma(-lam[2], lw, lf);
+  }
+  const double g4 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  // entropy
+#pragma unroll
+  for (int m = 0; m < NS; ++m) {
+    const double hr = 0.5 * ST(SF_RHO, m);
+    const double lw = fma(-2.0, A[m], hr), lf = fma(-2.0, FA[m], hr * ST(SF_U + D, m));
+    gp[m] = fma(lam[1], lw, lf);
+    gm[NS - 1 - m] = fma(-lam[1], lw, lf);
+  }
+  const double g1 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  // the two shear fields
+  double gs[2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int t = e == 0 ? T1 : T2;
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      const double lw = (0.5 * ST(SF_RHO, m)) * (ST(SF_U + t, m) - vb[t]);
+      const double lf = ST(SF_U + D, m) * lw;
+      gp[m] = fma(lam[1], lw, lf);
+      gm[NS - 1 - m] = fma(-lam[1], lw, lf);
+    }
+    gs[e] = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  }
+  // f = sum over the fields of g r: r(u-+c) = (1, vbar -+ c e_D, H -+ un c), r(entropy) = (1, vbar, q^2/2), r(shear t) = (0, e_t, vbar_t)
+  const double gsum = (g0 + g4) + g1, gdc = (g4 - g0) * cb;
+  f[0] = gsum;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) f[1 + a] = vb[a] * gsum;
+  f[1 + D] += gdc;
+  f[1 + T1] += gs[0];
+  f[1 + T2] += gs[1];
+  f[4] = fma(Hb, g0 + g4, fma(un, gdc, fma(qq, g1, fma(vb[T1], gs[0], vb[T2] * gs[1]))));
 }
+#undef ST
 
 // ---------------------------------------------------------------------------------------------
 // weno_kernel: blocks [0, nb0) work on x interfaces, [nb0, nb0 + nb1) on y, the rest on z.  A block owns
@@ -645,8 +661,9 @@ __device__ __forceinline__ void weno_block(const DevP& P, long long chunk, int* 
   double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs;
   for (int e = threadIdx.x; e < count; e += WTH) {
     const long long n = s_list[e];
-    double fw[5];
-    weno_flux<D, R>(P, n, s, fw, s_st + threadIdx.x);
+    double fw[5], lam[3];
+    weno_stencil<D, R>(P, n, s, s_st + threadIdx.x, lam);
+    weno_flux<D, R>(P, lam, fw, s_st + threadIdx.x);
     if (!DENSE) {
       double fc[5];
       central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);
@@ -683,9 +700,10 @@ __device__ __forceinline__ void weno_list_item(const DevP& P, int e, int count, 
   if (e >= count) return;
   const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
   const long long n = P.ilist[(long long)D * P.lcap + e];
-  double fw[5], fc[5];
-  weno_flux<D, R>(P, n, s, fw, s_st + threadIdx.x);
-  central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);
+  double fw[5], fc[5], lam[3];
+  weno_stencil<D, R>(P, n, s, s_st + threadIdx.x, lam);
+  central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);     // first: its registers are free before the WENO rows are live
+  weno_flux<D, R>(P, lam, fw, s_st + threadIdx.x);
   double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
 #pragma unroll
   for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q] - fc[q];
@@ -716,7 +734,7 @@ static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa,
   }
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int tiles = nbx * nby;
-  const int chunks = pick_chunks(tiles, P.nz, P.nsm);
+  const int chunks = pick_chunks(tiles, P.nz, P.nsm * STREAMS_MARCH_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
   kern<<<(unsigned)(tiles * chunks), G::NT, SM::TOTAL, st>>>(mp.centre, mp.ring, mp.w, mp.r, P, sa, nbx, nby, kz);
   return 1;
