@@ -232,6 +232,20 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     if (sa.update_w) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + P.ng, 0);
   };
 
+#ifndef STREAMS_MARCH_PF
+#define STREAMS_MARCH_PF 2
+#endif
+  // The streams that miss L2 (the new ring plane and the RK operands) are needed one plane after they are
+  // issued, which keeps too few bytes in flight to cover the DRAM latency: PF planes further ahead the same
+  // boxes are requested into L2 only.
+  constexpr int PF = (VISC || WENO) ? 0 : STREAMS_MARCH_PF;   // measured: helps the lean variant only
+  auto prefetch_ring_epi = [&](int k) {                // thread 0 only
+    if (PF > 0 && k < ke) {
+      tma_prefetch_4d(&tm_ring, cx0, cy0, k + NG + 1 + P.ng, 0);
+      if (sa.read_prev) tma_prefetch_4d(&tm_r, cx0, cy0, k + P.ng, 0);
+      if (sa.update_w) tma_prefetch_4d(&tm_w, cx0, cy0, k + P.ng, 0);
+    }
+  };
   if (tid == 0) {
     mbar_init(&full_c[0], 1); mbar_init(&full_c[1], 1);
     mbar_init(&full_e[0], 1); mbar_init(&full_e[1], 1);
@@ -242,6 +256,8 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     issue_centre(kb, 0);
     if (kb + 1 < ke) issue_centre(kb + 1, 1);
     issue_ring_epi(kb, 0);
+#pragma unroll
+    for (int a = 1; a <= PF; ++a) prefetch_ring_epi(kb + a);
   }
 
   // metrics of this row (constant along the march)
@@ -271,6 +287,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     const int it = k - kb, b = it & 1;
     const unsigned par = (unsigned)(it >> 1) & 1u;
     const int n = ncol + k * isz;
+    if (tid == G::NT - 32) prefetch_ring_epi(k + 1 + PF);   // no shared-memory hazard: any thread, off the issuing warp's path
     // flags of this plane (prefetched), of the next one, and this plane's flux corrections
     unsigned fl = 0;
     bool any_fl = false;
