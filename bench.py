@@ -47,7 +47,8 @@ def load_peaks():
 
 
 def make_case(index: int, seed_offset: int = 0):
-    """BASELINE.json configs[index] with the rank's seed (replicas differ only by seed)."""
+    """BASELINE.json configs[index] with the rank's seed (replicas differ only by seed: base + 100 * rank,
+    paper_2304_05494_b200.replicas.replica_seed)."""
     if index == 0:
         return W.config(0)
     if index == 1:
@@ -129,10 +130,12 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # algorithmic bytes per launch of each kernel class
 # ------------------------------------------------------------------------------------------------
-# fp64 instructions per unit of work (thread-level DFMA + DADD + DMUL of the straight-line SASS of each
-# kernel, `cuobjdump -sass`, orders 6/5/6)
+# fp64 instructions per unit of work: EXECUTED thread-level DFMA + DADD + DMUL (+ DSETP, MUFU.RCP64H) per node /
+# padded node / flagged interface, orders 6/5/6, from the per-instruction execution counts of the ncu source page
+# (profiles/r1c_fp64_counts.md; static SASS counts overstate kernels with branches: the IEEE-divide slow paths and
+# the wall branch of fill_prim are rarely taken)
 FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 30,
-             "weno_hybrid": 1085, "weno_dense": 975, "fill_prim": 270, "fill_prim_dt": 32, "sensor": 135}
+             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 115}
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
 
 
@@ -243,11 +246,9 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    from paper_2304_05494_b200 import binding, build as kbuild
+    from paper_2304_05494_b200 import binding, build as kbuild, replicas
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.rank_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; libstreams has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
@@ -267,17 +268,12 @@ def run_ours(args):
     dev = gpu.device
     state_bytes = 5 * N * 8
 
-    def sync_all():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
+    rep = replicas.Replicas(dist, dev)          # barrier + max over ranks (tests/test_replicas_gloo.py)
+    max_over_ranks = rep.max_over_ranks
 
-    def max_over_ranks(ms: float) -> float:
-        if dist is None:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    def sync_all():
+        rep.barrier()
+        torch.cuda.synchronize(dev)
 
     # Every timed region starts from the same state: the initial field advanced by `warmup` steps (the
     # workload is not stationary -- shocklets form and the WENO activation grows -- so regions that start
