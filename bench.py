@@ -347,7 +347,11 @@ def run_ours(args):
     # ---- per-kernel roofline from the event pairs of the timed region
     peak, peak_src = load_peaks()
     sm_mhz = (clk or {}).get("sm_mhz") or 1965.0
-    peak_inst = N_SM * FP64_LANES_PER_SM * sm_mhz * 1e6        # fp64 thread-instructions / s at the clock under load
+    nominal_inst = N_SM * FP64_LANES_PER_SM * sm_mhz * 1e6     # fp64 thread-instructions / s at the clock under load
+    # measured on this device through the C ABI (streams_measure_fp64): DFMA chains and DADD + DMUL chains
+    fp64_meas = {"dfma_ginst_s": binding.measure_fp64(0, 5, gpu.stream), "dadd_dmul_ginst_s": binding.measure_fp64(1, 5, gpu.stream),
+                 "nominal_ginst_s": nominal_inst / 1e9}
+    peak_inst = fp64_meas["dfma_ginst_s"] * 1e9
     B, I, per_point = work_model(case, act)
     kernels = {}
     for name, (kms, cnt) in prof.items():
@@ -368,10 +372,11 @@ def run_ours(args):
     else:   # fp64 pipe: 2 flop per instruction slot (DFMA), so 1 inst/s == 2 flop/s of the nominal peak
         roofline = {"kernel": dom, "bound": "alu", "achieved": 2 * kd["fp64_ginst_s"] / 1e3, "peak": 2 * peak_inst / 1e12,
                     "unit": "TFLOP/s", "frac": kd["frac_fp64"], "traffic": None,
-                    "peak_source": "148 SM x 64 fp64 FMA lanes x 2 x %.0f MHz (clock under load); achieved counts every "
-                                   "fp64 instruction as one FMA slot (DESIGN.md)" % sm_mhz}
+                    "peak_source": "measured DFMA issue rate of this device (streams_measure_fp64) x 2 flop; nominal 148 SM x "
+                                   "64 fp64 lanes x 2 x %.0f MHz = %.1f TFLOP/s; achieved counts every fp64 instruction as one "
+                                   "FMA slot (DESIGN.md)" % (sm_mhz, 2 * nominal_inst / 1e12)}
     roofline.update({"alg_bytes_per_point_rhs_main": per_point, "kernels": kernels, "events_dropped": dropped,
-                     "hbm_peak_gbs": peak, "hbm_peak_source": peak_src})
+                     "hbm_peak_gbs": peak, "hbm_peak_source": peak_src, "fp64_peak": fp64_meas})
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):           # dram bytes per launch from the committed ncu --set full capture
         with open(traffic_file) as f:

@@ -144,6 +144,13 @@ int streams_profile(streams_ctx* ctx, int enable, int max_records);
  * Synchronises the stream. */
 int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long long* dropped);
 
+/* Measures the fp64 pipe of the current device, the "alu" roof of SURVEY 8(d): kind 0 = independent DFMA chains,
+ * kind 1 = DADD and DMUL alternating.  *ginst_per_s (HOST) receives thread-level fp64 instructions per second in
+ * units of 1e9, the best of `repeats` launches timed with CUDA events on `cuda_stream` (each launch runs
+ * 8 x 256-thread blocks per SM, 16 chains per thread).  Needs no context and no workspace; synchronises the stream.
+ * Returns STREAMS_EINVAL for a bad kind / null output, STREAMS_ECUDA on a CUDA error. */
+int streams_measure_fp64(void* cuda_stream, int kind, int repeats, double* ginst_per_s);
+
 /* Name of a kernel class ("" if out of range); static storage. */
 const char* streams_kernel_name(int kind);
 

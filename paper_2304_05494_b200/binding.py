@@ -18,7 +18,7 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREA
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
            "streams_get_fields", "streams_get_sensor", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches",
-           "streams_profile", "streams_get_profile", "streams_kernel_name",
+           "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
            "streams_last_error", "streams_destroy")
 STREAMS_K_COUNT = 8
 
@@ -73,6 +73,7 @@ def load_library(path: str = LIB_PATH):
     lib.streams_kernel_launches.argtypes = [C.c_void_p]
     lib.streams_profile.argtypes = [C.c_void_p, C.c_int, C.c_int]
     lib.streams_get_profile.argtypes = [C.c_void_p, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    lib.streams_measure_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
     lib.streams_kernel_name.restype = C.c_char_p
     lib.streams_kernel_name.argtypes = [C.c_int]
     lib.streams_last_error.restype = C.c_char_p
@@ -100,6 +101,21 @@ def structs_from_case(case):
               "dt_fixed", "dt_every"):
         setattr(s, n, getattr(case, n))
     return g, a, s, keep
+
+
+def measure_fp64(kind: int = 0, repeats: int = 5, stream=None) -> float:
+    """streams_measure_fp64 on the current device: 1e9 thread-level fp64 instructions per second
+    (kind 0: DFMA chains, kind 1: DADD + DMUL)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: libstreams has no CPU fallback")
+    lib = load_library()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    out = C.c_double()
+    rc = lib.streams_measure_fp64(C.c_void_p(st.cuda_stream), int(kind), int(repeats), C.byref(out))
+    if rc != STREAMS_OK:
+        raise StreamsError(rc, lib.streams_last_error(None).decode())
+    return out.value
 
 
 class StreamsError(RuntimeError):

@@ -520,6 +520,14 @@ int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long lon
   return STREAMS_OK;
 }
 
+int streams_measure_fp64(void* cuda_stream, int kind, int repeats, double* ginst_per_s) {
+  if (!ginst_per_s || kind < 0 || kind > 1) return fail(nullptr, STREAMS_EINVAL, "streams_measure_fp64: bad argument");
+  const double v = measure_fp64((cudaStream_t)cuda_stream, kind, repeats < 1 ? 1 : repeats);
+  if (v < 0.0) return fail(nullptr, STREAMS_ECUDA, "streams_measure_fp64: CUDA error");
+  *ginst_per_s = v * 1e-9;
+  return STREAMS_OK;
+}
+
 const char* streams_kernel_name(int kind) {
   static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "weno", "rhs_apply", "misc"};
   return (kind >= 0 && kind < STREAMS_K_COUNT) ? names[kind] : "";

@@ -511,6 +511,56 @@ __global__ void reset_counters_kernel(const DevP P) {
   reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[2] += 1ull;   // sensor evaluations since set_fields
 }
 
+// ---------------------------------------------------------------------------------------------
+// fp64 pipe probe (streams_measure_fp64): 16 independent chains per thread, ITERS trips; KIND 0 chains are
+// x = fma(x, a, b), KIND 1 alternate x = x + b and x = x * a (this unit is built without contraction, so they
+// stay separate instructions).  The result is stored so that nothing is optimised away.
+// ---------------------------------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(256) fp64_probe_kernel(double* out, double a, double b, int iters) {
+  double x[16];
+#pragma unroll
+  for (int c = 0; c < 16; ++c) x[c] = 1.0 + 1e-3 * (threadIdx.x + 16 * c);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      if (KIND == 0) x[c] = fma(x[c], a, b);
+      else { x[c] = x[c] + b; x[c] = x[c] * a; }
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int c = 0; c < 16; ++c) s += x[c];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// Returns thread-level fp64 instructions per second (best of `repeats`), or a negative value on a CUDA error.
+double measure_fp64(cudaStream_t st, int kind, int repeats) {
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return -1.0;
+  const int blocks = nsm * 8, threads = 256, iters = 4096;
+  double* out = nullptr;
+  if (cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)) != cudaSuccess) return -1.0;   // probe only: not a hot path
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = -1.0;
+  for (int r = 0; r < repeats + 1; ++r) {            // the first launch warms up
+    cudaEventRecord(e0, st);
+    if (kind == 0) fp64_probe_kernel<0><<<blocks, threads, 0, st>>>(out, 0.999999, 1e-6, iters);
+    else fp64_probe_kernel<1><<<blocks, threads, 0, st>>>(out, 0.999999, 1e-6, iters);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double inst = (double)blocks * threads * 16.0 * iters * (kind == 0 ? 1.0 : 2.0);
+    if (r > 0 && ms > 0.f) best = fmax(best, inst / (ms * 1e-3));
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  return cudaGetLastError() == cudaSuccess ? best : -1.0;
+}
+
 // -------------------------------------------------------------------------- launch wrappers
 static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }
 

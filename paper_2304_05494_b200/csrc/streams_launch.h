@@ -35,6 +35,7 @@ int launch_step_end(const DevP& P, cudaStream_t st);
 // combination is not instantiated.
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st);
 int launch_rhs_main(const DevP& P, const MarchMaps& maps, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
+double measure_fp64(cudaStream_t st, int kind, int repeats);   // streams_measure_fp64
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law);
 
 }  // namespace streams

@@ -21,7 +21,7 @@ def lib():
 def _declared_symbols():
     txt = open(os.path.join(ROOT, "include", "streams.h")).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(streams_[a-z_]+)\s*\(", txt)))
+    return sorted(set(re.findall(r"\b(streams_[a-z0-9_]+)\s*\(", txt)))
 
 
 def test_library_exports_every_declared_symbol(lib):
