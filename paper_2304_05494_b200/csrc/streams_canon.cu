@@ -247,8 +247,11 @@ __device__ __forceinline__ double ddc_g(const DevP& P, const G& g, double metric
   return acc * metric;
 }
 
+#ifndef STREAMS_SENSOR_MINB
+#define STREAMS_SENSOR_MINB 3
+#endif
 template <bool MASK, bool THETA, int TY>
-__global__ void __launch_bounds__(MTX * TY, 3)
+__global__ void __launch_bounds__(MTX * TY, STREAMS_SENSOR_MINB)
 sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring, const DevP P,
                     int nbx, int nby, int kz) {
   using G = MarchGeom<TY>;
@@ -343,6 +346,8 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     }
     mbar_wait(&full_r[b], par);
     const double* __restrict__ rn = ring + (size_t)b * 3 * G::NT + tid;
+    // (register moves: renaming the ring through a phase switch measured slower, here and in rhs_march_kernel;
+    // so did 4 blocks / SM at 64 registers and 32 x 16 or 32 x 4 tiles)
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
 #pragma unroll
@@ -594,7 +599,7 @@ static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st
 }
 template <bool MASK, bool THETA>
 static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t st) {
-  constexpr int TY = STREAMS_MARCH_TY;
+  constexpr int TY = STREAMS_SENSOR_TY;
   using SM = SensorSmem<TY>;
   auto kern = sensor_march_kernel<MASK, THETA, TY>;
   static bool attr_set = false;
@@ -603,7 +608,7 @@ static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t 
     attr_set = true;
   }
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
-  const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * 3);
+  const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * STREAMS_SENSOR_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
   kern<<<(unsigned)(nbx * nby * chunks), MTX * TY, SM::TOTAL, st>>>(mp.s_centre, mp.s_ring, P, nbx, nby, kz);
   const long long ghosts = 2LL * P.ng * ((long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny);

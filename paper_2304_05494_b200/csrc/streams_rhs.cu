@@ -800,8 +800,9 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
   if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->w, P.w, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
   if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
-  if (make(&maps->s_centre, P.q, nf, MarchGeom<TY>::ROW, MarchGeom<TY>::ROWS, 3) != CUDA_SUCCESS) return -2;
-  if (make(&maps->s_ring, P.q, nf, MTX, TY, 3) != CUDA_SUCCESS) return -2;
+  constexpr int STY = STREAMS_SENSOR_TY;
+  if (make(&maps->s_centre, P.q, nf, MarchGeom<STY>::ROW, MarchGeom<STY>::ROWS, 3) != CUDA_SUCCESS) return -2;
+  if (make(&maps->s_ring, P.q, nf, MTX, STY, 3) != CUDA_SUCCESS) return -2;
   return 0;
 }
 

@@ -8,6 +8,10 @@
 #define STREAMS_MARCH_TY 8
 #endif
 
+#ifndef STREAMS_SENSOR_TY
+#define STREAMS_SENSOR_TY 8
+#endif
+
 namespace streams {
 
 // ------------------------------------------------------------------ async-copy / mbarrier / TMA primitives
