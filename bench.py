@@ -3,9 +3,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A "step" is one full low-storage RK3 step of the whole hot path over the whole grid: 3 x (ghost fill +
-primitives, sensor/mask, interface flags, fused convective x/y/z + viscous RHS + RK update) and the dt
-reduction.  value = grid points x K / device time of streams_step(K)
+A "step" is one full low-storage RK3 step of the whole hot path over the whole grid: 3 x (ghost fill, sensor/mask,
+interface flags, WENO fluxes of the flagged interfaces, fused convective x/y/z + viscous RHS + RK update + primitives
+of the updated state) and the dt reduction.  value = grid points x K / device time of streams_step(K)
 (= 1e8 / the paper's "grind time").  The workload is BASELINE.json configs[1] (128^3 decaying
 compressible isotropic turbulence, hybrid WENO, Sutherland viscosity) unless --config says otherwise.
 N > 1: the path is single-GPU by design (north_star); ranks run independent replicas with different
@@ -135,7 +135,8 @@ class ClockSampler:
 # (profiles/r1c_fp64_counts.md; static SASS counts overstate kernels with branches: the IEEE-divide slow paths and
 # the wall branch of fill_prim are rarely taken)
 FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 30,
-             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 115}
+             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 115,
+             "prims": 60}      # prims: cons -> prim of the updated node in the fused RHS epilogue (shared reciprocal, no IEEE divide)
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
 
 
@@ -155,8 +156,10 @@ def work_model(case, act):
     n_if = act["iface"] * N if hyb else (3 * N if weno else 0)
     n_sh = act["shock"] * N if hyb else (N if weno else 0)
     B, I = {}, {}
-    B["fill_prim"] = Np * (40 + 8 * nprim) + (Np - N) * 40     # read w, write primitives, write ghost w
-    I["fill_prim"] = Np * FP64_INST["fill_prim"] + N * FP64_INST["fill_prim_dt"] / 3.0   # dt rate: first stage only
+    # ghost shell only: the fused RHS kernel writes the primitives of the updated interior nodes (the one full pass
+    # after streams_set_fields, 1 launch in 3 K, is not modelled): read the image, write the ghost w and primitives
+    B["fill_prim"] = (Np - N) * (40 + 40 + 8 * nprim)
+    I["fill_prim"] = (Np - N) * FP64_INST["fill_prim"]
     B["sensor"] = N * (24 + 8 + (1 if hyb else 0))             # read u v w, write div [mask]
     I["sensor"] = N * FP64_INST["sensor"]
     B["flags"] = N * (1 + 1) + n_if * 4                        # read mask, write flags byte, append to the work lists
@@ -164,10 +167,11 @@ def work_model(case, act):
     # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
     # read R_prev (stages 2, 3), write R (stages 1, 2)
     # (+ hybrid / WENO: the flag byte of every node and the 5 flux corrections of every flagged interface)
-    per_point = (48 if conv else 0) + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40
+    # + the primitives of the updated node (a2 of the next stage), written to the other q buffer
+    per_point = (48 if conv else 0) + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40 + 8 * nprim
     B["rhs_main"] = N * per_point + (N * 1 if hyb else 0) + n_if * 40
     I["rhs_main"] = (N * FP64_INST["rhs_main_" + (("c" if conv else "") + ("v" if visc else "") or "0")]
-                     + n_sh * FP64_INST["rhs_corr"])
+                     + n_sh * FP64_INST["rhs_corr"] + N * (FP64_INST["prims"] + FP64_INST["fill_prim_dt"] / 3.0))
     # WENO: per flagged interface one new stencil node of 7 fields (runs of flagged interfaces share the
     # rest), a list entry, 5 flux values out
     B["weno"] = n_if * (56 + 4 + 40)                           # per timed group: the x, y and z launches of a stage

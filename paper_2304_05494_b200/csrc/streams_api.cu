@@ -23,7 +23,7 @@ struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
   size_t N, lcap;
-  size_t off_w, off_q, off_div, off_theta, off_mask, off_nflag, off_ilist, off_dF, off_counters, off_R,
+  size_t off_w, off_q, off_q2, off_theta, off_mask, off_nflag, off_ilist, off_dF, off_counters, off_R,
       off_metrics, off_scal, total;
   int nq;
 };
@@ -87,8 +87,8 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   S.off_w = take(5 * S.fs * 8);
-  S.off_q = take((size_t)S.nq * S.fs * 8);
-  S.off_div = S.off_q + (size_t)Q_DIV * S.fs * 8;
+  S.off_q = take((size_t)S.nq * S.fs * 8);       // two primitive buffers: a stage reads one while the fused RHS kernel
+  S.off_q2 = take((size_t)S.nq * S.fs * 8);      // writes the primitives of the updated state into the other
   S.off_theta = take(S.N * 8);
   S.off_mask = take(S.fs);
   S.off_nflag = take(hyb ? S.fs : 256);
@@ -113,8 +113,12 @@ struct streams_ctx {
   streams_gas gas;
   streams_scheme scheme;
   Sizes S;
-  DevP P;
-  MarchMaps maps;
+  DevP P;                   // P.q / P.div point at the CURRENT primitive buffer (qbuf[cur])
+  MarchMaps maps[2];        // TMA views of each primitive buffer
+  double* qbuf[2];
+  int cur;                  // index of the buffer that holds (or will receive) the primitives of the current state
+  bool prims_interior;      // qbuf[cur] already holds the primitives of every interior node (written by the last stage)
+  bool rate_ready;          // scal[S_RATE] already holds the rate of the current state (reduced by the last stage)
   cudaStream_t stream;
   char* base;
   bool have_fields;
@@ -223,19 +227,34 @@ cudaError_t prof_drain(streams_ctx* ctx) {
   return cudaSuccess;
 }
 
-// ghost fill + primitives (+ dt) + sensor + flags: everything a stage needs before the RHS kernels
+// ghost fill + primitives (+ dt) + sensor + flags: everything a stage needs before the RHS kernels.
+// After an updating stage the fused RHS kernel has already written the primitives of every interior node of the
+// new state (and, on request, reduced its time-step rate): only the ghost shell is left.  Otherwise (first
+// evaluation after streams_set_fields, or a dt wanted that no stage prepared) the full pass runs.
 int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
-  const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0);
-  timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
-  if (want_dt) timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, st); });
+  const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0) && !ctx->rate_ready;
+  if (ctx->prims_interior && !reduce_dt) timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
+  else timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
+  ctx->prims_interior = true;
+  if (want_dt) {
+    timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, st); });
+    ctx->rate_ready = false;                        // dt_finalize consumed (and zeroed) the rate
+  }
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
   if (hyb || visc || theta)
-    timed(ctx, STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps, ctx->S.L, hyb || theta, theta, st); });
+    timed(ctx, STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps[ctx->cur], ctx->S.L, hyb || theta, theta, st); });
   if (hyb) timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.r, st); });
   return STREAMS_OK;
+}
+
+// points DevP::q / div at primitive buffer b
+void use_qbuf(streams_ctx* ctx, int b) {
+  ctx->cur = b;
+  ctx->P.q = ctx->qbuf[b];
+  ctx->P.div = ctx->qbuf[b] + (size_t)Q_DIV * ctx->S.fs;
 }
 
 // the RHS (+ update) of one stage: the WENO flux corrections of the flagged interfaces first (they read the
@@ -246,7 +265,7 @@ int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   int b = 0;
   if (ctx->scheme.flux_mode != STREAMS_FLUX_CENTRAL)
     b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
-  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps, ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
+  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps[ctx->cur], ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
   return (a < 0 || b < 0) ? -1 : a + b;
 }
 
@@ -288,8 +307,9 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.px = S.px; P.py = S.py; P.pz = S.pz;
   P.sy = S.px; P.sz = (long long)S.px * S.py; P.fs = (long long)S.fs; P.N = (long long)S.N;
   P.w = (double*)(ctx->base + S.off_w);
-  P.q = (double*)(ctx->base + S.off_q);
-  P.div = (double*)(ctx->base + S.off_div);
+  ctx->qbuf[0] = (double*)(ctx->base + S.off_q);
+  ctx->qbuf[1] = (double*)(ctx->base + S.off_q2);
+  ctx->prims_interior = false; ctx->rate_ready = false;
   P.theta = (double*)(ctx->base + S.off_theta);
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
   P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
@@ -314,6 +334,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.sb2xz = -2.0 * P.sbv * (P.inv_dx * P.inv_dx + P.inv_dz * P.inv_dz);
   P.gamma = gas->gamma; P.gm1 = gas->gamma - 1.0; P.rgas = gas->rgas; P.prandtl = gas->prandtl;
   P.kfac = (gas->gamma * gas->rgas / (gas->gamma - 1.0)) / gas->prandtl;
+  P.inv_rgas = 1.0 / gas->rgas; P.inv_tref = gas->t_ref > 0.0 ? 1.0 / gas->t_ref : 0.0;
   P.mu_ref = gas->mu_ref; P.t_ref = gas->t_ref; P.suth_s = gas->suth_s_over_tref; P.pow_exp = gas->pow_exp;
   const double rr = gas->u_ref / gas->l_ref;
   P.eps_s = rr * rr;
@@ -331,7 +352,14 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
     }
     P.nsm = nsm;
   }
-  if (make_march_maps(P, &ctx->maps) != 0) {
+  int maps_rc = 0;
+  for (int b = 1; b >= 0; --b) {                    // ends on buffer 0, the first current one
+    P.q = ctx->qbuf[b];
+    P.div = P.q + (size_t)Q_DIV * S.fs;
+    ctx->cur = b;
+    if (make_march_maps(P, &ctx->maps[b]) != 0) maps_rc = -1;
+  }
+  if (maps_rc != 0) {
     delete ctx;
     return fail(nullptr, STREAMS_ECUDA, "cannot build the TMA descriptors (cuTensorMapEncodeTiled)");
   }
@@ -371,6 +399,8 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
   if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));   // the host buffer may be reused on return
   ctx->have_fields = true;
   ctx->step_count = 0;
+  ctx->prims_interior = false;                       // the next evaluation runs the full ghost + primitive pass
+  ctx->rate_ready = false;
   return STREAMS_OK;
 }
 
@@ -399,7 +429,7 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   enqueue_prepare(ctx, false, false);
   StageArgs sa;
   sa.gam = 0.0; sa.rhk = 0.0; sa.update_w = 0; sa.read_prev = 0; sa.write_r = 1;
-  sa.r_dense = rhs_out_dev;
+  sa.r_dense = rhs_out_dev; sa.q_out = nullptr; sa.want_rate = 0;
   if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
   CU(cudaGetLastError());
   return STREAMS_OK;
@@ -419,7 +449,13 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
       StageArgs sa;
       sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
       sa.r_dense = nullptr;
+      sa.q_out = ctx->qbuf[ctx->cur ^ 1];
+      // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
+      sa.want_rate = (l == 2 && !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0) ? 1 : 0;
       if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
+      use_qbuf(ctx, ctx->cur ^ 1);                   // the updated state's primitives are in the other buffer
+      ctx->prims_interior = true;
+      if (sa.want_rate) ctx->rate_ready = true;
     }
     timed(ctx, STREAMS_K_MISC, [&] { return launch_step_end(ctx->P, ctx->stream); });
     ctx->step_count += 1;

@@ -16,22 +16,10 @@ namespace streams {
 // T -> 2 T_w - T, p -> p, rho = p/(R T); O6) and then the primitives.
 // HBM: 40 B read (interior) + 8 B x (#primitive fields) write per padded node.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double viscosity(const DevP& P, double T) {
-  const double t = T / P.t_ref;
-  if (P.visc_law == VISC_SUTHERLAND) return ((P.mu_ref * (t * sqrt(t))) * (1.0 + P.suth_s)) / (t + P.suth_s);
-  return P.mu_ref * pow(t, P.pow_exp);
-}
-
-// With DT the same pass takes the time-step rate of every interior node (a9, O5 / S13): max over
-// directions of (|u_d| + c) m_d, nu m_d^2, gamma nu m_d^2 / Pr, reduced by warp shuffles on the bit patterns
-// (rates are non-negative, so unsigned order = numeric order, and a NaN wins and is detected) and one
-// atomicMax per block.
+// With DT the same pass takes the time-step rate of every interior node (a9) and reduces it (block_rate_max).
+// fill_node: one padded node (i, j, k in interior coordinates, ghosts negative or beyond the extents).
 template <bool VISC, bool STORE_C, bool DT>
-__global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
-  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-  const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
-  double rmax = 0.0;
-  if (i >= -P.ng && i < P.nx + P.ng) {
+__device__ __forceinline__ double fill_node(const DevP& P, int i, int j, int k) {
   int is = i, js = j, ks = k;
   bool fsx = false, fsy = false, fsz = false;
   double t_wall = 0.0;
@@ -87,58 +75,56 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
 #pragma unroll
     for (int q = 0; q < 5; ++q) P.w[q * P.fs + n] = s[q];
   }
-  const double rho = s[0];
-  const double uu = s[1] / rho, vv = s[2] / rho, wv = s[3] / rho;
-  const double ke = 0.5 * ((uu * uu + vv * vv) + wv * wv);
-  const double pp = P.gm1 * (s[4] - rho * ke);
-  P.q[Q_U * P.fs + n] = uu;
-  P.q[Q_V * P.fs + n] = vv;
-  P.q[Q_W * P.fs + n] = wv;
-  P.q[Q_H * P.fs + n] = (s[4] + pp) / rho;
-  P.q[Q_P * P.fs + n] = pp;
-  P.q[Q_RHO * P.fs + n] = rho;
-  double mu = 0.0;
-  if (VISC) {
-    const double TT = pp / (rho * P.rgas);
-    mu = viscosity(P, TT);
-    P.q[Q_T * P.fs + n] = TT;
-    P.q[Q_MU * P.fs + n] = mu;
-  }
-  double cc = 0.0;
-  if (STORE_C || DT) cc = sqrt(P.gamma * pp / rho);
-  if (STORE_C) P.q[Q_C * P.fs + n] = cc;
-  if (DT && !ghost) {
-    const double md[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
-    const double vel[3] = {uu, vv, wv};
-    double nu = 0.0;
-    if (VISC) nu = mu / rho;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      rmax = fmax(rmax, (fabs(vel[d]) + cc) * md[d]);
-      if (VISC) {
-        rmax = fmax(rmax, nu * (md[d] * md[d]));
-        rmax = fmax(rmax, (P.gamma * nu / P.prandtl) * (md[d] * md[d]));
-      }
-    }
-    if (!(rmax == rmax) || !(cc == cc)) rmax = __longlong_as_double(0x7ff8000000000000LL);
-  }
-  }
+  double mu, cc, vel[3];
+  prims_from_state<VISC, STORE_C>(P, s, P.q + n, DT, mu, cc, vel);
+  double rmax = 0.0;
+  if (DT && !ghost) rmax = dt_rate<VISC>(P, vel, cc, mu, s[0], P.eta_y_c[j]);
+  return rmax;
+}
+
+template <bool VISC, bool STORE_C, bool DT>
+__global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
+  double rmax = 0.0;
+  if (i >= -P.ng && i < P.nx + P.ng) rmax = fill_node<VISC, STORE_C, DT>(P, i, j, k);
   if (DT) {
-    unsigned long long bits = (unsigned long long)__double_as_longlong(rmax);
-#pragma unroll
-    for (int s = 16; s > 0; s >>= 1) {
-      const unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, s);
-      bits = o > bits ? o : bits;
-    }
     __shared__ unsigned long long sm[4];
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = bits;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-#pragma unroll
-      for (int wq = 1; wq < 4; ++wq) bits = sm[wq] > bits ? sm[wq] : bits;
-      if (bits) atomicMax(reinterpret_cast<unsigned long long*>(P.scal + S_RATE), bits);
-    }
+    block_rate_max(P, rmax, sm);
   }
+}
+
+// The ghost shell only (every stage but the first after streams_set_fields: the fused RHS kernel has already
+// written the primitives of the updated interior nodes).  Three segments of a flat index: the z slabs (whole padded
+// planes), the y slabs of the interior planes, the x columns of the interior rows.
+template <bool VISC, bool STORE_C>
+__global__ void __launch_bounds__(128) fill_ghost_kernel(const DevP P) {
+  const int g = P.ng, wx = P.nx + 2 * g;
+  const long long nZ = 2LL * g * P.py * wx, nY = (long long)P.nz * 2 * g * wx, nX = (long long)P.nz * P.ny * 2 * g;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (t < nZ) {
+    i = (int)(t % wx) - g;
+    const long long t2 = t / wx;
+    j = (int)(t2 % P.py) - g;
+    const int m = (int)(t2 / P.py);
+    k = m < g ? m - g : P.nz + (m - g);
+  } else if ((t -= nZ) < nY) {
+    i = (int)(t % wx) - g;
+    const long long t2 = t / wx;
+    const int m = (int)(t2 % (2 * g));
+    k = (int)(t2 / (2 * g));
+    j = m < g ? m - g : P.ny + (m - g);
+  } else if ((t -= nY) < nX) {
+    const int m = (int)(t % (2 * g));
+    const long long t2 = t / (2 * g);
+    j = (int)(t2 % P.ny);
+    k = (int)(t2 / P.ny);
+    i = m < g ? m - g : P.nx + (m - g);
+  } else {
+    return;
+  }
+  fill_node<VISC, STORE_C, false>(P, i, j, k);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -582,6 +568,19 @@ int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st) {
   else if (sc) STREAMS_FILL(false, true);
   else STREAMS_FILL(false, false);
 #undef STREAMS_FILL
+  return 1;
+}
+
+int launch_fill_ghosts(const DevP& P, cudaStream_t st) {
+  const int g = P.ng;
+  const long long wx = P.nx + 2 * g;
+  const long long total = 2LL * g * P.py * wx + (long long)P.nz * 2 * g * wx + (long long)P.nz * P.ny * 2 * g;
+  dim3 b(128), gr((unsigned)((total + 127) / 128));
+  const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
+  if (visc && sc) fill_ghost_kernel<true, true><<<gr, b, 0, st>>>(P);
+  else if (visc) fill_ghost_kernel<true, false><<<gr, b, 0, st>>>(P);
+  else if (sc) fill_ghost_kernel<false, true><<<gr, b, 0, st>>>(P);
+  else fill_ghost_kernel<false, false><<<gr, b, 0, st>>>(P);
   return 1;
 }
 

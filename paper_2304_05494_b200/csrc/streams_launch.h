@@ -14,6 +14,8 @@ struct StageArgs {
   int read_prev;        // stage uses the previous-stage RHS
   int write_r;          // keep R (padded layout, DevP::R) for the next stage
   double* r_dense;      // if not null: also write R here, interior [5][N] (streams_rhs output)
+  double* q_out;        // update_w: the primitives of the updated state go here (the other DevP::q buffer)
+  int want_rate;        // update_w: also reduce the time-step rate of the updated state into scal[S_RATE]
 };
 
 
@@ -21,11 +23,12 @@ struct StageArgs {
 
 // TMA descriptors of the fused RHS kernel (built once per context by make_march_maps):
 // centre planes with halo and ring planes of the primitives, RK operands w and R.
-struct MarchMaps { CUtensorMap centre, ring, w, r, s_centre, s_ring; };   // s_*: (u, v, w) boxes of the sensor kernel
+struct MarchMaps { CUtensorMap centre, ring, w, r, s_centre, s_ring; };   // centre / ring / s_*: views of ONE q buffer   // s_*: (u, v, w) boxes of the sensor kernel
 // Returns 0, or a negative code: -1 driver entry point missing, -2 encode failed.
 int make_march_maps(const DevP& P, MarchMaps* maps);
 
 int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st);   // with_dt: also reduce the time-step rate (a9)
+int launch_fill_ghosts(const DevP& P, cudaStream_t st);                // ghost shell only (interior primitives already current)
 int launch_sensor(const DevP& P, const MarchMaps& maps, int L, bool mask, bool theta, cudaStream_t st);
 int launch_flags(const DevP& P, int r, cudaStream_t st);
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);

@@ -175,7 +175,7 @@ struct MarchSmem {
   static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[5]
   static constexpr size_t DFS = WENO ? (size_t)30 * G::NT * 8 : 0;
   static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + 2 * RING, OFF_DFS = OFF_EPI + 2 * EPI,
-                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 64;
+                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 32 + 8 * 32;   // 4 mbarriers, rate scratch
   static_assert(BUF % 128 == 0 && RING % 128 == 0 && EPI % 128 == 0, "TMA destinations are 128-byte aligned");
 };
 
@@ -280,6 +280,8 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
 #pragma unroll
     for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
   }
+  double rate = 0.0;                                  // a9 of the next step (last stage only)
+  bool rate_nan = false;
   unsigned fl_next = 0;
   if (WENO && CONV && active) fl_next = ld_u8_now(P.nflag + ncol + (long long)kb * P.sz);
 
@@ -373,12 +375,20 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     }
     if (active) {
       if (sa.update_w) {
+        double wn[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           double inc = sa.gam * r[q];
           if (sa.read_prev) inc = fma(sa.rhk, ep[q * G::NT], inc);
-          P.w[(long long)q * P.fs + n] = fma(dt, inc, ep[(5 + q) * G::NT]);
+          wn[q] = fma(dt, inc, ep[(5 + q) * G::NT]);
+          P.w[(long long)q * P.fs + n] = wn[q];
         }
+        // a2 of the next stage: the primitives of the updated node go to the other q buffer (stencils of this
+        // stage still read the current one); the next stage only fills the ghost shell
+        double mu, cc, vel[3];
+        prims_from_state<VISC, WENO>(P, wn, sa.q_out + n, sa.want_rate != 0, mu, cc, vel);
+        if (sa.want_rate) rate = fmax(rate, dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc));
+        if (sa.want_rate && !(rate == rate)) rate_nan = true;   // fmax would drop a NaN on the next plane
       }
       if (sa.write_r) {
 #pragma unroll
@@ -400,6 +410,11 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       zr[f][2 * NG] = rn[f * G::NT];
     }
   }
+  // a9 of the next step: one atomicMax per block on the bit pattern of the largest rate (a NaN wins)
+  if (sa.want_rate) {
+    if (rate_nan) rate = __longlong_as_double(0x7ff8000000000000LL);
+    block_rate_max(P, rate, bars + 4);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -407,17 +422,6 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
 // value at the interface between v[R-1] and v[R].
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double sq(double x) { return x * x; }
-
-// 1/x for positive, normal x (sums of smoothness weights, sound speeds, 1 + sqrt(density ratio)): hardware
-// seed + two Newton steps, ~1 ulp, no special-case branches (an IEEE divide is ~3x the instructions).
-__device__ __forceinline__ double rcp_pos(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
-}
 
 template <int R>
 __device__ __forceinline__ double weno_rec(const double* v, double eps);
