@@ -343,6 +343,9 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.t_wall_lo = grid->t_wall_lo; P.t_wall_hi = grid->t_wall_hi;
   P.bc_x = grid->bc_x; P.bc_y_lo = grid->bc_y_lo; P.bc_y_hi = grid->bc_y_hi; P.bc_z = grid->bc_z;
   P.visc_law = gas->visc_law; P.flux_mode = scheme->flux_mode;
+  P.own_x = grid->bc_x == STREAMS_BC_PERIODIC && grid->nx >= 2 * S.ng;
+  P.own_y = grid->bc_y_lo == STREAMS_BC_PERIODIC && grid->ny >= 2 * S.ng;
+  P.own_z = grid->bc_z == STREAMS_BC_PERIODIC && grid->nz >= 2 * S.ng;
   {
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||

@@ -75,8 +75,9 @@ __device__ __forceinline__ double fill_node(const DevP& P, int i, int j, int k) 
 #pragma unroll
     for (int q = 0; q < 5; ++q) P.w[q * P.fs + n] = s[q];
   }
-  double mu, cc, vel[3];
-  prims_from_state<VISC, STORE_C>(P, s, P.q + n, DT, mu, cc, vel);
+  double mu, cc, vel[3], o[NQ];
+  prims_from_state<VISC, STORE_C>(P, s, DT, o, mu, cc, vel);
+  store_prims<VISC, STORE_C>(P, P.q + n, o);
   double rmax = 0.0;
   if (DT && !ghost) rmax = dt_rate<VISC>(P, vel, cc, mu, s[0], P.eta_y_c[j]);
   return rmax;
@@ -95,12 +96,14 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
 }
 
 // The ghost shell only (every stage but the first after streams_set_fields: the fused RHS kernel has already
-// written the primitives of the updated interior nodes).  Three segments of a flat index: the z slabs (whole padded
+// written the primitives of the updated interior nodes and of their periodic images, DevP::own_*).  Up to three
+// segments of a flat index (directions the RHS kernel owns are skipped): the z slabs (whole padded
 // planes), the y slabs of the interior planes, the x columns of the interior rows.
 template <bool VISC, bool STORE_C>
 __global__ void __launch_bounds__(128) fill_ghost_kernel(const DevP P) {
   const int g = P.ng, wx = P.nx + 2 * g;
-  const long long nZ = 2LL * g * P.py * wx, nY = (long long)P.nz * 2 * g * wx, nX = (long long)P.nz * P.ny * 2 * g;
+  const long long nZ = P.own_z ? 0 : 2LL * g * P.py * wx, nY = P.own_y ? 0 : (long long)P.nz * 2 * g * wx,
+                  nX = P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int i, j, k;
   if (t < nZ) {
@@ -574,7 +577,9 @@ int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st) {
 int launch_fill_ghosts(const DevP& P, cudaStream_t st) {
   const int g = P.ng;
   const long long wx = P.nx + 2 * g;
-  const long long total = 2LL * g * P.py * wx + (long long)P.nz * 2 * g * wx + (long long)P.nz * P.ny * 2 * g;
+  const long long total = (P.own_z ? 0 : 2LL * g * P.py * wx) + (P.own_y ? 0 : (long long)P.nz * 2 * g * wx) +
+                          (P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g);
+  if (total == 0) return 0;
   dim3 b(128), gr((unsigned)((total + 127) / 128));
   const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
   if (visc && sc) fill_ghost_kernel<true, true><<<gr, b, 0, st>>>(P);

@@ -280,6 +280,9 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
 #pragma unroll
     for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
   }
+  // offsets (doubles) of this node's periodic images in the ghost layers, 0 = none (DevP::own_*)
+  const int xoff = !P.own_x ? 0 : (i < NG ? P.nx : (i >= P.nx - NG ? -P.nx : 0));
+  const int yoff = !P.own_y ? 0 : (j < NG ? P.ny * (int)P.sy : (j >= P.ny - NG ? -P.ny * (int)P.sy : 0));
   double rate = 0.0;                                  // a9 of the next step (last stage only)
   bool rate_nan = false;
   unsigned fl_next = 0;
@@ -385,8 +388,15 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
         }
         // a2 of the next stage: the primitives of the updated node go to the other q buffer (stencils of this
         // stage still read the current one); the next stage only fills the ghost shell
-        double mu, cc, vel[3];
-        prims_from_state<VISC, WENO>(P, wn, sa.q_out + n, sa.want_rate != 0, mu, cc, vel);
+        double mu, cc, vel[3], o[NQ];
+        prims_from_state<VISC, WENO>(P, wn, sa.want_rate != 0, o, mu, cc, vel);
+        double* __restrict__ qo = sa.q_out + n;
+        store_prims<VISC, WENO>(P, qo, o);
+        // a1 of the next stage for the periodic directions: the owner also writes its images in the ghost layers
+        const int zoff = !P.own_z ? 0 : (k < NG ? P.nz * isz : (k >= P.nz - NG ? -P.nz * isz : 0));
+        if (xoff) store_prims<VISC, WENO>(P, qo + xoff, o);
+        if (yoff) store_prims<VISC, WENO>(P, qo + yoff, o);
+        if (zoff) store_prims<VISC, WENO>(P, qo + zoff, o);
         if (sa.want_rate) rate = fmax(rate, dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc));
         if (sa.want_rate && !(rate == rate)) rate_nan = true;   // fmax would drop a NaN on the next plane
       }
