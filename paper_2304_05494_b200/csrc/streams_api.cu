@@ -346,6 +346,8 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.own_x = grid->bc_x == STREAMS_BC_PERIODIC && grid->nx >= 2 * S.ng;
   P.own_y = grid->bc_y_lo == STREAMS_BC_PERIODIC && grid->ny >= 2 * S.ng;
   P.own_z = grid->bc_z == STREAMS_BC_PERIODIC && grid->nz >= 2 * S.ng;
+  P.sown = (P.own_x || grid->bc_x != STREAMS_BC_PERIODIC) && (P.own_y || grid->bc_y_lo != STREAMS_BC_PERIODIC) &&
+           (P.own_z || grid->bc_z != STREAMS_BC_PERIODIC);
   {
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||

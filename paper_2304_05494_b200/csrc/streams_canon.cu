@@ -324,13 +324,37 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     if (active) {
       const long long n = ncol + (long long)k * isz;
       P.div[n] = dv;
+      unsigned char mk = 0;
       if (MASK || THETA) {
         const double ox = gy[2] - gz[1], oy = gz[0] - gx[2], oz = gx[1] - gy[0];
         const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
         double th = -dv / sqrt(s);
         if (!(th > 0.0)) th = 0.0;
         if (THETA) P.theta[iidx(P, i, j, k)] = th;
-        if (MASK) P.mask[n] = (th > P.thr) ? 1 : 0;
+        mk = (th > P.thr) ? 1 : 0;
+        if (MASK) P.mask[n] = mk;
+      }
+      // face ghosts of div / mask (S6), written by the node they copy: its periodic image, or the NG ghost nodes
+      // beyond a non-periodic face (constant extrapolation)
+      if (P.sown) {
+        auto put = [&](long long m) { P.div[m] = dv; if (MASK) P.mask[m] = mk; };
+        auto face = [&](int a, int na, bool per, long long st) {      // a: index along the direction, st: its stride
+          if (per) {
+            if (a < NG) put(n + na * st);
+            else if (a >= na - NG) put(n - na * st);
+          } else {
+            if (a == 0) { for (int m = 1; m <= NG; ++m) put(n - m * st); }
+            if (a == na - 1) { for (int m = 1; m <= NG; ++m) put(n + m * st); }
+          }
+        };
+        face(i, P.nx, P.bc_x == BC_PERIODIC, 1);
+        if (j < NG || j >= P.ny - NG) {
+          if (j < NG && P.bc_y_lo == BC_PERIODIC) put(n + P.ny * P.sy);
+          if (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) put(n - P.ny * P.sy);
+          if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(n - m * P.sy); }
+          if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(n + m * P.sy); }
+        }
+        face(k, P.nz, P.bc_z == BC_PERIODIC, P.sz);
       }
     }
     mbar_wait(&full_r[b], par);
@@ -615,6 +639,7 @@ static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t 
   const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * STREAMS_SENSOR_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
   kern<<<(unsigned)(nbx * nby * chunks), MTX * TY, SM::TOTAL, st>>>(mp.s_centre, mp.s_ring, P, nbx, nby, kz);
+  if (P.sown) return 1;                              // the kernel wrote the face ghosts itself
   const long long ghosts = 2LL * P.ng * ((long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny);
   dim3 gg((unsigned)((ghosts + 255) / 256));
   if (MASK) scalar_ghost_kernel<true><<<gg, 256, 0, st>>>(P);
