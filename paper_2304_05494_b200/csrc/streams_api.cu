@@ -246,7 +246,7 @@ int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
   if (hyb || visc || theta)
     timed(ctx, STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps[ctx->cur], ctx->S.L, hyb || theta, theta, st); });
-  if (hyb) timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.r, st); });
+  if (hyb) timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.L, ctx->S.r, st); });
   return STREAMS_OK;
 }
 

@@ -277,6 +277,13 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     mbar_expect_tx(&full_r[b], (unsigned)SM::RING);
     tma_load_4d(ring + (size_t)b * 3 * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + 1 + P.ng, 0);
   };
+  if (MASK && tid == 0 && blockIdx.x == 0 && P.flux_mode == FLUX_HYBRID) {
+    // per-evaluation counters of flags_kernel (which runs after this kernel; their last readers ran before it)
+    P.counters[C_NSHOCK] = 0;
+    P.counters[C_NFLAGGED] = 0;
+    P.counters[C_NIFACE] = 0; P.counters[C_NIFACE + 1] = 0; P.counters[C_NIFACE + 2] = 0;
+    reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[2] += 1ull;   // sensor evaluations since set_fields
+  }
   if (tid == 0) {
     mbar_init(&full_c[0], 1); mbar_init(&full_c[1], 1);
     mbar_init(&full_r[0], 1); mbar_init(&full_r[1], 1);
@@ -454,7 +461,8 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   __shared__ int s_wsum[3][8], s_base[3];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
-  __syncthreads();
+  // most blocks see no flagged node at all: nothing to count or to append (the barrier also publishes s_cnt)
+  if (!__syncthreads_or(cnt[0] | cnt[1])) return;
 #pragma unroll
   for (int c = 0; c < 2; ++c) {
     int v = cnt[c];
@@ -661,18 +669,19 @@ int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool the
   }
 }
 
-int launch_flags(const DevP& P, int r, cudaStream_t st) {
+int launch_flags(const DevP& P, int L, int r, cudaStream_t st) {
   const int nwx = (P.nx + 7) / 8;
   const long long nwords = (long long)nwx * P.ny * P.nz;
   dim3 b(256), g((unsigned)((nwords + 255) / 256));
-  reset_counters_kernel<<<1, 1, 0, st>>>(P);
+  const bool reset_here = !(L == 3 && P.ng == 3);     // sensor_march_kernel resets the counters itself
+  if (reset_here) reset_counters_kernel<<<1, 1, 0, st>>>(P);
   switch (r) {
     case 1: flags_kernel<1><<<g, b, 0, st>>>(P, nwx); break;
     case 2: flags_kernel<2><<<g, b, 0, st>>>(P, nwx); break;
     case 3: flags_kernel<3><<<g, b, 0, st>>>(P, nwx); break;
     default: flags_kernel<4><<<g, b, 0, st>>>(P, nwx); break;
   }
-  return 2;
+  return reset_here ? 2 : 1;
 }
 
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st) {

@@ -30,7 +30,7 @@ int make_march_maps(const DevP& P, MarchMaps* maps);
 int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st);   // with_dt: also reduce the time-step rate (a9)
 int launch_fill_ghosts(const DevP& P, cudaStream_t st);                // ghost shell only (interior primitives already current)
 int launch_sensor(const DevP& P, const MarchMaps& maps, int L, bool mask, bool theta, cudaStream_t st);
-int launch_flags(const DevP& P, int r, cudaStream_t st);
+int launch_flags(const DevP& P, int L, int r, cudaStream_t st);
 int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);
 int launch_step_end(const DevP& P, cudaStream_t st);
 // The per-interface WENO flux corrections (run first) and the fused RHS + update over all nodes; each
