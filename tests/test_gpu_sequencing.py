@@ -1,0 +1,112 @@
+"""Call sequences through the C ABI against the oracle: the library keeps two primitive buffers (the fused RHS
+epilogue writes the primitives of the updated state into the other one), a "rate ready" state for the time step and
+owner-written periodic ghosts, so every order of calls a user can make must still give the oracle's numbers."""
+import numpy as np
+import pytest
+
+import workloads as W
+from tests.helpers import field_err, natural_scales
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS = 1e-11
+TOL_STEP = 1e-9
+
+
+@pytest.fixture(scope="module")
+def S():
+    from paper_2304_05494_b200 import build, binding
+    build.build()
+    return binding.Streams
+
+
+def _oracle(case):
+    from oracle.oracle import Oracle
+    return Oracle(case)
+
+
+def _cmp_fields(gpu, ora, case, tol=TOL_STEP):
+    floor_w, _ = natural_scales(case)
+    w_g, w_o = gpu.get_fields(), ora.get_fields()
+    errs = [field_err(w_g[q], w_o[q], floor_w[q]) for q in range(5)]
+    assert max(errs) <= tol, errs
+
+
+def _cmp_rhs(gpu, ora, case):
+    _, floor_r = natural_scales(case)
+    r_g, r_o = gpu.rhs().cpu().numpy(), ora.rhs()
+    errs = [field_err(r_g[q], r_o[q], floor_r[q]) for q in range(5)]
+    assert max(errs) <= TOL_RHS, errs
+
+
+def test_dt_every_three(S):
+    """dt recomputed every third step: the last stage of steps 2, 5, ... reduces the rate of the state it produces."""
+    case = W.isotropic_turbulence(nx=40, ny=36, nz=33, mach_t=0.5, k0=3.0, kmax=8, seed=21, dilatational=0.4).replace(dt_every=3)
+    gpu, ora = S(case), _oracle(case)
+    for n in (1, 1, 2, 3, 1):
+        dt_g, t_g = gpu.step(n)
+        dt_o, t_o = ora.step(n)
+        assert abs(dt_g - dt_o) <= 1e-12 * dt_o and abs(t_g - t_o) <= 1e-12 * t_o
+    _cmp_fields(gpu, ora, case)
+    gpu.destroy()
+
+
+def test_rhs_and_sensor_calls_between_steps(S):
+    """streams_rhs / streams_get_sensor between steps neither change the state nor confuse the buffer bookkeeping."""
+    case = W.channel(48, 40, 36, seed=7)
+    gpu, ora = S(case), _oracle(case)
+    _cmp_rhs(gpu, ora, case)
+    gpu.step(2); ora.step(2)
+    w_before = gpu.get_fields()
+    _cmp_rhs(gpu, ora, case)                       # RHS of the evolved state
+    gpu.get_sensor()
+    _cmp_rhs(gpu, ora, case)                       # twice in a row
+    assert np.array_equal(gpu.get_fields(), w_before)
+    gpu.step(3); ora.step(3)
+    _cmp_fields(gpu, ora, case)
+    gpu.destroy()
+
+
+def test_set_fields_mid_run_restarts_cleanly(S):
+    case = W.isotropic_turbulence(nx=36, ny=34, nz=38, mach_t=0.6, k0=3.0, kmax=8, seed=22, dilatational=0.5)
+    gpu, ora = S(case), _oracle(case)
+    gpu.step(3)
+    gpu.set_fields(case.w0)                        # back to the initial state: stale primitives / rate must not be used
+    dt_g, t_g = gpu.step(4)
+    dt_o, t_o = ora.step(4)
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o and abs(t_g - t_o) <= 1e-12 * t_o
+    _cmp_fields(gpu, ora, case)
+    gpu.destroy()
+
+
+@pytest.mark.parametrize("shape", [(40, 36, 5), (5, 34, 37), (38, 4, 33), (3, 3, 3)])
+def test_narrow_periodic_extents(S, shape):
+    """Extents below 2 ng: a node has two periodic images in the ghost layers, which the owner-writes path does not
+    cover; the library must fall back to the ghost kernels for that direction."""
+    nx, ny, nz = shape
+    rng = np.random.default_rng(5)
+    rho = 1.0 + 0.1 * rng.uniform(-1, 1, (nz, ny, nx))
+    u, v, w = (0.3 * rng.uniform(-1, 1, (nz, ny, nx)) for _ in range(3))
+    p = 1.0 + 0.1 * rng.uniform(-1, 1, (nz, ny, nx))
+    base = W.isotropic_turbulence(nx=12, ny=12, nz=12, mach_t=0.3, k0=2.0, kmax=3, seed=1)
+    case = base.replace(name="narrow", nx=nx, ny=ny, nz=nz, w0=W.conserved_from_primitive(rho, u, v, w, p, base.gamma),
+                        sensor_threshold=0.05)
+    gpu, ora = S(case), _oracle(case)
+    _cmp_rhs(gpu, ora, case)
+    th_g, mk_g = gpu.get_sensor()
+    th_o, mk_o, _ = ora.sensor()
+    assert np.array_equal(th_g, th_o) and np.array_equal(mk_g, mk_o)
+    gpu.step(3); ora.step(3)
+    _cmp_fields(gpu, ora, case)
+    gpu.destroy()
+
+
+def test_fixed_dt_and_central_inviscid(S):
+    """dt_fixed: no rate is ever reduced; the lean (central, inviscid) variant with its L2 prefetch."""
+    case = W.config(0).replace(dt_fixed=2e-3)
+    gpu, ora = S(case), _oracle(case)
+    dt_g, t_g = gpu.step(6)
+    dt_o, t_o = ora.step(6)
+    assert dt_g == 2e-3 and abs(t_g - t_o) <= 1e-12 * t_o
+    _cmp_fields(gpu, ora, case)
+    gpu.destroy()
