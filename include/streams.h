@@ -67,7 +67,10 @@ typedef struct {
   double freestream[5];       /* conserved free-stream state for STREAMS_BC_FREESTREAM ghosts   */
 } streams_gas;
 
-/* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5). */
+/* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5).
+ * This build instantiates the families m = 1, 2, 3: central order 2m with WENO order 2m-1 and viscous order 2m
+ * (2/1/2, 4/3/4, 6/5/6); an order the chosen mode does not use is ignored; any other combination makes
+ * streams_workspace_bytes return 0 and streams_init return STREAMS_EINVAL (never later). */
 typedef struct {
   int central_order;          /* 2L: 2, 4, 6, 8                                                 */
   int weno_order;             /* 2r-1: 1, 3, 5, 7; ignored when flux_mode == CENTRAL            */

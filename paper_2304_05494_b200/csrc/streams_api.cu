@@ -71,10 +71,9 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.L = sc->central_order / 2;
   S.Lv = gas->visc_law == STREAMS_VISC_NONE ? 0 : sc->visc_order / 2;
   S.r = sc->flux_mode == STREAMS_FLUX_CENTRAL ? 0 : (sc->weno_order + 1) / 2;
-  S.ng = S.L > S.Lv ? S.L : S.Lv;
-  if (S.r > S.ng) S.ng = S.r;
   if (!rhs_supported(S.L, S.Lv, S.r, sc->flux_mode, gas->visc_law))
-    return "this build instantiates central order 6, WENO order 5, viscous order 6 only";
+    return "this build instantiates the order families 2/1/2, 4/3/4 and 6/5/6 (central / WENO / viscous) only";
+  S.ng = 3;                                               // the layout and the tiles always carry three ghost layers
   if (g->nx < S.ng || g->ny < S.ng || g->nz < S.ng) return "each extent must be at least the ghost width";
   S.ox = 16;                                              // interior i = 0 starts a 128-byte line
   S.px = (int)align_up((size_t)S.ox + g->nx + S.ng, 16);

@@ -239,13 +239,14 @@ __device__ __forceinline__ double ddc_g(const DevP& P, const G& g, double metric
 #ifndef STREAMS_SENSOR_MINB
 #define STREAMS_SENSOR_MINB 3
 #endif
-template <bool MASK, bool THETA, int TY>
+template <int L, bool MASK, bool THETA, int TY>
 __global__ void __launch_bounds__(MTX * TY, STREAMS_SENSOR_MINB)
 sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring, const DevP P,
                     int nbx, int nby, int kz) {
   using G = MarchGeom<TY>;
   using SM = SensorSmem<TY>;
-  constexpr int L = 3, NG = 3;
+  constexpr int NG = 3;                    // ghost width / ring depth of the layout; the stencil uses L <= NG of it
+  static_assert(L <= NG, "ring depth");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][3][PLANE]
   double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][3][NT]
@@ -633,11 +634,11 @@ static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st
   else scalar_ghost_kernel<false><<<gg, 256, 0, st>>>(P);
   return 2;
 }
-template <bool MASK, bool THETA>
+template <int L, bool MASK, bool THETA>
 static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t st) {
   constexpr int TY = STREAMS_SENSOR_TY;
   using SM = SensorSmem<TY>;
-  auto kern = sensor_march_kernel<MASK, THETA, TY>;
+  auto kern = sensor_march_kernel<L, MASK, THETA, TY>;
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
@@ -656,10 +657,17 @@ static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t 
 }
 
 int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool theta, cudaStream_t st) {
-  if (L == 3 && P.ng == 3) {
-    if (theta) return launch_sensor_march<true, true>(P, mp, st);
-    if (mask) return launch_sensor_march<true, false>(P, mp, st);
-    return launch_sensor_march<false, false>(P, mp, st);
+  if (L <= 3 && P.ng == 3) {
+#define STREAMS_SENSOR(LL)                                              \
+  do {                                                                  \
+    if (theta) return launch_sensor_march<LL, true, true>(P, mp, st);   \
+    if (mask) return launch_sensor_march<LL, true, false>(P, mp, st);   \
+    return launch_sensor_march<LL, false, false>(P, mp, st);            \
+  } while (0)
+    if (L == 1) STREAMS_SENSOR(1);
+    if (L == 2) STREAMS_SENSOR(2);
+    STREAMS_SENSOR(3);
+#undef STREAMS_SENSOR
   }
   switch (L) {
     case 1: return launch_sensor_L<1>(P, mask, theta, st);
@@ -673,7 +681,7 @@ int launch_flags(const DevP& P, int L, int r, cudaStream_t st) {
   const int nwx = (P.nx + 7) / 8;
   const long long nwords = (long long)nwx * P.ny * P.nz;
   dim3 b(256), g((unsigned)((nwords + 255) / 256));
-  const bool reset_here = !(L == 3 && P.ng == 3);     // sensor_march_kernel resets the counters itself
+  const bool reset_here = !(L <= 3 && P.ng == 3);     // sensor_march_kernel resets the counters itself
   if (reset_here) reset_counters_kernel<<<1, 1, 0, st>>>(P);
   switch (r) {
     case 1: flags_kernel<1><<<g, b, 0, st>>>(P, nwx); break;

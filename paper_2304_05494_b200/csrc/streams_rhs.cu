@@ -832,18 +832,22 @@ static int launch_weno_T(const DevP& P, cudaStream_t st) {
   return 1;
 }
 
+// Instantiated scheme families: m = 1, 2, 3 with central order 2m, viscous order 2m and WENO order 2m - 1
+// (2/1/2, 4/3/4, 6/5/6); orders a mode does not use are ignored.  The layout always carries ng = 3 ghost layers.
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
-  const int lv = visc_law == VISC_NONE ? 3 : Lv;
-  const int rr = flux_mode == FLUX_CENTRAL ? 3 : r;
-  return L == 3 && lv == 3 && rr == 3;
+  return L >= 1 && L <= 3 && (visc_law == VISC_NONE || Lv == L) && (flux_mode == FLUX_CENTRAL || r == L);
 }
 
 int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
+  if (L == 1) return launch_main_T<1, 1, 1>(P, mp, sa, st);
+  if (L == 2) return launch_main_T<2, 2, 2>(P, mp, sa, st);
   return launch_main_T<3, 3, 3>(P, mp, sa, st);
 }
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st) {
   if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
+  if (L == 1) return launch_weno_T<1, 1>(P, st);
+  if (L == 2) return launch_weno_T<2, 2>(P, st);
   return launch_weno_T<3, 3>(P, st);
 }
 

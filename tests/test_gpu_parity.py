@@ -131,3 +131,38 @@ def test_state_errors(S):
     with pytest.raises(binding.StreamsError) as e:
         gpu.step(1)
     assert e.value.code == binding.STREAMS_ENAN
+
+
+# ---- the other instantiated order families: central / WENO / viscous = 2/1/2 and 4/3/4
+def _with_orders(case, m):
+    return case.replace(central_order=2 * m, weno_order=2 * m - 1, visc_order=2 * m, name=f"{case.name}_m{m}")
+
+
+@pytest.mark.parametrize("m", [1, 2])
+def test_order_family_hybrid_viscous_periodic(S, m):
+    case = W.isotropic_turbulence(nx=40, ny=37, nz=35, mach_t=0.6, k0=3.0, kmax=8, seed=31, dilatational=0.5)
+    check_case(S, _with_orders(case, m), 10, expect_activation=(0.002, 0.8))
+
+
+@pytest.mark.parametrize("m", [1, 2])
+def test_order_family_channel_walls(S, m):
+    check_case(S, _with_orders(W.channel(40, 36, 34, seed=32), m), 6)
+
+
+@pytest.mark.parametrize("m", [1, 2])
+def test_order_family_full_weno_and_central(S, m):
+    base = W.isotropic_turbulence(nx=34, ny=33, nz=36, mach_t=0.4, k0=3.0, kmax=8, seed=33, viscous=False,
+                                  flux_mode=W.FLUX_WENO)
+    check_case(S, _with_orders(base, m), 6)
+    check_case(S, _with_orders(base.replace(flux_mode=W.FLUX_CENTRAL), m), 6)
+
+
+def test_unsupported_order_mix_is_rejected_at_init(S):
+    from paper_2304_05494_b200 import binding
+    case = W.config(0).replace(central_order=8)
+    with pytest.raises(binding.StreamsError) as e:
+        S(case)
+    assert e.value.code == binding.STREAMS_EINVAL
+    mixed = W.isotropic_turbulence(nx=16, ny=16, nz=16, mach_t=0.3, k0=2.0, kmax=4, seed=1).replace(weno_order=3)
+    with pytest.raises(binding.StreamsError):
+        S(mixed)
