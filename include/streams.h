@@ -127,6 +127,13 @@ int streams_get_activation(streams_ctx* ctx, long long* flagged_nodes, long long
 int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long long* shock_sum,
                                   long long* interfaces_sum, long long* evaluations);
 
+/* Imposes the node mask of the shock sensor (hybrid mode): from the next evaluation on, the sensor still
+ * computes theta and the dilatation but flags exactly the nodes with mask[n] != 0 (values must be 0 or 1),
+ * mask = [nz][ny][nx] bytes, HOST or DEVICE (copied before return; synchronises the stream for a host source).
+ * NULL restores the sensor's own decision.  This is the hook of the paper's activation sweep (PAPER:497-501:
+ * WENO forced on a chosen fraction of the points).  STREAMS_EINVAL unless flux_mode == STREAMS_FLUX_HYBRID. */
+int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int src_is_device);
+
 /* Number of kernels the library has launched on this context since streams_init. */
 long long streams_kernel_launches(const streams_ctx* ctx);
 

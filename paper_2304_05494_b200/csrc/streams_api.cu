@@ -23,7 +23,7 @@ struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
   size_t N, lcap;
-  size_t off_w, off_q, off_q2, off_theta, off_mask, off_nflag, off_ilist, off_dF, off_counters, off_R,
+  size_t off_w, off_q, off_q2, off_theta, off_mask, off_movr, off_nflag, off_ilist, off_dF, off_counters, off_R,
       off_metrics, off_scal, total;
   int nq;
 };
@@ -90,6 +90,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.off_q2 = take((size_t)S.nq * S.fs * 8);      // writes the primitives of the updated state into the other
   S.off_theta = take(S.N * 8);
   S.off_mask = take(S.fs);
+  S.off_movr = take(hyb ? S.fs : 256);                    // imposed mask (streams_set_mask_override)
   S.off_nflag = take(hyb ? S.fs : 256);
   {
     const size_t face = std::max(std::max((size_t)g->ny * g->nz, (size_t)g->nx * g->nz), (size_t)g->nx * g->ny);
@@ -311,6 +312,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   ctx->prims_interior = false; ctx->rate_ready = false;
   P.theta = (double*)(ctx->base + S.off_theta);
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
+  P.mask_ovr = nullptr;
   P.nflag = (unsigned char*)(ctx->base + S.off_nflag);
   P.ilist = (int*)(ctx->base + S.off_ilist);
   P.lcap = (long long)S.lcap;
@@ -526,6 +528,25 @@ int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long
   if (flagged_sum) *flagged_sum = (long long)h[1];
   if (evaluations) *evaluations = (long long)h[2];
   if (interfaces_sum) for (int d = 0; d < 3; ++d) interfaces_sum[d] = (long long)h[3 + d];
+  return STREAMS_OK;
+}
+
+int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int src_is_device) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (ctx->scheme.flux_mode != STREAMS_FLUX_HYBRID) return fail(ctx, STREAMS_EINVAL, "a node mask exists in hybrid mode only");
+  DevP& P = ctx->P;
+  if (!mask) { P.mask_ovr = nullptr; return STREAMS_OK; }
+  unsigned char* dst = (unsigned char*)(ctx->base + ctx->S.off_movr);
+  cudaMemcpy3DParms p;
+  std::memset(&p, 0, sizeof p);
+  p.srcPtr = make_cudaPitchedPtr((void*)mask, (size_t)P.nx, P.nx, P.ny);
+  p.dstPtr = make_cudaPitchedPtr((void*)dst, (size_t)P.px, P.px, P.py);
+  p.dstPos = make_cudaPos((size_t)P.ox, P.ng, P.ng);
+  p.extent = make_cudaExtent((size_t)P.nx, P.ny, P.nz);
+  p.kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CU(cudaMemcpy3DAsync(&p, ctx->stream));
+  if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));
+  P.mask_ovr = dst;
   return STREAMS_OK;
 }
 

@@ -206,7 +206,8 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
     if (!(th > 0.0)) th = 0.0;
     if (THETA) P.theta[iidx(P, i, j, k)] = th;
     if (MASK) {
-      const unsigned char m = (th > P.thr) ? 1 : 0;
+      unsigned char m = (th > P.thr) ? 1 : 0;
+      if (P.mask_ovr) m = P.mask_ovr[n];
       P.mask[n] = m;
     }
   }
@@ -340,6 +341,7 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
         if (!(th > 0.0)) th = 0.0;
         if (THETA) P.theta[iidx(P, i, j, k)] = th;
         mk = (th > P.thr) ? 1 : 0;
+        if (MASK && P.mask_ovr) mk = P.mask_ovr[n];       // imposed mask (activation sweeps)
         if (MASK) P.mask[n] = mk;
       }
       // face ghosts of div / mask (S6), written by the node they copy: its periodic image, or the NG ghost nodes

@@ -110,3 +110,35 @@ def test_fixed_dt_and_central_inviscid(S):
     assert dt_g == 2e-3 and abs(t_g - t_o) <= 1e-12 * t_o
     _cmp_fields(gpu, ora, case)
     gpu.destroy()
+
+
+@pytest.mark.parametrize("kind", ["slab", "random", "all", "none"])
+def test_mask_override_matches_the_oracle(S, kind):
+    """streams_set_mask_override (the activation-sweep hook): WENO exactly where the mask says."""
+    case = W.isotropic_turbulence(nx=40, ny=36, nz=34, mach_t=0.5, k0=3.0, kmax=8, seed=41, dilatational=0.3)
+    rng = np.random.default_rng(3)
+    shape = (case.nz, case.ny, case.nx)
+    if kind == "slab":
+        mask = np.zeros(shape, np.uint8); mask[: case.nz // 3] = 1
+    elif kind == "random":
+        mask = (rng.uniform(size=shape) < 0.03).astype(np.uint8)
+    elif kind == "all":
+        mask = np.ones(shape, np.uint8)
+    else:
+        mask = np.zeros(shape, np.uint8)
+    gpu, ora = S(case), _oracle(case)
+    gpu.set_mask_override(mask)
+    ora.set_mask_override(mask)
+    _cmp_rhs(gpu, ora, case)
+    th_g, mk_g = gpu.get_sensor()
+    th_o, mk_o, _ = ora.sensor()
+    assert np.array_equal(mk_g, mask) and np.array_equal(mk_o, mask) and np.array_equal(th_g, th_o)
+    flagged, _, ifaces = gpu.get_activation()
+    assert flagged == int(mask.sum())
+    assert ifaces == [int(ora.interface_flags(d).sum()) for d in range(3)]
+    gpu.step(3); ora.step(3)
+    _cmp_fields(gpu, ora, case)
+    # back to the sensor's own decision
+    gpu.set_mask_override(None); ora.set_mask_override(None)
+    _cmp_rhs(gpu, ora, case)
+    gpu.destroy()
