@@ -61,6 +61,9 @@ def make_case(index: int, seed_offset: int = 0):
     if index == 4:
         return W.isotropic_turbulence(n=640, mach_t=0.8, k0=8.0, kmax=64, seed=4 + 100 * seed_offset, nsteps=10,
                                       name="cfg4_iso_640")
+    if index == 5:   # SURVEY 8(d) "opt": the paper's own grid shape, not divisible by any tile
+        return W.isotropic_turbulence(nx=420, ny=250, nz=320, mach_t=0.6, k0=4.0, kmax=32, seed=5 + 100 * seed_offset,
+                                      nsteps=20, name="opt_iso_420x250x320")
     raise SystemExit(f"unknown config {index}")
 
 
@@ -71,6 +74,7 @@ WORKLOAD_TEXT = {
     2: "configs[2]: supersonic isothermal-wall channel 256x192x128, tanh-stretched y, hybrid",
     3: "configs[3]: supersonic flat-plate boundary-layer box 1024x256x256, stretched y, hybrid, seeded shocklets",
     4: "configs[4]: capacity run 640^3 periodic compressible turbulence Mach_t 0.8, k0=8, hybrid",
+    5: "sweep grid 420x250x320 (the paper's grid shape, PAPER:355), periodic turbulence as configs[1]",
 }
 
 
@@ -209,6 +213,9 @@ def oracle_case_for(index: int):
     not depend on the grid size beyond cache effects)."""
     if index == 3:
         return W.boundary_layer(512, 128, 128, seed=3, nsteps=20), "same recipe on 512x128x128 (1/8 of the points)"
+    if index == 5:
+        return (W.isotropic_turbulence(nx=210, ny=125, nz=160, mach_t=0.6, k0=4.0, kmax=32, seed=5, nsteps=20,
+                                       name="opt_iso_210x125x160"), "same recipe on 210x125x160 (1/8 of the points)")
     if index == 4:
         return (W.isotropic_turbulence(n=200, mach_t=0.8, k0=8.0, kmax=64, seed=4, nsteps=10, name="cfg4_iso_200"),
                 "same recipe on 200^3 (1/33 of the points)")
@@ -267,9 +274,20 @@ def run_ours(args):
         dist.barrier()
 
     case = make_case(args.config, seed_offset=rank)
+    # sweep knobs (not used by the default run): order family, flux mode, imposed activation
+    m = args.order_family
+    case = case.replace(central_order=2 * m, weno_order=2 * m - 1, visc_order=2 * m)
+    if args.flux_mode:
+        case = case.replace(flux_mode={"central": W.FLUX_CENTRAL, "weno": W.FLUX_WENO, "hybrid": W.FLUX_HYBRID}[args.flux_mode])
     N = case.npoints
     gpu = binding.Streams(case, device=f"cuda:{local}")
     dev = gpu.device
+    if args.activation is not None:
+        if case.flux_mode != W.FLUX_HYBRID:
+            raise SystemExit("--activation needs hybrid mode")
+        imposed = np.zeros((case.nz, case.ny, case.nx), dtype=np.uint8)
+        imposed[: int(round(args.activation * case.nz))] = 1
+        gpu.set_mask_override(imposed)
     state_bytes = 5 * N * 8
 
     rep = replicas.Replicas(dist, dev)          # barrier + max over ranks (tests/test_replicas_gloo.py)
@@ -404,7 +422,9 @@ def run_ours(args):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD_TEXT[args.config], "grid": [case.nx, case.ny, case.nz], "points": N,
-                   "orders": "central 6 / WENO 5 / viscous 6", "parallelism": "1 GPU" if world == 1 else
+                   "orders": "central %d / WENO %d / viscous %d" % (case.central_order, case.weno_order, case.visc_order),
+                   "flux_mode": {W.FLUX_CENTRAL: "central", W.FLUX_WENO: "weno", W.FLUX_HYBRID: "hybrid"}[case.flux_mode],
+                   "imposed_activation": args.activation, "parallelism": "1 GPU" if world == 1 else
                    f"{world} independent replicas (no data-path collective)",
                    "l2": "inputs larger than L2 (workspace %.2f GB vs 126 MB)" % (gpu.workspace_bytes / 1e9)
                    if gpu.workspace_bytes > 4 * 126e6 else "workspace %.1f MB is L2-resident; latency point, not a roofline point"
@@ -437,6 +457,11 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--order-family", type=int, default=3, choices=[1, 2, 3],
+                    help="m: central order 2m / WENO order 2m-1 / viscous order 2m (default 3 = 6/5/6)")
+    ap.add_argument("--flux-mode", default=None, choices=["central", "weno", "hybrid"], help="override the config's flux mode")
+    ap.add_argument("--activation", type=float, default=None,
+                    help="hybrid mode: impose the node mask on this fraction of the z planes (PAPER:497-501 sweep)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
