@@ -745,10 +745,21 @@ __global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_list_kernel(const
   __shared__ double s_st[6 * 2 * R * WTH];
   const int c0 = P.counters[C_NIFACE], c1 = P.counters[C_NIFACE + 1], c2 = P.counters[C_NIFACE + 2];
   const int g0 = (c0 + WTH - 1) / WTH, g1 = (c1 + WTH - 1) / WTH, g2 = (c2 + WTH - 1) / WTH;
-  for (int g = blockIdx.x; g < g0 + g1 + g2; g += gridDim.x) {
-    if (g < g0) weno_list_item<0, L, R>(P, g * WTH + threadIdx.x, c0, s_st);
-    else if (g < g0 + g1) weno_list_item<1, L, R>(P, (g - g0) * WTH + threadIdx.x, c1, s_st);
-    else weno_list_item<2, L, R>(P, (g - g0 - g1) * WTH + threadIdx.x, c2, s_st);
+#ifndef STREAMS_WENO_CHUNK
+#define STREAMS_WENO_CHUNK 4
+#endif
+  // blocks take chunks of consecutive groups round-robin: list neighbours are grid neighbours, so the stencil rows
+  // of a group are still in this SM's L1 when the next rows' interfaces need them, while all blocks advance through
+  // the lists together (one direction's code in the instruction cache at a time)
+  constexpr int CH = STREAMS_WENO_CHUNK;
+  const int gt = g0 + g1 + g2;
+  for (int gc = blockIdx.x * CH; gc < gt; gc += gridDim.x * CH) {
+#pragma unroll 1
+    for (int g = gc; g < min(gt, gc + CH); ++g) {
+      if (g < g0) weno_list_item<0, L, R>(P, g * WTH + threadIdx.x, c0, s_st);
+      else if (g < g0 + g1) weno_list_item<1, L, R>(P, (g - g0) * WTH + threadIdx.x, c1, s_st);
+      else weno_list_item<2, L, R>(P, (g - g0 - g1) * WTH + threadIdx.x, c2, s_st);
+    }
   }
 }
 
