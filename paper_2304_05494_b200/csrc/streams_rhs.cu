@@ -486,6 +486,26 @@ __device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
   return (a0 * q0 + a1 * q1 + a2 * q2 + a3 * q3) * rcp_pos(((a0 + a1) + a2) + a3);
 }
 
+// Both reconstructions of a characteristic field (upwind and mirrored stencil) as ONE call with the arguments by
+// value, in registers: the five fields of an interface then share one copy of the code instead of ten inlined
+// reconstructions (instruction-cache footprint: the list kernel's straight-line code shrinks by 30 %), while the two
+// reconstructions of a field still interleave.  STREAMS_WENO_REC_INLINE restores the inlined form.
+template <int R>
+__device__ __forceinline__ double weno_rec_pair(const double* gp, const double* gm, double eps) {
+  return weno_rec<R>(gp, eps) + weno_rec<R>(gm, eps);
+}
+#ifndef STREAMS_WENO_REC_INLINE
+__device__ __noinline__ double weno_rec5_pair_call(double p0, double p1, double p2, double p3, double p4, double m0, double m1,
+                                                  double m2, double m3, double m4, double eps) {
+  const double gp[5] = {p0, p1, p2, p3, p4}, gm[5] = {m0, m1, m2, m3, m4};
+  return weno_rec<3>(gp, eps) + weno_rec<3>(gm, eps);
+}
+template <>
+__device__ __forceinline__ double weno_rec_pair<3>(const double* gp, const double* gm, double eps) {
+  return weno_rec5_pair_call(gp[0], gp[1], gp[2], gp[3], gp[4], gm[0], gm[1], gm[2], gm[3], gm[4], eps);
+}
+#endif
+
 // ---------------------------------------------------------------------------------------------
 // WENO characteristic flux at interface n+1/2 along D (O3), and the central flux (O1) it replaces.
 // Characteristic projections are formed from primitives: with W the conserved state and
@@ -604,7 +624,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[0], lw, lf);
     gm[NS - 1 - m] = fma(-lam[0], lw, lf);          // mirrored: gm[0] is node n+R
   }
-  const double g0 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  const double g0 = weno_rec_pair<R>(gp, gm, P.weno_eps);
   // u + c
 #pragma unroll
   for (int m = 0; m < NS; ++m) {
@@ -612,7 +632,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[2], lw, lf);
     gm[NS - 1 - m] = fma(-lam[2], lw, lf);
   }
-  const double g4 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  const double g4 = weno_rec_pair<R>(gp, gm, P.weno_eps);
   // entropy
 #pragma unroll
   for (int m = 0; m < NS; ++m) {
@@ -621,7 +641,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[1], lw, lf);
     gm[NS - 1 - m] = fma(-lam[1], lw, lf);
   }
-  const double g1 = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+  const double g1 = weno_rec_pair<R>(gp, gm, P.weno_eps);
   // the two shear fields
   double gs[2];
 #pragma unroll
@@ -634,7 +654,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
       gp[m] = fma(lam[1], lw, lf);
       gm[NS - 1 - m] = fma(-lam[1], lw, lf);
     }
-    gs[e] = weno_rec<R>(gp, P.weno_eps) + weno_rec<R>(gm, P.weno_eps);
+    gs[e] = weno_rec_pair<R>(gp, gm, P.weno_eps);
   }
   // f = sum over the fields of g r: r(u-+c) = (1, vbar -+ c e_D, H -+ un c), r(entropy) = (1, vbar, q^2/2), r(shear t) = (0, e_t, vbar_t)
   const double gsum = (g0 + g4) + g1, gdc = (g4 - g0) * cb;
