@@ -231,17 +231,15 @@ cudaError_t prof_drain(streams_ctx* ctx) {
 // After an updating stage the fused RHS kernel has already written the primitives of every interior node of the
 // new state (and, on request, reduced its time-step rate): only the ghost shell is left.  Otherwise (first
 // evaluation after streams_set_fields, or a dt wanted that no stage prepared) the full pass runs.
-int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta) {
+int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta, bool step_start = false) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
   const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0) && !ctx->rate_ready;
   if (ctx->prims_interior && !reduce_dt) timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
   else timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
   ctx->prims_interior = true;
-  if (want_dt) {
-    timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, st); });
-    ctx->rate_ready = false;                        // dt_finalize consumed (and zeroed) the rate
-  }
+  if (step_start) timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, want_dt, st); });
+  if (want_dt) ctx->rate_ready = false;             // dt_finalize consumed (and zeroed) the rate
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
   if (hyb || visc || theta)
@@ -451,7 +449,7 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
   for (int s = 0; s < nsteps; ++s) {
     const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
     for (int l = 0; l < 3; ++l) {
-      enqueue_prepare(ctx, want_dt && l == 0, false);
+      enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
       StageArgs sa;
       sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
       sa.r_dense = nullptr;
@@ -463,7 +461,6 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
       ctx->prims_interior = true;
       if (sa.want_rate) ctx->rate_ready = true;
     }
-    timed(ctx, STREAMS_K_MISC, [&] { return launch_step_end(ctx->P, ctx->stream); });
     ctx->step_count += 1;
   }
   CU(cudaGetLastError());

@@ -519,16 +519,17 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   }
 }
 
-// a9, second half: dt = CFL / (the rate fill_prim_kernel<.., DT> reduced), or the fixed step.
-__global__ void dt_finalize_kernel(const DevP P, double dt_fixed) {
-  const double rate = P.scal[S_RATE];
-  const double dt = dt_fixed > 0.0 ? dt_fixed : P.cfl / rate;
-  P.scal[S_DT] = dt;
-  P.scal[S_RATE] = 0.0;
-  if (!isfinite(dt)) P.scal[S_NAN] = 1.0;
-}
-
-__global__ void step_end_kernel(const DevP P) {
+// Step scalars, one thread at the start of every step.  recompute: a9, second half: dt = CFL / (the rate reduced by
+// fill_prim_kernel<.., DT> or by the last stage's RHS epilogue), or the fixed step.  Always: the time and the step count
+// the step will have reached when its three stages are done (read by streams_step after them).
+__global__ void dt_finalize_kernel(const DevP P, double dt_fixed, int recompute) {
+  if (recompute) {
+    const double rate = P.scal[S_RATE];
+    const double dt = dt_fixed > 0.0 ? dt_fixed : P.cfl / rate;
+    P.scal[S_DT] = dt;
+    P.scal[S_RATE] = 0.0;
+    if (!isfinite(dt)) P.scal[S_NAN] = 1.0;
+  }
   P.scal[S_TIME] = P.scal[S_TIME] + P.scal[S_DT];
   P.scal[S_NSTEP] = P.scal[S_NSTEP] + 1.0;
 }
@@ -694,13 +695,8 @@ int launch_flags(const DevP& P, int L, int r, cudaStream_t st) {
   return reset_here ? 2 : 1;
 }
 
-int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st) {
-  dt_finalize_kernel<<<1, 1, 0, st>>>(P, dt_fixed);
-  return 1;
-}
-
-int launch_step_end(const DevP& P, cudaStream_t st) {
-  step_end_kernel<<<1, 1, 0, st>>>(P);
+int launch_dt(const DevP& P, double dt_fixed, bool recompute, cudaStream_t st) {
+  dt_finalize_kernel<<<1, 1, 0, st>>>(P, dt_fixed, recompute ? 1 : 0);
   return 1;
 }
 

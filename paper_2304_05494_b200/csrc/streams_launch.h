@@ -31,8 +31,7 @@ int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st);   // with_dt
 int launch_fill_ghosts(const DevP& P, cudaStream_t st);                // ghost shell only (interior primitives already current)
 int launch_sensor(const DevP& P, const MarchMaps& maps, int L, bool mask, bool theta, cudaStream_t st);
 int launch_flags(const DevP& P, int L, int r, cudaStream_t st);
-int launch_dt(const DevP& P, double dt_fixed, cudaStream_t st);
-int launch_step_end(const DevP& P, cudaStream_t st);
+int launch_dt(const DevP& P, double dt_fixed, bool recompute, cudaStream_t st);   // step scalars (dt, time, step count)
 // The per-interface WENO flux corrections (run first) and the fused RHS + update over all nodes; each
 // returns the number of launches (0 when the flux mode does not need it) or < 0 if the (L, Lv, r)
 // combination is not instantiated.
