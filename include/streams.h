@@ -134,6 +134,17 @@ int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long
  * WENO forced on a chosen fraction of the points).  STREAMS_EINVAL unless flux_mode == STREAMS_FLUX_HYBRID. */
 int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int src_is_device);
 
+/* Sum reductions over the interior nodes (PAPER:218-236 compute_residual; Table 2 "forcing term evaluations (sum
+ * reduction)"), in a fixed order: the five doubles of out5 (HOST) are reproducible bit for bit.
+ *   STREAMS_SUM_STATE:    out5[q] = sum of w_q dV, dV = dx dz / (d eta/dy)(j): the volume integrals of mass, momentum
+ *                         and total energy, i.e. the quantities the scheme conserves discretely in a periodic box;
+ *   STREAMS_SUM_RESIDUAL: out5[q] = sum of R_q^2 with R the right-hand side (per unit time) of the CURRENT state as
+ *                         evaluated by the last streams_rhs (the paper's residual is entry 1, rho u);
+ *                         STREAMS_ESTATE if the state changed since (or no streams_rhs was called).
+ * Synchronises the stream. */
+enum { STREAMS_SUM_STATE = 0, STREAMS_SUM_RESIDUAL = 1 };
+int streams_get_sums(streams_ctx* ctx, int kind, double* out5);
+
 /* Number of kernels the library has launched on this context since streams_init. */
 long long streams_kernel_launches(const streams_ctx* ctx);
 

@@ -24,7 +24,7 @@ struct Sizes {
   size_t fs;            // doubles per padded field
   size_t N, lcap;
   size_t off_w, off_q, off_q2, off_theta, off_mask, off_movr, off_nflag, off_ilist, off_dF, off_counters, off_R,
-      off_metrics, off_scal, total;
+      off_metrics, off_scal, off_sums, total;
   int nq;
 };
 
@@ -102,6 +102,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.off_R = take(5 * S.fs * 8);
   S.off_metrics = take(3 * (size_t)g->ny * 8);
   S.off_scal = take(S_COUNT * 8);
+  S.off_sums = take((size_t)sums_scratch_doubles() * 8);
   S.total = off;
   return nullptr;
 }
@@ -118,6 +119,7 @@ struct streams_ctx {
   double* qbuf[2];
   int cur;                  // index of the buffer that holds (or will receive) the primitives of the current state
   bool prims_interior;      // qbuf[cur] already holds the primitives of every interior node (written by the last stage)
+  bool r_valid;             // DevP::R holds the right-hand side of the current state (after streams_rhs)
   bool rate_ready;          // scal[S_RATE] already holds the rate of the current state (reduced by the last stage)
   cudaStream_t stream;
   char* base;
@@ -307,7 +309,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.w = (double*)(ctx->base + S.off_w);
   ctx->qbuf[0] = (double*)(ctx->base + S.off_q);
   ctx->qbuf[1] = (double*)(ctx->base + S.off_q2);
-  ctx->prims_interior = false; ctx->rate_ready = false;
+  ctx->prims_interior = false; ctx->rate_ready = false; ctx->r_valid = false;
   P.theta = (double*)(ctx->base + S.off_theta);
   P.mask = (unsigned char*)(ctx->base + S.off_mask);
   P.mask_ovr = nullptr;
@@ -405,6 +407,7 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
   ctx->step_count = 0;
   ctx->prims_interior = false;                       // the next evaluation runs the full ghost + primitive pass
   ctx->rate_ready = false;
+  ctx->r_valid = false;
   return STREAMS_OK;
 }
 
@@ -436,6 +439,7 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   sa.r_dense = rhs_out_dev; sa.q_out = nullptr; sa.want_rate = 0;
   if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
   CU(cudaGetLastError());
+  ctx->r_valid = true;
   return STREAMS_OK;
 }
 
@@ -446,6 +450,7 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
   // Wray's low-storage RK3 (O5 / S12)
   const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
   const double rhk[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+  if (nsteps > 0) ctx->r_valid = false;              // R becomes the low-storage scheme's previous-stage register
   for (int s = 0; s < nsteps; ++s) {
     const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
     for (int l = 0; l < 3; ++l) {
@@ -544,6 +549,21 @@ int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int s
   CU(cudaMemcpy3DAsync(&p, ctx->stream));
   if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));
   P.mask_ovr = dst;
+  return STREAMS_OK;
+}
+
+int streams_get_sums(streams_ctx* ctx, int kind, double* out5) {
+  if (!ctx || !out5) return fail(ctx, STREAMS_EINVAL, "null argument");
+  if (kind != STREAMS_SUM_STATE && kind != STREAMS_SUM_RESIDUAL) return fail(ctx, STREAMS_EINVAL, "bad kind");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
+  if (kind == STREAMS_SUM_RESIDUAL && !ctx->r_valid)
+    return fail(ctx, STREAMS_ESTATE, "the residual needs a streams_rhs of the current state");
+  double* scratch = (double*)(ctx->base + ctx->S.off_sums);
+  double* out_dev = scratch + (sums_scratch_doubles() - 8);
+  timed(ctx, STREAMS_K_MISC, [&] { return launch_sums(ctx->P, kind, scratch, out_dev, ctx->stream); });
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(out5, out_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
   return STREAMS_OK;
 }
 

@@ -591,6 +591,66 @@ double measure_fp64(cudaStream_t st, int kind, int repeats) {
   return cudaGetLastError() == cudaSuccess ? best : -1.0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Sum reductions ("compute_residual", Table 2 "forcing term evaluations"): five sums over the interior
+// nodes in a FIXED order, so the result is reproducible bit for bit: block b owns the rows b, b + gridDim.x, ... and
+// sums them in that order (threads stride the row, shuffle tree, warps in index order), a second one-block launch adds
+// the per-block partials in index order.  KIND 0: sum_q of w_q dV with dV = dx dz / eta_y(j) (volume integrals of the
+// conserved variables: the discretely conserved quantities); KIND 1: sum of R_q^2 (the paper's residual of the
+// right-hand side held in DevP::R).
+// ---------------------------------------------------------------------------------------------
+constexpr int SUM_BLOCKS = 592, SUM_THREADS = 256;
+
+template <int KIND>
+__global__ void __launch_bounds__(SUM_THREADS) sum_partial_kernel(const DevP P, double* __restrict__ partial) {
+  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  const long long rows = (long long)P.ny * P.nz;
+  const double dxdz = 1.0 / (P.inv_dx * P.inv_dz);
+  for (long long row = blockIdx.x; row < rows; row += gridDim.x) {
+    const int k = (int)(row / P.ny), j = (int)(row - (long long)k * P.ny);
+    const double wgt = KIND == 0 ? dxdz / P.eta_y_c[j] : 1.0;
+    const long long n0 = pidx(P, 0, j, k);
+    for (int i = threadIdx.x; i < P.nx; i += SUM_THREADS) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) {
+        const double v = (KIND == 0 ? P.w : P.R)[q * P.fs + n0 + i];
+        acc[q] += KIND == 0 ? v * wgt : v * v;
+      }
+    }
+  }
+  __shared__ double sm[5][SUM_THREADS / 32];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    double v = acc[q];
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+    if ((threadIdx.x & 31) == 0) sm[q][threadIdx.x >> 5] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 5) {
+    double v = 0.0;
+    for (int w = 0; w < SUM_THREADS / 32; ++w) v += sm[threadIdx.x][w];
+    partial[threadIdx.x * SUM_BLOCKS + blockIdx.x] = v;
+  }
+}
+
+__global__ void sum_final_kernel(const double* __restrict__ partial, double* __restrict__ out) {
+  if (threadIdx.x < 5) {
+    double v = 0.0;
+    for (int b = 0; b < SUM_BLOCKS; ++b) v += partial[threadIdx.x * SUM_BLOCKS + b];
+    out[threadIdx.x] = v;
+  }
+}
+
+// partial: 5 * SUM_BLOCKS doubles of scratch, out: 5 doubles (device)
+int launch_sums(const DevP& P, int kind, double* partial, double* out, cudaStream_t st) {
+  if (kind == 0) sum_partial_kernel<0><<<SUM_BLOCKS, SUM_THREADS, 0, st>>>(P, partial);
+  else sum_partial_kernel<1><<<SUM_BLOCKS, SUM_THREADS, 0, st>>>(P, partial);
+  sum_final_kernel<<<1, 32, 0, st>>>(partial, out);
+  return 2;
+}
+int sums_scratch_doubles() { return 5 * SUM_BLOCKS + 8; }
+
 // -------------------------------------------------------------------------- launch wrappers
 static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }
 

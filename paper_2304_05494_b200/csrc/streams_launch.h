@@ -37,6 +37,8 @@ int launch_dt(const DevP& P, double dt_fixed, bool recompute, cudaStream_t st); 
 // combination is not instantiated.
 int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st);
 int launch_rhs_main(const DevP& P, const MarchMaps& maps, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st);
+int launch_sums(const DevP& P, int kind, double* partial, double* out, cudaStream_t st);   // streams_get_sums
+int sums_scratch_doubles();
 double measure_fp64(cudaStream_t st, int kind, int repeats);   // streams_measure_fp64
 bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law);
 

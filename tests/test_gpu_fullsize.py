@@ -122,7 +122,11 @@ def run_sampled(S, case, boxes, need_flagged=True):
         boxes = list(boxes) + [(i - mx // 2, jj, k - mz // 2, mx, my, mz)]
     rhs_h = rhs.cpu().numpy()
     del rhs
+    sums0 = gpu.get_sums(0)
     dt, _ = gpu.step(1)
+    sums1 = gpu.get_sums(0)
+    if case.bc_y_lo == W.BC_PERIODIC:          # mass is conserved to round-off at any size (library's own fixed-order sums)
+        assert abs(sums1[0] - sums0[0]) <= 1e-13 * abs(sums0[0]), (sums0, sums1)
     w1 = gpu.get_fields()
     gpu.destroy()
     flagged = 0

@@ -142,3 +142,53 @@ def test_mask_override_matches_the_oracle(S, kind):
     gpu.set_mask_override(None); ora.set_mask_override(None)
     _cmp_rhs(gpu, ora, case)
     gpu.destroy()
+
+
+def _volume_weights(case):
+    """dV(j) of the oracle's reading S3: dx dz / (d eta/dy)(j), from the oracle's own metrics."""
+    ora = _oracle(case)
+    eta_y_c, _, _, _ = ora.metrics()
+    ora.close()
+    return (case.lx / case.nx) * (case.lz / case.nz) / eta_y_c
+
+
+def test_sum_reductions_match_plain_sums(S):
+    """streams_get_sums against the definitions written out with numpy on the oracle's numbers."""
+    from paper_2304_05494_b200 import binding
+    case = W.channel(48, 40, 36, seed=9)
+    gpu, ora = S(case), _oracle(case)
+    dv = _volume_weights(case)
+    state = gpu.get_sums(0)
+    ref = np.array([np.sum(case.w0[q] * dv[None, :, None]) for q in range(5)])
+    assert np.all(np.abs(state - ref) <= 1e-12 * np.maximum(np.abs(ref), 1.0)), (state, ref)
+    with pytest.raises(binding.StreamsError) as e:      # no streams_rhs yet
+        gpu.get_sums(1)
+    assert e.value.code == binding.STREAMS_ESTATE
+    gpu.rhs()
+    r_o = ora.rhs()
+    res = gpu.get_sums(1)
+    ref = np.array([np.sum(r_o[q] ** 2) for q in range(5)])
+    assert np.all(np.abs(res - ref) <= 1e-10 * ref), (res, ref)
+    assert np.array_equal(res, gpu.get_sums(1))         # fixed summation order: bit-reproducible
+    gpu.step(1)
+    with pytest.raises(binding.StreamsError):            # the state moved on: R is no longer its right-hand side
+        gpu.get_sums(1)
+    gpu.destroy()
+
+
+def test_discrete_conservation_on_the_gpu(S):
+    """Periodic box: mass is conserved to round-off by the hybrid viscous scheme, and so are momentum and total energy
+    without the (Laplacian-form, non-conservative) viscous terms (S11) -- measured with the library's own sums."""
+    for viscous in (True, False):
+        case = W.isotropic_turbulence(nx=48, ny=44, nz=40, mach_t=0.6, k0=3.0, kmax=8, seed=23, dilatational=0.4,
+                                      viscous=viscous)
+        gpu = S(case)
+        s0 = gpu.get_sums(0)
+        gpu.step(20)
+        s1 = gpu.get_sums(0)
+        scale = np.array([s0[0], s0[0], s0[0], s0[0], s0[4]])     # momentum sums are ~0: measure against the mass
+        drift = np.abs(s1 - s0) / scale
+        assert drift[0] <= 1e-13, drift
+        if not viscous:
+            assert np.all(drift <= 1e-12), drift
+        gpu.destroy()
