@@ -16,7 +16,7 @@ _c_ubyte_p = C.POINTER(C.c_ubyte)
 
 DBG_WENO_LINEAR = 1
 DBG_NO_PRESSURE = 2
-PART_X, PART_Y, PART_Z, PART_VISC, PART_ALL = 1, 2, 4, 8, 15
+PART_X, PART_Y, PART_Z, PART_VISC, PART_FORCE, PART_ALL = 1, 2, 4, 8, 16, 31
 
 
 class OracleParams(C.Structure):
@@ -36,6 +36,7 @@ class OracleParams(C.Structure):
         ("freestream", C.c_double * 5),
         ("sensor_threshold", C.c_double), ("weno_eps", C.c_double),
         ("cfl", C.c_double), ("dt_fixed", C.c_double),
+        ("accel", C.c_double * 3),
     ]
 
 
@@ -87,6 +88,8 @@ def params_from_case(case, dbg_flags: int = 0) -> OracleParams:
     p.dbg_flags = dbg_flags
     for q in range(5):
         p.freestream[q] = case.freestream[q]
+    for a in range(3):
+        p.accel[a] = case.accel[a]
     return p
 
 

@@ -27,6 +27,8 @@
 //                        uniform state, stretched-y order
 //   O5 RK3 / dt        : exp(z) Taylor polynomial, sum of coefficients, order 3
 //   O6 ghost fill      : wall at rest => R = 0 to round-off, Poiseuille balance
+//   S17 body force     : uniform state => R = (0, rho g, rho u.g) exactly; momentum budget of a periodic box;
+//                        Poiseuille flow driven by g instead of a pressure gradient
 // Unpinned against the real STREAmS code (not in the container): S1, S2, S4, S5,
 // S6, S7, S8, S9, S10, S12, S13, S15, S16 -- "parity unpinned vs STREAmS"; the
 // oracle's reading is the definition for this build.
@@ -46,7 +48,7 @@ enum { BC_PERIODIC = 0, BC_WALL = 1, BC_FREESTREAM = 2 };
 enum { VISC_NONE = 0, VISC_POWER = 1, VISC_SUTHERLAND = 2 };
 enum { FLUX_CENTRAL = 0, FLUX_WENO = 1, FLUX_HYBRID = 2 };
 enum { DBG_WENO_LINEAR = 1, DBG_NO_PRESSURE = 2 };
-enum { PART_X = 1, PART_Y = 2, PART_Z = 4, PART_VISC = 8, PART_ALL = 15 };
+enum { PART_X = 1, PART_Y = 2, PART_Z = 4, PART_VISC = 8, PART_FORCE = 16, PART_ALL = 31 };
 
 }  // namespace
 
@@ -67,6 +69,7 @@ extern "C" struct oracle_params {
   double freestream[5];
   double sensor_threshold, weno_eps;
   double cfl, dt_fixed;
+  double accel[3];              // uniform body acceleration g (S17)
 };
 
 namespace {
@@ -711,6 +714,26 @@ struct Solver {
         }
   }
 
+  // ---------------------------------------------------------------------------
+  // S17 forcing ("Forcing term evaluations"; Table 2): a uniform body acceleration g drives the flow
+  // (the streamwise pressure gradient of a channel): rho g on the momentum equations and its work (rho u) . g on
+  // the total energy.  The paper's controller, which adjusts g to hold the bulk flow rate, is host logic on top
+  // of the bulk sums and not part of the right-hand side.
+  // ---------------------------------------------------------------------------
+  void body_force() {
+    const double* g = P.accel;
+    if (g[0] == 0.0 && g[1] == 0.0 && g[2] == 0.0) return;
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          const size_t n = idx(i, j, k), o = iidx(i, j, k);
+          R[1][o] += w[0][n] * g[0];
+          R[2][o] += w[0][n] * g[1];
+          R[3][o] += w[0][n] * g[2];
+          R[4][o] += (w[1][n] * g[0] + w[2][n] * g[1]) + w[3][n] * g[2];
+        }
+  }
+
   // Per RK stage (O5): fill ghosts -> prims -> sensor/div (+ghosts) -> R.
   void rhs(int parts) {
     fill_ghosts();
@@ -721,6 +744,7 @@ struct Solver {
     if (parts & PART_Y) convective(1);
     if (parts & PART_Z) convective(2);
     if ((parts & PART_VISC) && P.visc_law != VISC_NONE) viscous();
+    if (parts & PART_FORCE) body_force();
   }
 
   // ---------------------------------------------------------------------------

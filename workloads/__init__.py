@@ -56,6 +56,7 @@ class Case:
     u_ref: float = 1.0
     l_ref: float = 1.0
     freestream: tuple = (1.0, 0.0, 0.0, 0.0, 2.5)
+    accel: tuple = (0.0, 0.0, 0.0)           # uniform body acceleration (channel driving force)
     # scheme
     central_order: int = 6
     weno_order: int = 5
