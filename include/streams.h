@@ -65,6 +65,8 @@ typedef struct {
   double pow_exp;             /* power law:  mu = mu_ref t^pow_exp                              */
   double u_ref, l_ref;        /* sensor regulariser eps_s = (u_ref/l_ref)^2                     */
   double freestream[5];       /* conserved free-stream state for STREAMS_BC_FREESTREAM ghosts   */
+  double accel[3];            /* uniform body acceleration g (PAPER:377 forcing; e.g. the driving  */
+                              /* force of a channel): rho g on momentum, (rho u).g on total energy */
 } streams_gas;
 
 /* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5).

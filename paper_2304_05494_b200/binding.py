@@ -37,7 +37,8 @@ class streams_gas(C.Structure):
     _fields_ = [("gamma", C.c_double), ("rgas", C.c_double), ("prandtl", C.c_double),
                 ("visc_law", C.c_int), ("mu_ref", C.c_double), ("t_ref", C.c_double),
                 ("suth_s_over_tref", C.c_double), ("pow_exp", C.c_double),
-                ("u_ref", C.c_double), ("l_ref", C.c_double), ("freestream", C.c_double * 5)]
+                ("u_ref", C.c_double), ("l_ref", C.c_double), ("freestream", C.c_double * 5),
+                ("accel", C.c_double * 3)]
 
 
 class streams_scheme(C.Structure):
@@ -99,6 +100,8 @@ def structs_from_case(case):
         setattr(a, n, getattr(case, n))
     for q in range(5):
         a.freestream[q] = case.freestream[q]
+    for d in range(3):
+        a.accel[d] = case.accel[d]
     for n in ("central_order", "weno_order", "visc_order", "flux_mode", "sensor_threshold", "weno_eps", "cfl",
               "dt_fixed", "dt_every"):
         setattr(s, n, getattr(case, n))

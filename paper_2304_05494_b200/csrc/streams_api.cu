@@ -341,6 +341,8 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.eps_s = rr * rr;
   P.thr = scheme->sensor_threshold; P.weno_eps = scheme->weno_eps; P.cfl = scheme->cfl;
   for (int q = 0; q < 5; ++q) P.fsw[q] = gas->freestream[q];
+  for (int d = 0; d < 3; ++d) P.accel[d] = gas->accel[d];
+  P.has_accel = gas->accel[0] != 0.0 || gas->accel[1] != 0.0 || gas->accel[2] != 0.0;
   P.t_wall_lo = grid->t_wall_lo; P.t_wall_hi = grid->t_wall_hi;
   P.bc_x = grid->bc_x; P.bc_y_lo = grid->bc_y_lo; P.bc_y_hi = grid->bc_y_hi; P.bc_z = grid->bc_z;
   P.visc_law = gas->visc_law; P.flux_mode = scheme->flux_mode;

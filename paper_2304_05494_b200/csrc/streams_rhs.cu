@@ -376,6 +376,12 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
         }
       }
     }
+    if (P.has_accel) {                               // S17: uniform body acceleration and its work
+      const double rho0 = c0[F_RHO];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) r[1 + a] = fma(rho0, P.accel[a], r[1 + a]);
+      r[4] = fma(rho0, fma(c0[F_U], P.accel[0], fma(c0[F_V], P.accel[1], c0[F_W] * P.accel[2])), r[4]);
+    }
     if (active) {
       if (sa.update_w) {
         double wn[5];

@@ -166,3 +166,33 @@ def test_unsupported_order_mix_is_rejected_at_init(S):
     mixed = W.isotropic_turbulence(nx=16, ny=16, nz=16, mach_t=0.3, k0=2.0, kmax=4, seed=1).replace(weno_order=3)
     with pytest.raises(binding.StreamsError):
         S(mixed)
+
+
+# ---- uniform body acceleration (S17; PAPER:377 forcing)
+def test_body_force_periodic_hybrid(S):
+    case = W.isotropic_turbulence(nx=40, ny=38, nz=36, mach_t=0.5, k0=3.0, kmax=8, seed=51, dilatational=0.4)
+    check_case(S, case.replace(accel=(0.3, -0.2, 0.15), name="forced_box"), 10, expect_activation=(0.001, 0.8))
+
+
+def test_body_force_drives_the_channel(S):
+    case = W.channel(48, 40, 36, seed=52)
+    check_case(S, case.replace(accel=(0.02, 0.0, 0.0), name="forced_channel"), 10)
+
+
+def test_body_force_momentum_budget_with_the_library_sums(S):
+    """Inviscid periodic box: d/dt sum(rho u) = g sum(rho) exactly, so after time t the momentum integral has grown by
+    g M t and the energy integral by g . (P(0) t + g M t^2 / 2), whatever the flow does (checked with streams_get_sums)."""
+    g = np.array([0.25, 0.0, -0.1])
+    case = W.isotropic_turbulence(nx=36, ny=34, nz=32, mach_t=0.4, k0=3.0, kmax=8, seed=53, viscous=False,
+                                  dilatational=0.3).replace(accel=tuple(g), dt_fixed=2e-3)
+    gpu = S(case)
+    s0 = gpu.get_sums(0)
+    _, t = gpu.step(15)
+    s1 = gpu.get_sums(0)
+    mass = s0[0]
+    assert abs(s1[0] - mass) <= 1e-13 * mass
+    assert np.all(np.abs((s1[1:4] - s0[1:4]) - g * mass * t) <= 1e-12 * mass)
+    # RK3 integrates the quadratic-in-time energy growth exactly (third order)
+    de = float(g @ s0[1:4]) * t + 0.5 * float(g @ g) * mass * t * t
+    assert abs((s1[4] - s0[4]) - de) <= 1e-11 * abs(s0[4])
+    gpu.destroy()
