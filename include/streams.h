@@ -136,6 +136,11 @@ int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long
  * WENO forced on a chosen fraction of the points).  STREAMS_EINVAL unless flux_mode == STREAMS_FLUX_HYBRID. */
 int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int src_is_device);
 
+/* Replaces the uniform body acceleration streams_gas.accel (3 HOST doubles, copied) from the next evaluation on.
+ * With streams_get_sums(STREAMS_SUM_STATE) this is what a bulk-flow controller needs (the forcing term is
+ * re-evaluated from sum reductions every step); the controller itself is host logic (paper_2304_05494_b200/forcing.py). */
+int streams_set_body_force(streams_ctx* ctx, const double* accel3);
+
 /* Sum reductions over the interior nodes (PAPER:218-236 compute_residual; Table 2 "forcing term evaluations (sum
  * reduction)"), in a fixed order: the five doubles of out5 (HOST) are reproducible bit for bit.
  *   STREAMS_SUM_STATE:    out5[q] = sum of w_q dV, dV = dx dz / (d eta/dy)(j): the volume integrals of mass, momentum

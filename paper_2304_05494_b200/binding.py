@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
 
 STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
-           "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_get_activation", "streams_get_activation_totals",
+           "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
            "streams_last_error", "streams_destroy")
@@ -70,6 +70,7 @@ def load_library(path: str = LIB_PATH):
     lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_set_mask_override.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_sums.argtypes = [C.c_void_p, C.c_int, _dp]
+    lib.streams_set_body_force.argtypes = [C.c_void_p, _dp]
     lib.streams_get_activation.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 3
     lib.streams_get_activation_totals.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4
     lib.streams_kernel_launches.restype = C.c_longlong
@@ -216,6 +217,10 @@ class Streams:
         assert tuple(mask.shape) == self.shape
         p, dev = self._ptr(mask)
         self._check(self.lib.streams_set_mask_override(self.h, p, dev))
+
+    def set_body_force(self, accel):
+        g = (C.c_double * 3)(*[float(x) for x in accel])
+        self._check(self.lib.streams_set_body_force(self.h, g))
 
     def get_sums(self, kind=0):
         """kind 0: volume integrals of the five conserved variables; kind 1: sums of R_q^2 of the last streams_rhs."""

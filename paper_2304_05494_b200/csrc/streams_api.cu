@@ -554,6 +554,18 @@ int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int s
   return STREAMS_OK;
 }
 
+int streams_set_body_force(streams_ctx* ctx, const double* accel3) {
+  if (!ctx || !accel3) return fail(ctx, STREAMS_EINVAL, "null argument");
+  for (int d = 0; d < 3; ++d) {
+    if (!std::isfinite(accel3[d])) return fail(ctx, STREAMS_EINVAL, "accel must be finite");
+    ctx->P.accel[d] = accel3[d];
+    ctx->gas.accel[d] = accel3[d];
+  }
+  ctx->P.has_accel = accel3[0] != 0.0 || accel3[1] != 0.0 || accel3[2] != 0.0;
+  ctx->r_valid = false;                              // R no longer is the right-hand side under the new force
+  return STREAMS_OK;
+}
+
 int streams_get_sums(streams_ctx* ctx, int kind, double* out5) {
   if (!ctx || !out5) return fail(ctx, STREAMS_EINVAL, "null argument");
   if (kind != STREAMS_SUM_STATE && kind != STREAMS_SUM_RESIDUAL) return fail(ctx, STREAMS_EINVAL, "bad kind");

@@ -192,3 +192,25 @@ def test_discrete_conservation_on_the_gpu(S):
         if not viscous:
             assert np.all(drift <= 1e-12), drift
         gpu.destroy()
+
+
+def test_bulk_flow_controller_holds_the_channel_flow_rate(S):
+    """paper_2304_05494_b200.forcing: the unforced channel loses bulk momentum to wall friction; with the controller
+    (library sums + streams_set_body_force every step) it stays at its target and the force settles at the friction level."""
+    from paper_2304_05494_b200.forcing import BulkFlowController
+    case = W.channel(48, 40, 36, seed=61)
+    free = S(case)
+    p0 = free.get_sums(0)[1]
+    free.step(30)
+    loss = 1.0 - free.get_sums(0)[1] / p0
+    free.destroy()
+    assert loss > 1e-4                                   # friction is at work
+    gpu = S(case)
+    ctl = BulkFlowController(gpu)
+    ratios = []
+    for _ in range(30):
+        _, _, g, ratio = ctl.step(1)
+        ratios.append(ratio)
+    assert max(abs(r - 1.0) for r in ratios[2:]) < 0.02 * loss, (loss, ratios[-5:])
+    assert g[0] > 0.0 and g[1] == 0.0 and g[2] == 0.0
+    gpu.destroy()
