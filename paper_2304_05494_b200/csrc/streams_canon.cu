@@ -1,5 +1,6 @@
 // Kernels whose arithmetic decides an integer (the shock-sensor mask) or feeds it:
-// ghost fill + conservative->primitive, sensor/mask, interface flags, time-step reduction.
+// ghost fill + conservative->primitive (first evaluation, non-periodic ghost shell), sensor/mask, interface flags and
+// work lists; plus the one-thread step scalars, the fixed-order sum reductions and the fp64 probe.
 // This translation unit is compiled with -fmad=false so that every operation is a single
 // IEEE fp64 operation in source order: the
 // mask is then bit-identical to any IEEE evaluation of the same formulas on the same state.

@@ -1,15 +1,16 @@
-// a4-a8: the fused right-hand side + RK update.  One pass over the primitives produces, per
-// interior node, the convective terms in x, y, z (central split form, O1), the viscous
-// terms (O4) and the low-storage RK3 update (O5), so R is written once and w is updated in place
-// (stencils read the primitive copy q, never w, so no ping-pong buffer is needed).
+// a4-a8 (+ a2, a1 and a9 of the next stage): the fused right-hand side, RK update and primitives.
 //
-//   weno_kernel      : runs first.  Each block takes a chunk of interfaces of one direction, compacts the flagged
-//                      ones (hybrid: the flag bits of flags_kernel; full-WENO: all) into a block-local list and
-//                      evaluates them with full warps: WENO characteristic flux (O3) minus, in hybrid mode, the
-//                      central flux that rhs_main_kernel will use there -> dF at the left node's index.
-//   rhs_main_kernel  : every node: central scheme + viscous terms, adds -(dF_{n+1/2} - dF_{n-1/2}) metric at nodes
-//                      next to a flagged interface, then the RK update.  R and w are written once.
-// Every flagged interface is evaluated exactly once, by a warp whose lanes all do WENO work.
+//   weno_list_kernel : hybrid mode, runs first.  The flagged interfaces of each direction were compacted into work lists by
+//                      flags_kernel; persistent blocks evaluate them with full warps: WENO characteristic flux (O3) minus
+//                      the central flux that rhs_march_kernel implies there -> dF at the left node's index.
+//   weno_kernel      : full-WENO mode: every interface, the WENO flux itself.
+//   rhs_march_kernel : every node, one pass (2.5-D z-march, TMA + mbarrier pipeline): central split convective terms in
+//                      x, y, z (O1), viscous terms (O4), -(dF_{n+1/2} - dF_{n-1/2}) metric at nodes next to a
+//                      flagged interface, body force (S17), low-storage RK3 update (O5); then the primitives of the updated
+//                      node into the OTHER primitive buffer (stencils of this stage still read the current one), also at
+//                      its periodic images in the ghost layers, and in the last stage the time-step rate (a9).
+// R, w and the primitives are written once per stage; every flagged interface is evaluated exactly once, by a warp
+// whose lanes all do WENO work.
 #include "streams_dev.cuh"
 #include "streams_launch.h"
 #include "streams_tma.cuh"
