@@ -703,10 +703,12 @@ static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t 
   constexpr int TY = STREAMS_SENSOR_TY;
   using SM = SensorSmem<TY>;
   auto kern = sensor_march_kernel<L, MASK, THETA, TY>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int attr_dev = -1;                          // the opt-in is per device: redo it when the current device changes
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
-    attr_set = true;
+    attr_dev = dev;
   }
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * STREAMS_SENSOR_MINB);

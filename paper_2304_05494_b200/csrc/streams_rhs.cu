@@ -809,10 +809,12 @@ static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa,
   using G = MarchGeom<TY>;
   using SM = MarchSmem<TY, VISC, WENO>;
   auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int attr_dev = -1;                          // the opt-in is per device: redo it when the current device changes
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
-    attr_set = true;
+    attr_dev = dev;
   }
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int tiles = nbx * nby;
