@@ -26,7 +26,12 @@
 //   O4 viscous         : manufactured solution vs symbolic derivatives, zero on
 //                        uniform state, stretched-y order
 //   O5 RK3 / dt        : exp(z) Taylor polynomial, sum of coefficients, order 3
-//   O6 ghost fill      : wall at rest => R = 0 to round-off, Poiseuille balance
+//   O6 ghost fill      : wall at rest => R = 0 to round-off, Poiseuille balance, odd reflection, the
+//                        T_ghost >= 0.1 T_w clamp read back from the conserved ghosts
+//   S6 scalar ghosts   : flags next to non-periodic faces vs a clamped brute-force dilation; div ghosts at
+//                        a wall via (mu/3) grad(div) of a 1-D flow (clamped, not mirrored or wrapped)
+//   O4 power law       : mu_ref (T/T_ref)^n closed form (n = 0.5, 0.76, 1, 2; T_ref != 1) and the
+//                        manufactured Navier-Stokes terms with n = 0.76 at design order
 //   S17 body force     : uniform state => R = (0, rho g, rho u.g) exactly; momentum budget of a periodic box;
 //                        Poiseuille flow driven by g instead of a pressure gradient
 // Unpinned against the real STREAmS code (not in the container): S1, S2, S4, S5,
@@ -844,7 +849,7 @@ int oracle_get_fields(void* h, double* wout) {
         for (int i = 0; i < s->nx; ++i) wout[q * N + s->iidx(i, j, k)] = s->w[q][s->idx(i, j, k)];
   return 0;
 }
-// parts: bit0 x-convective, bit1 y, bit2 z, bit3 viscous (15 = the full RHS).
+// parts: bit0 x-convective, bit1 y, bit2 z, bit3 viscous, bit4 body force (PART_ALL = 31 = the full RHS).
 int oracle_rhs(void* h, int parts, double* rhs_out) {
   Solver* s = static_cast<Solver*>(h);
   if (!s->have_fields) return -4;
