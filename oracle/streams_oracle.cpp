@@ -144,18 +144,22 @@ double weno_reconstruct(const double* v, int r, double eps, bool linear, double*
     q[1] = (b - 5.0 * c + 13.0 * e + 3.0 * f) / 12.0;
     q[2] = (-c + 7.0 * e + 7.0 * f - g) / 12.0;
     q[3] = (3.0 * e + 13.0 * f - 5.0 * g + h) / 12.0;
-    beta[0] = (a * (547.0 * a - 3882.0 * b + 4642.0 * c - 1854.0 * e) +
-               b * (7043.0 * b - 17246.0 * c + 7042.0 * e) +
-               c * (11003.0 * c - 9402.0 * e) + 2107.0 * e * e) / 240.0;
-    beta[1] = (b * (267.0 * b - 1642.0 * c + 1602.0 * e - 494.0 * f) +
-               c * (2843.0 * c - 5966.0 * e + 1922.0 * f) +
-               e * (3443.0 * e - 2522.0 * f) + 547.0 * f * f) / 240.0;
-    beta[2] = (c * (547.0 * c - 2522.0 * e + 1922.0 * f - 494.0 * g) +
-               e * (3443.0 * e - 5966.0 * f + 1602.0 * g) +
-               f * (2843.0 * f - 1642.0 * g) + 267.0 * g * g) / 240.0;
-    beta[3] = (e * (2107.0 * e - 9402.0 * f + 7042.0 * g - 1854.0 * h) +
-               f * (11003.0 * f - 17246.0 * g + 4642.0 * h) +
-               g * (7043.0 * g - 3882.0 * h) + 547.0 * h * h) / 240.0;
+    // beta_k = sum_{m=1..3} int (d^m p_k / dx^m)^2 dx of the cubic p_k = c0 + c1 x + c2 x^2 + c3 x^3 through the four
+    // cell averages: = (c1 + c3/4)^2 + (13/3) c2^2 + (781/20) c3^2 = U^2/36 + (13/12) S^2 + (781/720) T^2 with
+    // U = 6 (c1 + c3/4), S = 2 c2, T = 6 c3 (undivided difference combinations; derived in exact rationals by
+    // tests/test_oracle_weno.py).  This is the Jiang-Shu definition written as the sum of squares it is; the
+    // expanded polynomial of Balsara & Shu (coefficients 547, -3882, ...) is the same quadratic form but loses
+    // ~8 digits to cancellation on smooth data (S8).
+    {
+      const double U0 = ((2.0 * a - 9.0 * b) + 18.0 * c) - 11.0 * e, S0 = ((a - 4.0 * b) + 5.0 * c) - 2.0 * e, T0 = ((a - 3.0 * b) + 3.0 * c) - e;
+      const double U1 = ((b - 6.0 * c) + 3.0 * e) + 2.0 * f, S1 = (c - 2.0 * e) + f, T1 = ((b - 3.0 * c) + 3.0 * e) - f;
+      const double U2 = ((2.0 * c + 3.0 * e) - 6.0 * f) + g, S2 = (c - 2.0 * e) + f, T2 = ((c - 3.0 * e) + 3.0 * f) - g;
+      const double U3 = ((11.0 * e - 18.0 * f) + 9.0 * g) - 2.0 * h, S3 = ((2.0 * e - 5.0 * f) + 4.0 * g) - h, T3 = ((e - 3.0 * f) + 3.0 * g) - h;
+      beta[0] = (U0 * U0) / 36.0 + (13.0 / 12.0) * (S0 * S0) + (781.0 / 720.0) * (T0 * T0);
+      beta[1] = (U1 * U1) / 36.0 + (13.0 / 12.0) * (S1 * S1) + (781.0 / 720.0) * (T1 * T1);
+      beta[2] = (U2 * U2) / 36.0 + (13.0 / 12.0) * (S2 * S2) + (781.0 / 720.0) * (T2 * T2);
+      beta[3] = (U3 * U3) / 36.0 + (13.0 / 12.0) * (S3 * S3) + (781.0 / 720.0) * (T3 * T3);
+    }
     d[0] = 1.0 / 35.0; d[1] = 12.0 / 35.0; d[2] = 18.0 / 35.0; d[3] = 4.0 / 35.0;
   }
   if (beta_out) for (int k = 0; k < r; ++k) beta_out[k] = beta[k];

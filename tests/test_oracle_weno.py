@@ -100,6 +100,25 @@ def test_weno_matches_exact_rational_derivation(r):
         assert abs(val - np.sum(al / al.sum() * q_ref)) < 1e-12
 
 
+@pytest.mark.parametrize("r", [3, 4])
+def test_smoothness_indicators_keep_their_digits_on_smooth_data(r):
+    """S8: beta_k from the definition, on data that varies by 1e-4 around an O(1) mean (a well-resolved wave): the
+    exact-rational value is matched to 1e-9 relative.  The expanded Balsara-Shu polynomial for r = 4 (coefficients
+    547, -3882, ...) is the same quadratic form but cancels ~8 digits here (beta ~ 1e-8 out of terms ~ 50), which
+    is what made the nonlinear weights differ at 1e-10 between two correct implementations; the oracle writes the
+    indicator as the sum of squares the definition gives."""
+    v, qs, betas, dks, full = _derive_weno(r)
+    rng = np.random.default_rng(40 + r)
+    for _ in range(5):
+        base, amp, ph = rng.uniform(0.5, 3.0), 1e-4, rng.uniform(0, 6.28)
+        vals = base + amp * np.sin(0.3 * np.arange(2 * r - 1) + ph)
+        sub = dict(zip(v, [sp.Rational(float(t)) for t in vals]))          # the doubles, exactly
+        beta_ref = np.array([float(b.subs(sub)) for b in betas])
+        _, beta = O.weno_reconstruct(vals, r)
+        assert np.all(beta_ref > 0)
+        assert np.allclose(beta, beta_ref, rtol=1e-9, atol=0.0), (beta, beta_ref)
+
+
 def test_weno5_linear_stencil_is_the_printed_one():
     """linear weights give (2,-13,47,27,-3)/60."""
     c = [O.weno_reconstruct(np.eye(5)[m], 3, linear=True)[0] for m in range(5)]
