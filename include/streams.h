@@ -19,7 +19,8 @@
  *     = [5][nz][ny][nx] (conserved rho, rho u, rho v, rho w, rho E) or [nz][ny][nx].
  *   - Every pointer argument says whether it is HOST or DEVICE memory.
  *   - The caller owns the workspace and the CUDA stream and keeps both alive until
- *     streams_destroy.  The library never allocates device memory itself.
+ *     streams_destroy.  The library never allocates device memory itself (the fp64 probe
+ *     streams_measure_fp64 takes its scratch buffer from the caller as well).
  *   - Host arrays passed in (y_nodes, the structs) are copied before the call returns.
  *   - Calls enqueue work on the caller's stream.  Calls that return host scalars or
  *     copy to host memory synchronise that stream before returning.
@@ -69,10 +70,13 @@ typedef struct {
                               /* force of a channel): rho g on momentum, (rho u).g on total energy */
 } streams_gas;
 
-/* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5).
- * This build instantiates the families m = 1, 2, 3: central order 2m with WENO order 2m-1 and viscous order 2m
- * (2/1/2, 4/3/4, 6/5/6); an order the chosen mode does not use is ignored; any other combination makes
- * streams_workspace_bytes return 0 and streams_init return STREAMS_EINVAL (never later). */
+/* Scheme (PAPER:38 orders "up to 8th and 7th"; production pair 6/5; the paper's order sweep runs the
+ * families 2/1/2, 4/3/4, 6/5/6, 8/7/8).  Every combination of central order 2..8, WENO order 1..7 and
+ * viscous order 2..8 is accepted; an order the chosen mode does not use is ignored.  The four families above are
+ * template instances of their own; a mixed combination runs on the smallest instance that covers it with zero-padded
+ * coefficient tables (same numbers, the speed of the covering instance).  The layout carries three ghost layers, four
+ * when an order reaches further (central / viscous 8, WENO 7).  Invalid orders make streams_workspace_bytes return 0
+ * and streams_init return STREAMS_EINVAL (never later). */
 typedef struct {
   int central_order;          /* 2L: 2, 4, 6, 8                                                 */
   int weno_order;             /* 2r-1: 1, 3, 5, 7; ignored when flux_mode == CENTRAL            */
@@ -106,7 +110,9 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device);
 int streams_rhs(streams_ctx* ctx, double* rhs_out_dev);
 
 /* nsteps full RK3 steps (3 RHS + 3 updates each, dt per scheme).  dt_last, time: HOST, nullable.
- * Returns STREAMS_ENAN if the time step or the state became non-finite. */
+ * Returns STREAMS_ENAN if the time step or the state became non-finite: the last stage of every step checks the
+ * updated state for Inf / NaN, and the time-step rate of every node keeps a NaN (a negative pressure); the error
+ * is reported when the call returns (the remaining steps of the call still run). */
 int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time);
 
 /* Copy the conserved state out, w_out[5][nz][ny][nx].  dst_is_device: 0 = HOST, 1 = DEVICE. */
@@ -158,7 +164,7 @@ long long streams_kernel_launches(const streams_ctx* ctx);
 /* Per-kernel device timing, the measurement of BASELINE metric part 2 ("per-kernel % of roofline";
  * the paper's analogue is its per-kernel table).  Kernel classes: */
 enum { STREAMS_K_FILL_PRIM = 0, STREAMS_K_DT = 1, STREAMS_K_SENSOR = 2, STREAMS_K_FLAGS = 3,
-       STREAMS_K_RHS_MAIN = 4, STREAMS_K_WENO = 5, STREAMS_K_APPLY = 6, STREAMS_K_MISC = 7,
+       STREAMS_K_RHS_MAIN = 4, STREAMS_K_WENO = 5, STREAMS_K_CORR = 6, STREAMS_K_MISC = 7,
        STREAMS_K_COUNT = 8 };
 
 /* enable != 0: from now on every launch is bracketed by a CUDA event pair on the context's stream
@@ -175,9 +181,13 @@ int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long lon
 /* Measures the fp64 pipe of the current device, the "alu" roof of SURVEY 8(d): kind 0 = independent DFMA chains,
  * kind 1 = DADD and DMUL alternating.  *ginst_per_s (HOST) receives thread-level fp64 instructions per second in
  * units of 1e9, the best of `repeats` launches timed with CUDA events on `cuda_stream` (each launch runs
- * 8 x 256-thread blocks per SM, 16 chains per thread).  Needs no context and no workspace; synchronises the stream.
- * Returns STREAMS_EINVAL for a bad kind / null output, STREAMS_ECUDA on a CUDA error. */
-int streams_measure_fp64(void* cuda_stream, int kind, int repeats, double* ginst_per_s);
+ * 8 x 256-thread blocks per SM, 16 chains per thread).  scratch_dev: DEVICE buffer of at least
+ * streams_measure_fp64_scratch_bytes() bytes, owned by the caller (the probe stores one double per thread there).
+ * Needs no context; synchronises the stream.  Returns STREAMS_EINVAL for a bad kind / null output, STREAMS_ENOMEM for
+ * a missing or short scratch buffer, STREAMS_ECUDA on a CUDA error. */
+size_t streams_measure_fp64_scratch_bytes(void);
+int streams_measure_fp64(void* cuda_stream, int kind, int repeats, void* scratch_dev, size_t scratch_bytes,
+                         double* ginst_per_s);
 
 /* Name of a kernel class ("" if out of range); static storage. */
 const char* streams_kernel_name(int kind);

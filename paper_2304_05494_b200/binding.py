@@ -19,6 +19,7 @@ EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "str
            "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
+           "streams_measure_fp64_scratch_bytes",
            "streams_last_error", "streams_destroy")
 STREAMS_K_COUNT = 8
 
@@ -77,7 +78,9 @@ def load_library(path: str = LIB_PATH):
     lib.streams_kernel_launches.argtypes = [C.c_void_p]
     lib.streams_profile.argtypes = [C.c_void_p, C.c_int, C.c_int]
     lib.streams_get_profile.argtypes = [C.c_void_p, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
-    lib.streams_measure_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
+    lib.streams_measure_fp64_scratch_bytes.restype = C.c_size_t
+    lib.streams_measure_fp64_scratch_bytes.argtypes = []
+    lib.streams_measure_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, _dp]
     lib.streams_kernel_name.restype = C.c_char_p
     lib.streams_kernel_name.argtypes = [C.c_int]
     lib.streams_last_error.restype = C.c_char_p
@@ -118,7 +121,10 @@ def measure_fp64(kind: int = 0, repeats: int = 5, stream=None) -> float:
     lib = load_library()
     st = stream if stream is not None else torch.cuda.current_stream()
     out = C.c_double()
-    rc = lib.streams_measure_fp64(C.c_void_p(st.cuda_stream), int(kind), int(repeats), C.byref(out))
+    nbytes = lib.streams_measure_fp64_scratch_bytes()
+    scratch = torch.empty(max(nbytes, 8), dtype=torch.uint8, device="cuda")
+    rc = lib.streams_measure_fp64(C.c_void_p(st.cuda_stream), int(kind), int(repeats), C.c_void_p(scratch.data_ptr()),
+                                  C.c_size_t(nbytes), C.byref(out))
     if rc != STREAMS_OK:
         raise StreamsError(rc, lib.streams_last_error(None).decode())
     return out.value

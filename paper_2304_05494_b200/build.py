@@ -4,6 +4,7 @@
 
 streams_canon.cu is compiled with -fmad=false (canonical, contraction-free evaluation of the
 sensor path); the other translation units use the default FMA contraction.
+The translation units compile in parallel (the two heavy ones, streams_march.cu and streams_weno.cu, first).
 """
 from __future__ import annotations
 
@@ -17,7 +18,8 @@ OUT = os.path.join(HERE, "lib")
 LIB = os.path.join(OUT, "libstreams.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", *ARCH]
-UNITS = [("streams_canon.cu", ["-fmad=false"]), ("streams_rhs.cu", []), ("streams_api.cu", [])]
+UNITS = [("streams_march.cu", []), ("streams_weno.cu", []), ("streams_canon.cu", ["-fmad=false"]), ("streams_fill.cu", []),
+         ("streams_api.cu", [])]
 
 
 def _newest_source() -> float:

@@ -23,7 +23,7 @@ struct Sizes {
   int L, Lv, r, ng, ox, px, py, pz;
   size_t fs;            // doubles per padded field
   size_t N, lcap;
-  size_t off_w, off_q, off_q2, off_theta, off_mask, off_movr, off_nflag, off_ilist, off_dF, off_counters, off_R,
+  size_t off_w, off_q, off_q2, off_theta, off_mask, off_movr, off_nflag, off_ilist, off_dF, off_corr, off_counters, off_R,
       off_metrics, off_scal, off_sums, total;
   int nq;
 };
@@ -49,7 +49,7 @@ bool valid_bc(int b) { return b == STREAMS_BC_PERIODIC || b == STREAMS_BC_WALL_I
 const char* plan(const streams_grid* g, const streams_gas* gas, const streams_scheme* sc, Sizes& S) {
   if (!g || !gas || !sc) return "null argument";
   if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid extents must be positive";
-  if (((long long)g->nx + 40) * ((long long)g->ny + 8) * ((long long)g->nz + 8) > 2000000000LL)
+  if (((long long)g->nx + 48) * ((long long)g->ny + 8) * ((long long)g->nz + 8) > 2000000000LL)
     return "grid too large for 32-bit node indices";
   if (!(g->lx > 0) || !(g->lz > 0)) return "lx, lz must be positive";
   if (!valid_bc(g->bc_x) || !valid_bc(g->bc_y_lo) || !valid_bc(g->bc_y_hi) || !valid_bc(g->bc_z)) return "bad bc code";
@@ -71,10 +71,10 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   S.L = sc->central_order / 2;
   S.Lv = gas->visc_law == STREAMS_VISC_NONE ? 0 : sc->visc_order / 2;
   S.r = sc->flux_mode == STREAMS_FLUX_CENTRAL ? 0 : (sc->weno_order + 1) / 2;
-  if (!rhs_supported(S.L, S.Lv, S.r, sc->flux_mode, gas->visc_law))
-    return "this build instantiates the order families 2/1/2, 4/3/4 and 6/5/6 (central / WENO / viscous) only";
-  S.ng = 3;                                               // the layout and the tiles always carry three ghost layers
+  // three ghost layers, four when an order of the scheme reaches further (central / viscous 8, WENO 7)
+  S.ng = std::max(3, std::max(S.L, std::max(S.Lv, S.r)));
   if (g->nx < S.ng || g->ny < S.ng || g->nz < S.ng) return "each extent must be at least the ghost width";
+  if (g->ny + 2 * S.ng > 65535 || g->nz + 2 * S.ng > 65535) return "ny and nz (with ghosts) must not exceed 65535";
   S.ox = 16;                                              // interior i = 0 starts a 128-byte line
   S.px = (int)align_up((size_t)S.ox + g->nx + S.ng, 16);
   S.py = g->ny + 2 * S.ng;
@@ -98,6 +98,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
     S.off_ilist = take(hyb ? 3 * S.lcap * 4 : 256);
   }
   S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
+  S.off_corr = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 5 * S.fs * 8 : 256);
   S.off_counters = take(C_COUNT * 4);
   S.off_R = take(5 * S.fs * 8);
   S.off_metrics = take(3 * (size_t)g->ny * 8);
@@ -204,7 +205,7 @@ int timed(streams_ctx* ctx, int kind, F&& launch) {
   if (ctx->prof_on && !rec) ctx->prof_dropped += 1;
   if (rec) cudaEventRecord(ctx->prof_pool[2 * ctx->prof_used], ctx->stream);
   const int n = launch();
-  if (rec) {
+  if (rec && n > 0) {                                 // a wrapper that launched nothing leaves no record
     cudaEventRecord(ctx->prof_pool[2 * ctx->prof_used + 1], ctx->stream);
     ctx->prof_kind[ctx->prof_used] = kind;
     ctx->prof_used += 1;
@@ -237,17 +238,25 @@ int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta, bool step_start 
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
   const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0) && !ctx->rate_ready;
-  if (ctx->prims_interior && !reduce_dt) timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
-  else timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
+  int rc = 0;
+  auto run = [&](int kind, auto&& launch) { const int n = timed(ctx, kind, launch); if (n < 0 && rc == 0) rc = n; };
+  if (ctx->prims_interior && !reduce_dt) run(STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
+  else run(STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
   ctx->prims_interior = true;
-  if (step_start) timed(ctx, STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, want_dt, st); });
+  if (step_start) run(STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, want_dt, st); });
   if (want_dt) ctx->rate_ready = false;             // dt_finalize consumed (and zeroed) the rate
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
   if (hyb || visc || theta)
-    timed(ctx, STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps[ctx->cur], ctx->S.L, hyb || theta, theta, st); });
-  if (hyb) timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.L, ctx->S.r, st); });
-  return STREAMS_OK;
+    run(STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps[ctx->cur], ctx->S.L, hyb || theta, theta, st, false); });
+  if (hyb) run(STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.r, st); });
+  return rc;
+}
+
+// error of a negative launch code (streams_launch.h)
+int launch_fail(streams_ctx* ctx, int rc) {
+  if (rc == -2) return fail(ctx, STREAMS_ECUDA, "cudaFuncSetAttribute: cannot opt a kernel in to its dynamic shared memory");
+  return fail(ctx, STREAMS_EINVAL, "order combination outside the instantiated kernels");
 }
 
 // points DevP::q / div at primitive buffer b
@@ -262,11 +271,13 @@ void use_qbuf(streams_ctx* ctx, int b) {
 int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
-  int b = 0;
-  if (ctx->scheme.flux_mode != STREAMS_FLUX_CENTRAL)
-    b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.Lv, ctx->S.r, st); });
-  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps[ctx->cur], ctx->S.L, ctx->S.Lv, ctx->S.r, sa, st); });
-  return (a < 0 || b < 0) ? -1 : a + b;
+  int b = 0, c = 0;
+  if (ctx->scheme.flux_mode != STREAMS_FLUX_CENTRAL) {
+    b = timed(ctx, STREAMS_K_WENO, [&] { return launch_weno(P, ctx->S.L, ctx->S.r, st); });
+    c = timed(ctx, STREAMS_K_CORR, [&] { return launch_corr(P, st); });
+  }
+  const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps[ctx->cur], ctx->S.L, ctx->S.Lv, sa, st, false); });
+  return a < 0 ? a : (b < 0 ? b : (c < 0 ? c : a + b + c));
 }
 
 }  // namespace
@@ -317,6 +328,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.ilist = (int*)(ctx->base + S.off_ilist);
   P.lcap = (long long)S.lcap;
   P.dF = (double*)(ctx->base + S.off_dF);
+  P.corr = (double*)(ctx->base + S.off_corr);
   P.counters = (int*)(ctx->base + S.off_counters);
   P.R = (double*)(ctx->base + S.off_R);
   double* met = (double*)(ctx->base + S.off_metrics);
@@ -370,6 +382,19 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   if (maps_rc != 0) {
     delete ctx;
     return fail(nullptr, STREAMS_ECUDA, "cannot build the TMA descriptors (cuTensorMapEncodeTiled)");
+  }
+
+  {
+    // opt the z-marching kernels this context launches in to their dynamic shared memory on this device, once
+    StageArgs sa0{};
+    int rc = launch_rhs_main(P, ctx->maps[0], S.L, S.Lv, sa0, ctx->stream, true);
+    if (rc == 0)                                     // (streams_get_sensor may run the sensor in any mode)
+      rc = launch_sensor(P, ctx->maps[0], S.L, true, true, ctx->stream, true);
+    if (rc != 0) {
+      delete ctx;
+      return rc == -2 ? fail(nullptr, STREAMS_ECUDA, "cudaFuncSetAttribute: cannot opt a kernel in to its dynamic shared memory")
+                      : fail(nullptr, STREAMS_EINVAL, "order combination outside the instantiated kernels");
+    }
   }
 
   std::vector<double> eyc, eyv, eyyv;
@@ -435,11 +460,12 @@ int streams_get_fields(streams_ctx* ctx, double* w_out, int dst_is_device) {
 int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
   if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_rhs before streams_set_fields");
-  enqueue_prepare(ctx, false, false);
+  int rc = enqueue_prepare(ctx, false, false);
+  if (rc < 0) return launch_fail(ctx, rc);
   StageArgs sa;
   sa.gam = 0.0; sa.rhk = 0.0; sa.update_w = 0; sa.read_prev = 0; sa.write_r = 1;
-  sa.r_dense = rhs_out_dev; sa.q_out = nullptr; sa.want_rate = 0;
-  if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
+  sa.r_dense = rhs_out_dev; sa.q_out = nullptr; sa.want_rate = 0; sa.check_state = 0;
+  if ((rc = enqueue_rhs(ctx, sa)) < 0) return launch_fail(ctx, rc);
   CU(cudaGetLastError());
   ctx->r_valid = true;
   return STREAMS_OK;
@@ -456,14 +482,16 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
   for (int s = 0; s < nsteps; ++s) {
     const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
     for (int l = 0; l < 3; ++l) {
-      enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
+      int rc = enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
+      if (rc < 0) return launch_fail(ctx, rc);
       StageArgs sa;
       sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
       sa.r_dense = nullptr;
       sa.q_out = ctx->qbuf[ctx->cur ^ 1];
       // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
       sa.want_rate = (l == 2 && !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0) ? 1 : 0;
-      if (enqueue_rhs(ctx, sa) < 0) return fail(ctx, STREAMS_EINVAL, "unsupported order combination");
+      sa.check_state = (l == 2);
+      if ((rc = enqueue_rhs(ctx, sa)) < 0) return launch_fail(ctx, rc);
       use_qbuf(ctx, ctx->cur ^ 1);                   // the updated state's primitives are in the other buffer
       ctx->prims_interior = true;
       if (sa.want_rate) ctx->rate_ready = true;
@@ -476,8 +504,8 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
   CU(cudaStreamSynchronize(ctx->stream));
   if (dt_last) *dt_last = h[S_DT];
   if (time) *time = h[S_TIME];
-  if (h[S_NAN] != 0.0 || !std::isfinite(h[S_DT]) || !std::isfinite(h[S_TIME]))
-    return fail(ctx, STREAMS_ENAN, "non-finite time step");
+  if (h[S_NAN] != 0.0 || !std::isfinite(h[S_DT]) || !std::isfinite(h[S_TIME]) || !std::isfinite(h[S_RATE]))
+    return fail(ctx, STREAMS_ENAN, "the state or the time step became non-finite");
   return STREAMS_OK;
 }
 
@@ -485,7 +513,8 @@ int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
   if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
   const DevP& P = ctx->P;
-  enqueue_prepare(ctx, false, true);
+  const int prc = enqueue_prepare(ctx, false, true);
+  if (prc < 0) return launch_fail(ctx, prc);
   CU(cudaGetLastError());
   const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
   if (theta_out) CU(cudaMemcpyAsync(theta_out, P.theta, (size_t)P.N * 8, kind, ctx->stream));
@@ -612,16 +641,19 @@ int streams_get_profile(streams_ctx* ctx, double* ms, long long* count, long lon
   return STREAMS_OK;
 }
 
-int streams_measure_fp64(void* cuda_stream, int kind, int repeats, double* ginst_per_s) {
+size_t streams_measure_fp64_scratch_bytes(void) { return measure_fp64_scratch_bytes(); }
+
+int streams_measure_fp64(void* cuda_stream, int kind, int repeats, void* scratch_dev, size_t scratch_bytes, double* ginst_per_s) {
   if (!ginst_per_s || kind < 0 || kind > 1) return fail(nullptr, STREAMS_EINVAL, "streams_measure_fp64: bad argument");
-  const double v = measure_fp64((cudaStream_t)cuda_stream, kind, repeats < 1 ? 1 : repeats);
+  const double v = measure_fp64((cudaStream_t)cuda_stream, kind, repeats < 1 ? 1 : repeats, (double*)scratch_dev, scratch_bytes);
+  if (v == -2.0) return fail(nullptr, STREAMS_ENOMEM, "streams_measure_fp64: scratch buffer missing or too small");
   if (v < 0.0) return fail(nullptr, STREAMS_ECUDA, "streams_measure_fp64: CUDA error");
   *ginst_per_s = v * 1e-9;
   return STREAMS_OK;
 }
 
 const char* streams_kernel_name(int kind) {
-  static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "weno", "rhs_apply", "misc"};
+  static const char* names[STREAMS_K_COUNT] = {"fill_prim", "dt", "sensor", "flags", "rhs_main", "weno", "corr_gather", "misc"};
   return (kind >= 0 && kind < STREAMS_K_COUNT) ? names[kind] : "";
 }
 

@@ -1,6 +1,5 @@
-// Kernels whose arithmetic decides an integer (the shock-sensor mask) or feeds it:
-// ghost fill + conservative->primitive (first evaluation, non-periodic ghost shell), sensor/mask, interface flags and
-// work lists; plus the one-thread step scalars, the fixed-order sum reductions and the fp64 probe.
+// Kernels whose arithmetic decides an integer (the shock-sensor mask): sensor/mask, interface flags and work lists;
+// plus the one-thread step scalars, the fixed-order sum reductions and the fp64 probe.
 // This translation unit is compiled with -fmad=false so that every operation is a single
 // IEEE fp64 operation in source order: the
 // mask is then bit-identical to any IEEE evaluation of the same formulas on the same state.
@@ -11,141 +10,10 @@
 namespace streams {
 
 // ---------------------------------------------------------------------------------------------
-// a1 + a2: ghost / boundary fill and conservative -> primitive in one pass over the padded box.
-// Each padded node finds the interior node it images (periodic wrap, wall mirror) or takes the
-// free-stream state, rebuilds the conserved ghost state (isothermal no-slip wall: u -> -u,
-// T -> 2 T_w - T, p -> p, rho = p/(R T); O6) and then the primitives.
-// HBM: 40 B read (interior) + 8 B x (#primitive fields) write per padded node.
-// ---------------------------------------------------------------------------------------------
-// With DT the same pass takes the time-step rate of every interior node (a9) and reduces it (block_rate_max).
-// fill_node: one padded node (i, j, k in interior coordinates, ghosts negative or beyond the extents).
-template <bool VISC, bool STORE_C, bool DT>
-__device__ __forceinline__ double fill_node(const DevP& P, int i, int j, int k) {
-  int is = i, js = j, ks = k;
-  bool fsx = false, fsy = false, fsz = false;
-  double t_wall = 0.0;
-  bool wall = false;
-  if (i < 0) { if (P.bc_x == BC_PERIODIC) is = i + P.nx; else { fsx = true; is = 0; } }
-  else if (i >= P.nx) { if (P.bc_x == BC_PERIODIC) is = i - P.nx; else { fsx = true; is = P.nx - 1; } }
-  if (j < 0) {
-    if (P.bc_y_lo == BC_PERIODIC) js = j + P.ny;
-    else if (P.bc_y_lo == BC_WALL) { js = -1 - j; wall = true; t_wall = P.t_wall_lo; }
-    else { fsy = true; js = 0; }
-  } else if (j >= P.ny) {
-    if (P.bc_y_hi == BC_PERIODIC) js = j - P.ny;
-    else if (P.bc_y_hi == BC_WALL) { js = 2 * P.ny - 1 - j; wall = true; t_wall = P.t_wall_hi; }
-    else { fsy = true; js = P.ny - 1; }
-  }
-  if (k < 0) { if (P.bc_z == BC_PERIODIC) ks = k + P.nz; else { fsz = true; ks = 0; } }
-  else if (k >= P.nz) { if (P.bc_z == BC_PERIODIC) ks = k - P.nz; else { fsz = true; ks = P.nz - 1; } }
-
-  const long long ns = pidx(P, is, js, ks);
-  double s[5];
-#pragma unroll
-  for (int q = 0; q < 5; ++q) s[q] = P.w[q * P.fs + ns];
-  if (fsx) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
-  }
-  if (fsy) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
-  } else if (wall) {
-    const double rho = s[0];
-    const double uu = s[1] / rho, vv = s[2] / rho, wv = s[3] / rho;
-    const double ke = 0.5 * ((uu * uu + vv * vv) + wv * wv);
-    const double pp = P.gm1 * (s[4] - rho * ke);
-    const double TT = pp / (rho * P.rgas);
-    double Tg = 2.0 * t_wall - TT;
-    const double Tmin = 0.1 * t_wall;
-    if (Tg < Tmin) Tg = Tmin;
-    const double rg = pp / (P.rgas * Tg);
-    s[0] = rg;
-    s[1] = -(rg * uu);
-    s[2] = -(rg * vv);
-    s[3] = -(rg * wv);
-    s[4] = pp / P.gm1 + rg * ke;
-  }
-  if (fsz) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) s[q] = P.fsw[q];
-  }
-  const long long n = pidx(P, i, j, k);
-  const bool ghost = (is != i) || (js != j) || (ks != k) || fsx || fsy || fsz;
-  if (ghost) {
-#pragma unroll
-    for (int q = 0; q < 5; ++q) P.w[q * P.fs + n] = s[q];
-  }
-  double mu, cc, vel[3], o[NQ];
-  prims_from_state<VISC, STORE_C>(P, s, DT, o, mu, cc, vel);
-  store_prims<VISC, STORE_C>(P, P.q + n, o);
-  double rmax = 0.0;
-  if (DT && !ghost) rmax = dt_rate<VISC>(P, vel, cc, mu, s[0], P.eta_y_c[j]);
-  return rmax;
-}
-
-template <bool VISC, bool STORE_C, bool DT>
-__global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
-  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-  const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
-  double rmax = 0.0;
-  if (i >= -P.ng && i < P.nx + P.ng) rmax = fill_node<VISC, STORE_C, DT>(P, i, j, k);
-  if (DT) {
-    __shared__ unsigned long long sm[4];
-    block_rate_max(P, rmax, sm);
-  }
-}
-
-// The ghost shell only (every stage but the first after streams_set_fields: the fused RHS kernel has already
-// written the primitives of the updated interior nodes and of their periodic images, DevP::own_*).  Up to three
-// segments of a flat index (directions the RHS kernel owns are skipped): the z slabs (whole padded
-// planes), the y slabs of the interior planes, the x columns of the interior rows.
-template <bool VISC, bool STORE_C>
-__global__ void __launch_bounds__(128) fill_ghost_kernel(const DevP P) {
-  const int g = P.ng, wx = P.nx + 2 * g;
-  const long long nZ = P.own_z ? 0 : 2LL * g * P.py * wx, nY = P.own_y ? 0 : (long long)P.nz * 2 * g * wx,
-                  nX = P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  int i, j, k;
-  if (t < nZ) {
-    i = (int)(t % wx) - g;
-    const long long t2 = t / wx;
-    j = (int)(t2 % P.py) - g;
-    const int m = (int)(t2 / P.py);
-    k = m < g ? m - g : P.nz + (m - g);
-  } else if ((t -= nZ) < nY) {
-    i = (int)(t % wx) - g;
-    const long long t2 = t / wx;
-    const int m = (int)(t2 % (2 * g));
-    k = (int)(t2 / (2 * g));
-    j = m < g ? m - g : P.ny + (m - g);
-  } else if ((t -= nY) < nX) {
-    const int m = (int)(t % (2 * g));
-    const long long t2 = t / (2 * g);
-    j = (int)(t2 % P.ny);
-    k = (int)(t2 / P.ny);
-    i = m < g ? m - g : P.nx + (m - g);
-  } else {
-    return;
-  }
-  fill_node<VISC, STORE_C, false>(P, i, j, k);
-}
-
-// ---------------------------------------------------------------------------------------------
-// a3: Ducros-type sensor, node mask and dilatation (O2).  One thread per interior node.
+// a3: Ducros-type sensor, node mask and dilatation (O2): sensor_march_kernel below.
 // Canonical order: delta_l = f(+l) - f(-l); acc = a_1 delta_1; acc = acc + a_l delta_l; d = acc * metric;
 // div = (u_x + v_y) + w_z; s = (((div^2 + ox^2) + oy^2) + oz^2) + eps_s; theta = max(-div/sqrt(s), 0).
-// The face ghosts of div / mask are filled by scalar_ghost_kernel right after.
-// HBM: 24 B read + 8 B (div) + 1 B (mask) write per node.
 // ---------------------------------------------------------------------------------------------
-template <int L>
-__device__ __forceinline__ double ddc(const DevP& P, const double* __restrict__ f, long long n, long long s, double metric) {
-  double acc = P.a1[0] * (f[n + s] - f[n - s]);
-#pragma unroll
-  for (int l = 2; l <= L; ++l) acc = acc + P.a1[l - 1] * (f[n + l * s] - f[n - l * s]);
-  return acc * metric;
-}
-
 // Face ghosts of the nodal scalars div and mask (S6): periodic wrap, else constant extrapolation of the
 // nearest interior value.  One thread per face-ghost node (edges and corners are never read: every
 // consumer is a star stencil).  Segments of the flat index: x faces, y faces, z faces.
@@ -184,36 +52,6 @@ __global__ void __launch_bounds__(256) scalar_ghost_kernel(const DevP P) {
   if (MASK) P.mask[n] = P.mask[ns];
 }
 
-template <int L, bool MASK, bool THETA>
-__global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  if (i >= P.nx || j >= P.ny) return;
-  const long long n = pidx(P, i, j, k);
-  const double* __restrict__ u = P.q + Q_U * P.fs;
-  const double* __restrict__ v = P.q + Q_V * P.fs;
-  const double* __restrict__ w = P.q + Q_W * P.fs;
-  const double my = P.eta_y_c[j];
-  const double ux = ddc<L>(P, u, n, 1, P.inv_dx), uy = ddc<L>(P, u, n, P.sy, my), uz = ddc<L>(P, u, n, P.sz, P.inv_dz);
-  const double vx = ddc<L>(P, v, n, 1, P.inv_dx), vy = ddc<L>(P, v, n, P.sy, my), vz = ddc<L>(P, v, n, P.sz, P.inv_dz);
-  const double wx = ddc<L>(P, w, n, 1, P.inv_dx), wy = ddc<L>(P, w, n, P.sy, my), wz = ddc<L>(P, w, n, P.sz, P.inv_dz);
-  const double dv = (ux + vy) + wz;
-  P.div[n] = dv;
-  if (MASK || THETA) {
-    const double ox = wy - vz, oy = uz - wx, oz = vx - uy;
-    const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
-    double th = -dv / sqrt(s);
-    if (!(th > 0.0)) th = 0.0;
-    if (THETA) P.theta[iidx(P, i, j, k)] = th;
-    if (MASK) {
-      unsigned char m = (th > P.thr) ? 1 : 0;
-      if (P.mask_ovr) m = P.mask_ovr[n];
-      P.mask[n] = m;
-    }
-  }
-}
-
 // ---------------------------------------------------------------------------------------------
 // sensor_march_kernel: the same sensor (identical operations in identical order, so identical bits) as a
 // z-marching kernel like rhs_march_kernel (streams_rhs.cu): a block owns a 32 x TY tile and a chunk of z
@@ -221,9 +59,9 @@ __global__ void __launch_bounds__(256) sensor_kernel(const DevP P) {
 // planes ahead), the z neighbours live in a 7-plane register ring fed by a second TMA box per plane.
 // HBM: 24 B read + 8 B (div) + 1 B (mask) write per node; every stencil offset is an immediate.
 // ---------------------------------------------------------------------------------------------
-template <int TY>
+template <int TY, int NG>
 struct SensorSmem {
-  using G = MarchGeom<TY>;
+  using G = MarchGeom<TY, NG>;
   static constexpr size_t BUF = (size_t)3 * G::PLANE * 8, RING = (size_t)3 * G::NT * 8;
   static constexpr size_t OFF_RING = 2 * BUF, OFF_BAR = OFF_RING + 2 * RING, TOTAL = OFF_BAR + 64;
   static_assert(BUF % 128 == 0 && RING % 128 == 0, "TMA destinations are 128-byte aligned");
@@ -241,13 +79,12 @@ __device__ __forceinline__ double ddc_g(const DevP& P, const G& g, double metric
 #ifndef STREAMS_SENSOR_MINB
 #define STREAMS_SENSOR_MINB 3
 #endif
-template <int L, bool MASK, bool THETA, int TY>
+template <int L, bool MASK, bool THETA, int TY, int NG>
 __global__ void __launch_bounds__(MTX * TY, STREAMS_SENSOR_MINB)
 sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring, const DevP P,
                     int nbx, int nby, int kz) {
-  using G = MarchGeom<TY>;
-  using SM = SensorSmem<TY>;
-  constexpr int NG = 3;                    // ghost width / ring depth of the layout; the stencil uses L <= NG of it
+  using G = MarchGeom<TY, NG>;             // NG = DevP::ng: ghost width / ring depth of the layout
+  using SM = SensorSmem<TY, NG>;
   static_assert(L <= NG, "ring depth");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][3][PLANE]
@@ -266,19 +103,19 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
   if (kb >= ke) return;
   const int i = i0 + tx, j = j0 + ty;
   const bool active = i < P.nx && j < P.ny;
-  const int ic = min(i, P.nx + P.ng - 1), jc = min(j, P.ny + P.ng - 1);
+  const int ic = min(i, P.nx + NG - 1), jc = min(j, P.ny + NG - 1);
   const int isz = (int)P.sz;
   const int ncol = (int)pidx(P, ic, jc, 0);
-  const int s0 = (ty + 3) * G::ROW + tx + 4;
-  const int cx0 = i0 + P.ox, cy0 = j0 + P.ng;
+  const int s0 = (ty + NG) * G::ROW + tx + 4;
+  const int cx0 = i0 + P.ox, cy0 = j0 + NG;
 
   auto issue_centre = [&](int k, int b) {
     mbar_expect_tx(&full_c[b], (unsigned)SM::BUF);
-    tma_load_4d(buf + (size_t)b * 3 * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - 3, k + P.ng, 0);
+    tma_load_4d(buf + (size_t)b * 3 * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
   };
-  auto issue_ring = [&](int k, int b) {              // ring plane k+4 into slot b
+  auto issue_ring = [&](int k, int b) {              // ring plane k+NG+1 into slot b
     mbar_expect_tx(&full_r[b], (unsigned)SM::RING);
-    tma_load_4d(ring + (size_t)b * 3 * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + 1 + P.ng, 0);
+    tma_load_4d(ring + (size_t)b * 3 * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + 1 + NG, 0);
   };
   if (MASK && tid == 0 && blockIdx.x == 0 && P.flux_mode == FLUX_HYBRID) {
     // per-evaluation counters of flags_kernel (which runs after this kernel; their last readers ran before it)
@@ -535,13 +372,6 @@ __global__ void dt_finalize_kernel(const DevP P, double dt_fixed, int recompute)
   P.scal[S_NSTEP] = P.scal[S_NSTEP] + 1.0;
 }
 
-__global__ void reset_counters_kernel(const DevP P) {
-  P.counters[C_NSHOCK] = 0;
-  P.counters[C_NFLAGGED] = 0;
-  P.counters[C_NIFACE] = 0; P.counters[C_NIFACE + 1] = 0; P.counters[C_NIFACE + 2] = 0;
-  reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[2] += 1ull;   // sensor evaluations since set_fields
-}
-
 // ---------------------------------------------------------------------------------------------
 // fp64 pipe probe (streams_measure_fp64): 16 independent chains per thread, ITERS trips; KIND 0 chains are
 // x = fma(x, a, b), KIND 1 alternate x = x + b and x = x * a (this unit is built without contraction, so they
@@ -566,20 +396,27 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double* out, double a, 
 }
 
 // Returns thread-level fp64 instructions per second (best of `repeats`), or a negative value on a CUDA error.
-double measure_fp64(cudaStream_t st, int kind, int repeats) {
+// scratch: caller's device buffer of measure_fp64_scratch_bytes() (the library allocates no device memory).
+size_t measure_fp64_scratch_bytes() {
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return 0;
+  return (size_t)nsm * 8 * 256 * sizeof(double);
+}
+double measure_fp64(cudaStream_t st, int kind, int repeats, double* scratch, size_t scratch_bytes) {
   int dev = 0, nsm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
     return -1.0;
   const int blocks = nsm * 8, threads = 256, iters = 4096;
-  double* out = nullptr;
-  if (cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)) != cudaSuccess) return -1.0;   // probe only: not a hot path
+  if (!scratch || scratch_bytes < (size_t)blocks * threads * sizeof(double)) return -2.0;
   cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  if (cudaEventCreate(&e0) != cudaSuccess) return -1.0;
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return -1.0; }
   double best = -1.0;
   for (int r = 0; r < repeats + 1; ++r) {            // the first launch warms up
     cudaEventRecord(e0, st);
-    if (kind == 0) fp64_probe_kernel<0><<<blocks, threads, 0, st>>>(out, 0.999999, 1e-6, iters);
-    else fp64_probe_kernel<1><<<blocks, threads, 0, st>>>(out, 0.999999, 1e-6, iters);
+    if (kind == 0) fp64_probe_kernel<0><<<blocks, threads, 0, st>>>(scratch, 0.999999, 1e-6, iters);
+    else fp64_probe_kernel<1><<<blocks, threads, 0, st>>>(scratch, 0.999999, 1e-6, iters);
     cudaEventRecord(e1, st);
     if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
     float ms = 0.f;
@@ -588,7 +425,6 @@ double measure_fp64(cudaStream_t st, int kind, int repeats) {
     if (r > 0 && ms > 0.f) best = fmax(best, inst / (ms * 1e-3));
   }
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(out);
   return cudaGetLastError() == cudaSuccess ? best : -1.0;
 }
 
@@ -653,63 +489,14 @@ int launch_sums(const DevP& P, int kind, double* partial, double* out, cudaStrea
 int sums_scratch_doubles() { return 5 * SUM_BLOCKS + 8; }
 
 // -------------------------------------------------------------------------- launch wrappers
-static inline dim3 grid2d(const DevP& P, dim3 b) { return dim3((P.nx + b.x - 1) / b.x, (P.ny + b.y - 1) / b.y, P.nz); }
-
-int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st) {
-  dim3 b(128), g((P.px + 127) / 128, P.py, P.pz);
-  const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
-#define STREAMS_FILL(V, C)                                            \
-  do {                                                                \
-    if (with_dt) fill_prim_kernel<V, C, true><<<g, b, 0, st>>>(P);    \
-    else fill_prim_kernel<V, C, false><<<g, b, 0, st>>>(P);           \
-  } while (0)
-  if (visc && sc) STREAMS_FILL(true, true);
-  else if (visc) STREAMS_FILL(true, false);
-  else if (sc) STREAMS_FILL(false, true);
-  else STREAMS_FILL(false, false);
-#undef STREAMS_FILL
-  return 1;
-}
-
-int launch_fill_ghosts(const DevP& P, cudaStream_t st) {
-  const int g = P.ng;
-  const long long wx = P.nx + 2 * g;
-  const long long total = (P.own_z ? 0 : 2LL * g * P.py * wx) + (P.own_y ? 0 : (long long)P.nz * 2 * g * wx) +
-                          (P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g);
-  if (total == 0) return 0;
-  dim3 b(128), gr((unsigned)((total + 127) / 128));
-  const bool visc = P.visc_law != VISC_NONE, sc = P.flux_mode != FLUX_CENTRAL;
-  if (visc && sc) fill_ghost_kernel<true, true><<<gr, b, 0, st>>>(P);
-  else if (visc) fill_ghost_kernel<true, false><<<gr, b, 0, st>>>(P);
-  else if (sc) fill_ghost_kernel<false, true><<<gr, b, 0, st>>>(P);
-  else fill_ghost_kernel<false, false><<<gr, b, 0, st>>>(P);
-  return 1;
-}
-
-template <int L>
-static int launch_sensor_L(const DevP& P, bool mask, bool theta, cudaStream_t st) {
-  dim3 b(64, 4), g = grid2d(P, b);
-  if (theta) sensor_kernel<L, true, true><<<g, b, 0, st>>>(P);
-  else if (mask) sensor_kernel<L, true, false><<<g, b, 0, st>>>(P);
-  else sensor_kernel<L, false, false><<<g, b, 0, st>>>(P);
-  const long long ghosts = 2LL * P.ng * ((long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny);
-  dim3 gg((unsigned)((ghosts + 255) / 256));
-  if (mask || theta) scalar_ghost_kernel<true><<<gg, 256, 0, st>>>(P);
-  else scalar_ghost_kernel<false><<<gg, 256, 0, st>>>(P);
-  return 2;
-}
-template <int L, bool MASK, bool THETA>
-static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t st) {
+// configure: only opt the instantiation in to its dynamic shared memory on the current device (streams_init).
+template <int L, bool MASK, bool THETA, int NG>
+static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t st, bool configure) {
   constexpr int TY = STREAMS_SENSOR_TY;
-  using SM = SensorSmem<TY>;
-  auto kern = sensor_march_kernel<L, MASK, THETA, TY>;
-  static int attr_dev = -1;                          // the opt-in is per device: redo it when the current device changes
-  int dev = 0;
-  cudaGetDevice(&dev);
-  if (attr_dev != dev) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
-    attr_dev = dev;
-  }
+  using SM = SensorSmem<TY, NG>;
+  auto kern = sensor_march_kernel<L, MASK, THETA, TY, NG>;
+  if (configure)
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) == cudaSuccess ? 0 : -2;
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int chunks = pick_chunks(nbx * nby, P.nz, P.nsm * STREAMS_SENSOR_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
@@ -722,40 +509,42 @@ static int launch_sensor_march(const DevP& P, const MarchMaps& mp, cudaStream_t 
   return 2;
 }
 
-int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool theta, cudaStream_t st) {
-  if (L <= 3 && P.ng == 3) {
-#define STREAMS_SENSOR(LL)                                              \
-  do {                                                                  \
-    if (theta) return launch_sensor_march<LL, true, true>(P, mp, st);   \
-    if (mask) return launch_sensor_march<LL, true, false>(P, mp, st);   \
-    return launch_sensor_march<LL, false, false>(P, mp, st);            \
+// L = central_order / 2 on the three-layer layout; the four-layer layout runs the L = 4 instance on the zero-padded
+// coefficient table (acc + 0 * delta = acc exactly: the canonical order and its bits are those of order 2L).
+// variant: 0 dilatation only, 1 + mask, 2 + mask + theta; bit 2 set = configure all three variants.
+int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool theta, cudaStream_t st, bool configure) {
+  if (L < 1 || L > P.ng || (P.ng != 3 && P.ng != 4)) return -1;
+#define STREAMS_SENSOR(LL, GG)                                                                  \
+  do {                                                                                          \
+    if (configure) {                                                                            \
+      const int a = launch_sensor_march<LL, true, true, GG>(P, mp, st, true);                   \
+      const int b = launch_sensor_march<LL, true, false, GG>(P, mp, st, true);                  \
+      const int c = launch_sensor_march<LL, false, false, GG>(P, mp, st, true);                 \
+      return (a | b | c) ? -2 : 0;                                                              \
+    }                                                                                           \
+    if (theta) return launch_sensor_march<LL, true, true, GG>(P, mp, st, false);                \
+    if (mask) return launch_sensor_march<LL, true, false, GG>(P, mp, st, false);                \
+    return launch_sensor_march<LL, false, false, GG>(P, mp, st, false);                         \
   } while (0)
-    if (L == 1) STREAMS_SENSOR(1);
-    if (L == 2) STREAMS_SENSOR(2);
-    STREAMS_SENSOR(3);
+  if (P.ng == 4) STREAMS_SENSOR(4, 4);
+  if (L == 1) STREAMS_SENSOR(1, 3);
+  if (L == 2) STREAMS_SENSOR(2, 3);
+  STREAMS_SENSOR(3, 3);
 #undef STREAMS_SENSOR
-  }
-  switch (L) {
-    case 1: return launch_sensor_L<1>(P, mask, theta, st);
-    case 2: return launch_sensor_L<2>(P, mask, theta, st);
-    case 3: return launch_sensor_L<3>(P, mask, theta, st);
-    default: return launch_sensor_L<4>(P, mask, theta, st);
-  }
 }
 
-int launch_flags(const DevP& P, int L, int r, cudaStream_t st) {
+int launch_flags(const DevP& P, int r, cudaStream_t st) {
   const int nwx = (P.nx + 7) / 8;
   const long long nwords = (long long)nwx * P.ny * P.nz;
-  dim3 b(256), g((unsigned)((nwords + 255) / 256));
-  const bool reset_here = !(L <= 3 && P.ng == 3);     // sensor_march_kernel resets the counters itself
-  if (reset_here) reset_counters_kernel<<<1, 1, 0, st>>>(P);
+  dim3 b(256), g((unsigned)((nwords + 255) / 256));       // (sensor_march_kernel has reset the per-evaluation counters)
   switch (r) {
     case 1: flags_kernel<1><<<g, b, 0, st>>>(P, nwx); break;
     case 2: flags_kernel<2><<<g, b, 0, st>>>(P, nwx); break;
     case 3: flags_kernel<3><<<g, b, 0, st>>>(P, nwx); break;
-    default: flags_kernel<4><<<g, b, 0, st>>>(P, nwx); break;
+    case 4: flags_kernel<4><<<g, b, 0, st>>>(P, nwx); break;
+    default: return -1;
   }
-  return reset_here ? 2 : 1;
+  return 1;
 }
 
 int launch_dt(const DevP& P, double dt_fixed, bool recompute, cudaStream_t st) {

@@ -1,16 +1,12 @@
 // a4-a8 (+ a2, a1 and a9 of the next stage): the fused right-hand side, RK update and primitives.
 //
-//   weno_list_kernel : hybrid mode, runs first.  The flagged interfaces of each direction were compacted into work lists by
-//                      flags_kernel; persistent blocks evaluate them with full warps: WENO characteristic flux (O3) minus
-//                      the central flux that rhs_march_kernel implies there -> dF at the left node's index.
-//   weno_kernel      : full-WENO mode: every interface, the WENO flux itself.
 //   rhs_march_kernel : every node, one pass (2.5-D z-march, TMA + mbarrier pipeline): central split convective terms in
-//                      x, y, z (O1), viscous terms (O4), -(dF_{n+1/2} - dF_{n-1/2}) metric at nodes next to a
-//                      flagged interface, body force (S17), low-storage RK3 update (O5); then the primitives of the updated
-//                      node into the OTHER primitive buffer (stencils of this stage still read the current one), also at
-//                      its periodic images in the ghost layers, and in the last stage the time-step rate (a9).
-// R, w and the primitives are written once per stage; every flagged interface is evaluated exactly once, by a warp
-// whose lanes all do WENO work.
+//                      x, y, z (O1), viscous terms (O4), the net WENO correction of the node where an adjacent
+//                      interface is flagged (DevP::corr, gathered by corr_gather_kernel, streams_weno.cu), body force
+//                      (S17), low-storage RK3 update (O5); then the primitives of the updated node into the OTHER
+//                      primitive buffer (stencils of this stage still read the current one), also at its periodic images
+//                      in the ghost layers, and in the last stage the time-step rate (a9) and a finiteness check.
+// R, w and the primitives are written once per stage.
 #include "streams_dev.cuh"
 #include "streams_launch.h"
 #include "streams_tma.cuh"
@@ -71,10 +67,11 @@ __device__ __forceinline__ void scalar_terms(const DevP& P, const G& g, const YM
 //   f_{n+1/2} - f_{n-1/2} = sum_l [ m(n,n+l)(phi_n+phi_{n+l}) - m(n-l,n)(phi_{n-l}+phi_n) ]
 //                         = phi_n S0 + sum_l [ m(n,n+l) phi_{n+l} - m(n-l,n) phi_{n-l} ],  S0 = sum_l [m(n,n+l) - m(n-l,n)]
 // (the oracle's interface-flux sum, regrouped), plus sum_l a_l (p_{n+l} - p_{n-l}) on the D-momentum.
-// c0 = (u, v, w, H, p, rho) at the node, alr[l] = (a_l/4) rho_0.
+// c0 = (u, v, w, H, p, rho) at the node, alr[l] = (a_l/4) rho_0.  Orders below the instantiated one run on
+// zero-padded coefficient tables (DevP::a1 ...): the extra terms are exact zeros.
 template <int D, int L, int LV, bool CONV, bool VISC, class G>
 __device__ __forceinline__ void dir_terms(const DevP& P, const G& g, const YMet& ym, const double c0[6],
-                                          const double alr[3], double r[5], Visc& V) {
+                                          const double alr[4], double r[5], Visc& V) {
   constexpr int LC = CONV ? L : 0;
   constexpr int LVV = VISC ? LV : 0;
   constexpr int LM = LC > LVV ? LC : LVV;
@@ -155,49 +152,49 @@ __device__ __forceinline__ void viscous_close(const DevP& P, const double c0[6],
 
 // ---------------------------------------------------------------------------------------------
 // rhs_march_kernel (a4-a8 in one pass).  A block owns a 32 x TY tile of (x, y) and marches through a chunk
-// of z planes (2.5-D blocking):
-//   - z neighbours: every thread keeps the 7-plane column (k-3 .. k+3) of its node for all fields in
-//     registers; plane k+4 arrives by TMA in a shared-memory slot and enters the ring at the shift;
-//   - x / y neighbours: the centre plane of all fields with its 3-wide halo is ONE 4-D TMA box
-//     (x, y, z, field) = (40, TY+6, 1, 9) into one of two shared-memory buffers, issued two planes ahead;
+// of z planes (2.5-D blocking); NG = DevP::ng (3, or 4 for the order-8 / WENO-7 layouts):
+//   - z neighbours: every thread keeps the (2 NG + 1)-plane column (k-NG .. k+NG) of its node for all fields in
+//     registers; plane k+NG+1 arrives by TMA in a shared-memory slot and enters the ring at the shift;
+//   - x / y neighbours: the centre plane of all fields with its NG-wide halo is ONE 4-D TMA box
+//     (x, y, z, field) = (40, TY+2NG, 1, NF) into one of two shared-memory buffers, issued two planes ahead;
 //     every stencil offset is a compile-time immediate;
 //   - RK operands (w, previous-stage R) of the plane arrive by TMA one plane ahead;
-//   - flux corrections of flagged interfaces (hybrid / WENO): cp.async with zero fill, by the warps that
-//     have a flagged node only.
+//   - the net WENO correction of nodes next to a flagged interface (hybrid / WENO; 5 values per node, already
+//     multiplied by the metrics): cp.async with zero fill, by the warps that have such a node only.
 // One thread issues the TMA copies after a split barrier (bar.arrive by the other warps, bar.sync by
 // its warp), so no warp but that one waits for the slowest.  Completion is tracked by mbarriers.
 // ---------------------------------------------------------------------------------------------
-template <int TY, bool VISC, bool WENO>
+template <int TY, int NG, bool VISC, bool WENO>
 struct MarchSmem {
-  using G = MarchGeom<TY>;
+  using G = MarchGeom<TY, NG>;
   static constexpr int NF = VISC ? 9 : 6;
   static constexpr size_t BUF = (size_t)NF * G::PLANE * 8;     // one centre-plane buffer
   static constexpr size_t RING = (size_t)NF * G::NT * 8;       // one ring-plane slot
   static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[5]
-  static constexpr size_t DFS = WENO ? (size_t)30 * G::NT * 8 : 0;
+  static constexpr size_t DFS = WENO ? (size_t)5 * G::NT * 8 : 0;
   static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + 2 * RING, OFF_DFS = OFF_EPI + 2 * EPI,
                           OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 32 + 8 * 32;   // 4 mbarriers, rate scratch
   static_assert(BUF % 128 == 0 && RING % 128 == 0 && EPI % 128 == 0, "TMA destinations are 128-byte aligned");
+  static_assert(TOTAL <= 227 * 1024, "shared memory of one block");
 };
 
-template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
 #ifndef STREAMS_MARCH_MINB
 #define STREAMS_MARCH_MINB 1
 #endif
+template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY, int NG>
 __global__ void __launch_bounds__(MTX * TY, STREAMS_MARCH_MINB)
 rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
                  const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r, const DevP P,
                  const StageArgs sa, int nbx, int nby, int kz) {
-  using G = MarchGeom<TY>;
-  using SM = MarchSmem<TY, VISC, WENO>;
+  using G = MarchGeom<TY, NG>;
+  using SM = MarchSmem<TY, NG, VISC, WENO>;
   constexpr int NF = SM::NF;
-  constexpr int NG = 3;
   static_assert(L <= NG && LV <= NG, "ring depth");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][NF][PLANE]
   double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][NF][NT]
   double* const epi = reinterpret_cast<double*>(smem_raw + SM::OFF_EPI);    // [2][10][NT]
-  double* const dfs = reinterpret_cast<double*>(smem_raw + SM::OFF_DFS);    // [30][NT]
+  double* const dfs = reinterpret_cast<double*>(smem_raw + SM::OFF_DFS);    // [5][NT]
   unsigned long long* const bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
   unsigned long long* const full_c = bars;        // [2] centre plane landed
   unsigned long long* const full_e = bars + 2;    // [2] ring plane + RK operands landed
@@ -213,24 +210,24 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   if (kb >= ke) return;
   const int i = i0 + tx, j = j0 + ty;
   const bool active = i < P.nx && j < P.ny;
-  const int ic = min(i, P.nx + P.ng - 1), jc = min(j, P.ny + P.ng - 1);
+  const int ic = min(i, P.nx + NG - 1), jc = min(j, P.ny + NG - 1);
   const int isz = (int)P.sz;
   const int ncol = (int)pidx(P, ic, jc, 0);            // this thread's column at k = 0 (padded index < 2^31)
-  const int s0 = (ty + 3) * G::ROW + tx + 4;           // this node in a shared-memory plane
+  const int s0 = (ty + NG) * G::ROW + tx + 4;          // this node in a shared-memory plane
 
   const unsigned bytes_c = (unsigned)SM::BUF;
   const unsigned bytes_e = (unsigned)SM::RING + (sa.update_w ? 5u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
-  const int cx0 = i0 + P.ox, cy0 = j0 + P.ng;          // tile origin in padded coordinates
+  const int cx0 = i0 + P.ox, cy0 = j0 + NG;            // tile origin in padded coordinates
 
   auto issue_centre = [&](int k, int b) {              // thread 0 only
     mbar_expect_tx(&full_c[b], bytes_c);
-    tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - 3, k + P.ng, 0);
+    tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
   };
-  auto issue_ring_epi = [&](int k, int b) {            // ring plane k+4 and the RK operands of plane k into slot b
+  auto issue_ring_epi = [&](int k, int b) {            // ring plane k+NG+1 and the RK operands of plane k into slot b
     mbar_expect_tx(&full_e[b], bytes_e);
-    tma_load_4d(ring + (size_t)b * NF * G::NT, &tm_ring, &full_e[b], cx0, cy0, k + NG + 1 + P.ng, 0);
-    if (sa.read_prev) tma_load_4d(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + P.ng, 0);
-    if (sa.update_w) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + P.ng, 0);
+    tma_load_4d(ring + (size_t)b * NF * G::NT, &tm_ring, &full_e[b], cx0, cy0, k + NG + 1 + NG, 0);
+    if (sa.read_prev) tma_load_4d(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + NG, 0);
+    if (sa.update_w) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + NG, 0);
   };
 
 #ifndef STREAMS_MARCH_PF
@@ -239,12 +236,16 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   // The streams that miss L2 (the new ring plane and the RK operands) are needed one plane after they are
   // issued, which keeps too few bytes in flight to cover the DRAM latency: PF planes further ahead the same
   // boxes are requested into L2 only.
+#ifdef STREAMS_MARCH_PF_ALL
+  constexpr int PF = STREAMS_MARCH_PF;
+#else
   constexpr int PF = (VISC || WENO) ? 0 : STREAMS_MARCH_PF;   // measured: helps the lean variant only
+#endif
   auto prefetch_ring_epi = [&](int k) {                // thread 0 only
     if (PF > 0 && k < ke) {
-      tma_prefetch_4d(&tm_ring, cx0, cy0, k + NG + 1 + P.ng, 0);
-      if (sa.read_prev) tma_prefetch_4d(&tm_r, cx0, cy0, k + P.ng, 0);
-      if (sa.update_w) tma_prefetch_4d(&tm_w, cx0, cy0, k + P.ng, 0);
+      tma_prefetch_4d(&tm_ring, cx0, cy0, k + NG + 1 + NG, 0);
+      if (sa.read_prev) tma_prefetch_4d(&tm_r, cx0, cy0, k + NG, 0);
+      if (sa.update_w) tma_prefetch_4d(&tm_w, cx0, cy0, k + NG, 0);
     }
   };
   if (tid == 0) {
@@ -273,7 +274,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const double sb2 = fma(-2.0 * P.sbv, ym.eyv2, P.sb2xz);
   const double dt = sa.update_w ? P.scal[S_DT] : 0.0;
 
-  // ring = planes kb-3 .. kb+3 of this thread's column
+  // ring = planes kb-NG .. kb+NG of this thread's column
   double zr[NF][2 * NG + 1];
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
@@ -285,7 +286,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const int xoff = !P.own_x ? 0 : (i < NG ? P.nx : (i >= P.nx - NG ? -P.nx : 0));
   const int yoff = !P.own_y ? 0 : (j < NG ? P.ny * (int)P.sy : (j >= P.ny - NG ? -P.ny * (int)P.sy : 0));
   double rate = 0.0;                                  // a9 of the next step (last stage only)
-  bool rate_nan = false;
+  bool bad = false;                                   // a NaN rate, or a non-finite updated state
   unsigned fl_next = 0;
   if (WENO && CONV && active) fl_next = ld_u8_now(P.nflag + ncol + (long long)kb * P.sz);
 
@@ -294,24 +295,16 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     const unsigned par = (unsigned)(it >> 1) & 1u;
     const int n = ncol + k * isz;
     if (tid == G::NT - 32) prefetch_ring_epi(k + 1 + PF);   // no shared-memory hazard: any thread, off the issuing warp's path
-    // flags of this plane (prefetched), of the next one, and this plane's flux corrections
-    unsigned fl = 0;
-    bool any_fl = false;
+    // does this node have a net WENO correction (an adjacent flagged interface)?  Flags of this plane were
+    // prefetched, the next plane's are requested now; the five values are staged while the stencils run
+    bool fl = false, any_fl = false;
     if (WENO) {
-      fl = CONV ? fl_next : (active ? 0x3fu : 0u);
+      fl = CONV ? (fl_next != 0) : active;
       if (CONV && active && k + 1 < ke) fl_next = ld_u8_now(P.nflag + n + isz);
-      any_fl = __any_sync(0xffffffffu, fl != 0);
+      any_fl = __any_sync(0xffffffffu, fl);
       if (any_fl) {
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-          const int sd = d == 0 ? 1 : (d == 1 ? (int)P.sy : isz);
-          const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
-#pragma unroll
-          for (int q = 0; q < 5; ++q) {
-            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 0) * G::NT + tid, f + (long long)q * P.fs, (fl >> (2 * d + 1)) & 1u);
-            cp_async8_zfill(dfs + ((d * 5 + q) * 2 + 1) * G::NT + tid, f + (long long)q * P.fs - sd, (fl >> (2 * d)) & 1u);
-          }
-        }
+        for (int q = 0; q < 5; ++q) cp_async8_zfill(dfs + q * G::NT + tid, P.corr + (long long)q * P.fs + n, fl);
       }
     }
 
@@ -324,9 +317,9 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     double c0[6];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c0[q] = zr[q][NG];
-    double alr[3];
+    double alr[4];
 #pragma unroll
-    for (int l = 0; l < 3; ++l) alr[l] = P.kc[l] * c0[F_RHO];
+    for (int l = 0; l < 4; ++l) alr[l] = P.kc[l] * c0[F_RHO];
     double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     Visc V;
     if (VISC) {
@@ -361,21 +354,13 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       }
     }
 
-    // (D) flux corrections of flagged interfaces, RK update, stores
+    // (D) net correction of the flagged interfaces around the node, body force, RK update, stores
     mbar_wait(&full_e[b], par);
     const double* __restrict__ ep = epi + (size_t)b * 10 * G::NT + tid;
     if (WENO && any_fl) {
       cp_async_wait_all();
-      const double met[3] = {P.inv_dx, ym.eyc, P.inv_dz};
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const double fp = dfs[((d * 5 + q) * 2 + 0) * G::NT + tid];
-          const double fm = dfs[((d * 5 + q) * 2 + 1) * G::NT + tid];
-          r[q] = fma(-met[d], fp - fm, r[q]);
-        }
-      }
+      for (int q = 0; q < 5; ++q) r[q] -= dfs[q * G::NT + tid];     // each thread reads what it staged itself
     }
     if (P.has_accel) {                               // S17: uniform body acceleration and its work
       const double rho0 = c0[F_RHO];
@@ -404,8 +389,13 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
         if (xoff) store_prims<VISC, WENO>(P, qo + xoff, o);
         if (yoff) store_prims<VISC, WENO>(P, qo + yoff, o);
         if (zoff) store_prims<VISC, WENO>(P, qo + zoff, o);
-        if (sa.want_rate) rate = fmax(rate, dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc));
-        if (sa.want_rate && !(rate == rate)) rate_nan = true;   // fmax would drop a NaN on the next plane
+        if (sa.want_rate) {                            // fmax drops a NaN operand: test the rate before the max
+          const double rr = dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc);
+          bad |= !(rr == rr);
+          rate = fmax(rate, rr);
+        }
+        if (sa.check_state)                            // the step's last stage: Inf or NaN anywhere in the new state
+          bad |= !(fabs((wn[0] + wn[1]) + (wn[2] + wn[3]) + wn[4]) <= 1.7976931348623157e308);
       }
       if (sa.write_r) {
 #pragma unroll
@@ -427,395 +417,23 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       zr[f][2 * NG] = rn[f * G::NT];
     }
   }
+  if (bad) P.scal[S_NAN] = 1.0;                       // streams_step returns STREAMS_ENAN
   // a9 of the next step: one atomicMax per block on the bit pattern of the largest rate (a NaN wins)
   if (sa.want_rate) {
-    if (rate_nan) rate = __longlong_as_double(0x7ff8000000000000LL);
+    if (bad) rate = __longlong_as_double(0x7ff8000000000000LL);
     block_rate_max(P, rate, bars + 4);
   }
 }
 
-// ---------------------------------------------------------------------------------------------
-// WENO reconstruction of order 2R-1 with Jiang-Shu weights (O3 step 4); v[0..2R-2] upwind->downwind,
-// value at the interface between v[R-1] and v[R].
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double sq(double x) { return x * x; }
-
-template <int R>
-__device__ __forceinline__ double weno_rec(const double* v, double eps);
-
-template <>
-__device__ __forceinline__ double weno_rec<1>(const double* v, double) { return v[0]; }
-
-// The Jiang-Shu weights alpha_k = d_k / (eps + beta_k)^2 are scaled by prod_j (eps + beta_j)^2, which leaves
-// omega_k = alpha_k / sum(alpha) unchanged and needs one division per reconstruction instead of R + 1.
-template <>
-__device__ __forceinline__ double weno_rec<2>(const double* v, double eps) {
-  const double q0 = 0.5 * (3.0 * v[1] - v[0]), q1 = 0.5 * (v[1] + v[2]);
-  const double s0 = eps + sq(v[1] - v[0]), s1 = eps + sq(v[2] - v[1]);
-  const double a0 = (1.0 / 3.0) * sq(s1), a1 = (2.0 / 3.0) * sq(s0);
-  return (a0 * q0 + a1 * q1) * rcp_pos(a0 + a1);
-}
-
-template <>
-__device__ __forceinline__ double weno_rec<3>(const double* v, double eps) {
-  const double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) * (1.0 / 6.0);
-  const double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) * (1.0 / 6.0);
-  const double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) * (1.0 / 6.0);
-  const double s0 = eps + ((13.0 / 12.0) * sq(v[0] - 2.0 * v[1] + v[2]) + 0.25 * sq(v[0] - 4.0 * v[1] + 3.0 * v[2]));
-  const double s1 = eps + ((13.0 / 12.0) * sq(v[1] - 2.0 * v[2] + v[3]) + 0.25 * sq(v[1] - v[3]));
-  const double s2 = eps + ((13.0 / 12.0) * sq(v[2] - 2.0 * v[3] + v[4]) + 0.25 * sq(3.0 * v[2] - 4.0 * v[3] + v[4]));
-  const double a0 = 0.1 * sq(s1 * s2), a1 = 0.6 * sq(s0 * s2), a2 = 0.3 * sq(s0 * s1);
-  return (a0 * q0 + a1 * q1 + a2 * q2) * rcp_pos((a0 + a1) + a2);
-}
-
-template <>
-__device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
-  const double q0 = (-3.0 * v[0] + 13.0 * v[1] - 23.0 * v[2] + 25.0 * v[3]) * (1.0 / 12.0);
-  const double q1 = (v[1] - 5.0 * v[2] + 13.0 * v[3] + 3.0 * v[4]) * (1.0 / 12.0);
-  const double q2 = (-v[2] + 7.0 * v[3] + 7.0 * v[4] - v[5]) * (1.0 / 12.0);
-  const double q3 = (3.0 * v[3] + 13.0 * v[4] - 5.0 * v[5] + v[6]) * (1.0 / 12.0);
-  const double k = 1.0 / 240.0;
-  const double s0 = eps + k * (v[0] * (547.0 * v[0] - 3882.0 * v[1] + 4642.0 * v[2] - 1854.0 * v[3]) +
-                               v[1] * (7043.0 * v[1] - 17246.0 * v[2] + 7042.0 * v[3]) +
-                               v[2] * (11003.0 * v[2] - 9402.0 * v[3]) + 2107.0 * v[3] * v[3]);
-  const double s1 = eps + k * (v[1] * (267.0 * v[1] - 1642.0 * v[2] + 1602.0 * v[3] - 494.0 * v[4]) +
-                               v[2] * (2843.0 * v[2] - 5966.0 * v[3] + 1922.0 * v[4]) +
-                               v[3] * (3443.0 * v[3] - 2522.0 * v[4]) + 547.0 * v[4] * v[4]);
-  const double s2 = eps + k * (v[2] * (547.0 * v[2] - 2522.0 * v[3] + 1922.0 * v[4] - 494.0 * v[5]) +
-                               v[3] * (3443.0 * v[3] - 5966.0 * v[4] + 1602.0 * v[5]) +
-                               v[4] * (2843.0 * v[4] - 1642.0 * v[5]) + 267.0 * v[5] * v[5]);
-  const double s3 = eps + k * (v[3] * (2107.0 * v[3] - 9402.0 * v[4] + 7042.0 * v[5] - 1854.0 * v[6]) +
-                               v[4] * (11003.0 * v[4] - 17246.0 * v[5] + 4642.0 * v[6]) +
-                               v[5] * (7043.0 * v[5] - 3882.0 * v[6]) + 547.0 * v[6] * v[6]);
-  const double p01 = s0 * s1, p23 = s2 * s3;
-  const double a0 = (1.0 / 35.0) * sq(s1 * p23), a1 = (12.0 / 35.0) * sq(s0 * p23);
-  const double a2 = (18.0 / 35.0) * sq(p01 * s3), a3 = (4.0 / 35.0) * sq(p01 * s2);
-  return (a0 * q0 + a1 * q1 + a2 * q2 + a3 * q3) * rcp_pos(((a0 + a1) + a2) + a3);
-}
-
-// Both reconstructions of a characteristic field (upwind and mirrored stencil) as ONE call with the arguments by
-// value, in registers: the five fields of an interface then share one copy of the code instead of ten inlined
-// reconstructions (instruction-cache footprint: the list kernel's straight-line code shrinks by 30 %), while the two
-// reconstructions of a field still interleave.  STREAMS_WENO_REC_INLINE restores the inlined form.
-template <int R>
-__device__ __forceinline__ double weno_rec_pair(const double* gp, const double* gm, double eps) {
-  return weno_rec<R>(gp, eps) + weno_rec<R>(gm, eps);
-}
-#ifndef STREAMS_WENO_REC_INLINE
-__device__ __noinline__ double weno_rec5_pair_call(double p0, double p1, double p2, double p3, double p4, double m0, double m1,
-                                                  double m2, double m3, double m4, double eps) {
-  const double gp[5] = {p0, p1, p2, p3, p4}, gm[5] = {m0, m1, m2, m3, m4};
-  return weno_rec<3>(gp, eps) + weno_rec<3>(gm, eps);
-}
-template <>
-__device__ __forceinline__ double weno_rec_pair<3>(const double* gp, const double* gm, double eps) {
-  return weno_rec5_pair_call(gp[0], gp[1], gp[2], gp[3], gp[4], gm[0], gm[1], gm[2], gm[3], gm[4], eps);
-}
-#endif
-
-// ---------------------------------------------------------------------------------------------
-// WENO characteristic flux at interface n+1/2 along D (O3), and the central flux (O1) it replaces.
-// Characteristic projections are formed from primitives: with W the conserved state and
-// F = u_D W + p (0, e_D, u_D), l.W = rho (l0 + l1 u + l2 v + l3 w + l4 H) - l4 p and
-// l.F = u_D (l.W) + p (l_{1+D} + l4 u_D).  With b1 = (gamma-1)/c^2, b2 = b1 q^2/2 and the 1/2 of the
-// Lax-Friedrichs splitting folded into l, the three non-shear rows share per node
-//   A  = [rho (b2 - b1 vbar.v + b1 H) - b1 p] / 4        B  = rho (un - u_D) / (4 c)
-//   FA = u_D A + b1 p (u_D - un) / 4                     FB = u_D B - p / (4 c)
-// as  u-c: (l.W, l.F) = (A + B, FA + FB);  u+c: (A - B, FA - FB);  entropy: (rho/2 - 2A, rho u_D/2 - 2FA);
-// the two shear rows (l = (-vbar_t, e_t, 0)) collapse to l.W = rho (v_t - vbar_t)/2, l.F = u_D (l.W).
-// The 2R-node stencil of (rho, u, v, w, H, p) lives in a per-thread column of shared memory
-// (st[(f * 2R + m) * WTH], conflict-free) so that the kernel fits 4 blocks of 128 threads per SM; every node is
-// read once per pass (central pairs, shared rows, entropy row, shear rows): ~120 loads per interface.
-// ---------------------------------------------------------------------------------------------
-constexpr int WTH = 128;       // threads per block of weno_kernel
-constexpr int WCH = 2048;      // interface slots per block
-
-#define ST(fld, m) (((volatile double*)st)[((fld) * NS + (m)) * WTH])
-enum { SF_RHO = 0, SF_U = 1, SF_V = 2, SF_W = 3, SF_H = 4, SF_P = 5 };
-
-// Central interface flux (O1) from the shared-memory stencil (needs L <= R): the flux that rhs_march_kernel's
-// pair-difference form implies at this interface.  f = 1/4 sum_l a_l sum_{m<l} (rho_a+rho_b)(ud_a+ud_b)(phi_a+phi_b),
-// pairs (a, b) = (n-m, n-m+l).  The L left nodes stay in registers, the right nodes stream past them.
-template <int D, int L, int R>
-__device__ __forceinline__ void central_flux_st(const DevP& P, double f[5], const double* st) {
-  static_assert(L <= R, "the central stencil must fit in the WENO stencil");
-  constexpr int NS = 2 * R;
-  double lf[L][6];                                 // left nodes n, n-1, .., n-L+1: rho, u, v, w, H, p
-#pragma unroll
-  for (int m = 0; m < L; ++m) {
-#pragma unroll
-    for (int q = 0; q < 6; ++q) lf[m][q] = ST(q, R - 1 - m);
-  }
-  double fs[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ps = 0.0;
-#pragma unroll
-  for (int j = 0; j < L; ++j) {                    // right node n+1+j pairs with left node n-m at distance l = j+1+m
-    double rt[6];
-#pragma unroll
-    for (int q = 0; q < 6; ++q) rt[q] = ST(q, R + j);
-#pragma unroll
-    for (int m = 0; m + j < L; ++m) {
-      const double al = P.a1[j + m];
-      const double ru = (al * (lf[m][SF_RHO] + rt[SF_RHO])) * (lf[m][SF_U + D] + rt[SF_U + D]);
-      fs[0] += ru;
-#pragma unroll
-      for (int q = 1; q < 5; ++q) fs[q] = fma(ru, lf[m][q] + rt[q], fs[q]);
-      ps = fma(al, lf[m][SF_P] + rt[SF_P], ps);
-    }
-  }
-  f[0] = 0.5 * fs[0];
-#pragma unroll
-  for (int q = 1; q < 5; ++q) f[q] = 0.25 * fs[q];
-  f[1 + D] += ps;
-}
-
-// Fills the stencil column of interface n+1/2 (left node index n, stride s along D) and returns the local
-// Lax-Friedrichs speeds max |u_D - c|, |u_D|, |u_D + c| over its 2R nodes.
-template <int D, int R>
-__device__ __forceinline__ void weno_stencil(const DevP& P, long long n, long long s, double* __restrict__ st, double lam[3]) {
-  constexpr int NS = 2 * R;
-  lam[0] = lam[1] = lam[2] = 0.0;
-#pragma unroll
-  for (int m = 0; m < NS; ++m) {
-    const long long a = n + (long long)(m - R + 1) * s;
-    const double u = P.q[Q_U * P.fs + a], v = P.q[Q_V * P.fs + a], w = P.q[Q_W * P.fs + a];
-    const double c = P.q[Q_C * P.fs + a];
-    ST(SF_RHO, m) = P.q[Q_RHO * P.fs + a];
-    ST(SF_U, m) = u;
-    ST(SF_V, m) = v;
-    ST(SF_W, m) = w;
-    ST(SF_H, m) = P.q[Q_H * P.fs + a];
-    ST(SF_P, m) = P.q[Q_P * P.fs + a];
-    const double ud = D == 0 ? u : (D == 1 ? v : w);
-    lam[0] = fmax(lam[0], fabs(ud - c));
-    lam[1] = fmax(lam[1], fabs(ud));
-    lam[2] = fmax(lam[2], fabs(ud + c));
-  }
-}
-
-template <int D, int R>
-__device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], double f[5], const double* __restrict__ st) {
-  constexpr int NS = 2 * R;
-  // Roe average of nodes n (slot R-1) and n+1 (slot R)
-  const double rw = sqrt(ST(SF_RHO, R) * rcp_pos(ST(SF_RHO, R - 1)));
-  const double iden = rcp_pos(1.0 + rw);
-  double vb[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) vb[a] = (ST(SF_U + a, R - 1) + rw * ST(SF_U + a, R)) * iden;
-  const double Hb = (ST(SF_H, R - 1) + rw * ST(SF_H, R)) * iden;
-  const double qq = 0.5 * (vb[0] * vb[0] + vb[1] * vb[1] + vb[2] * vb[2]);
-  const double cb = sqrt(P.gm1 * (Hb - qq));
-  const double ic = rcp_pos(cb);
-  const double un = vb[D];
-  const double k1 = 0.25 * (P.gm1 * (ic * ic)), k2 = qq * k1, ki = 0.25 * ic;
-  constexpr int T1 = (D == 0) ? 1 : 0;
-  constexpr int T2 = (D == 2) ? 1 : 2;
-  double gp[NS], gm[NS];
-
-  // shared rows of the two acoustic fields and the entropy field, one pass over the nodes
-  double A[NS], B[NS], FA[NS], FB[NS];
-#pragma unroll
-  for (int m = 0; m < NS; ++m) {
-    const double rho = ST(SF_RHO, m), um = ST(SF_U, m), vm = ST(SF_V, m), wm = ST(SF_W, m), hm = ST(SF_H, m), pm = ST(SF_P, m);
-    const double ud = D == 0 ? um : (D == 1 ? vm : wm);
-    const double dot = fma(vb[2], wm, fma(vb[1], vm, vb[0] * um));
-    const double kp = k1 * pm, du = ud - un;
-    A[m] = fma(rho, fma(k1, hm - dot, k2), -kp);
-    B[m] = -((rho * ki) * du);
-    FA[m] = fma(ud, A[m], kp * du);
-    FB[m] = fma(ud, B[m], -(ki * pm));
-  }
-  // u - c
-#pragma unroll
-  for (int m = 0; m < NS; ++m) {
-    const double lw = A[m] + B[m], lf = FA[m] + FB[m];
-    gp[m] = fma(lam[0], lw, lf);
-    gm[NS - 1 - m] = fma(-lam[0], lw, lf);          // mirrored: gm[0] is node n+R
-  }
-  const double g0 = weno_rec_pair<R>(gp, gm, P.weno_eps);
-  // u + c
-#pragma unroll
-  for (int m = 0; m < NS; ++m) {
-    const double lw = A[m] - B[m], lf = FA[m] - FB[m];
-    gp[m] = fma(lam[2], lw, lf);
-    gm[NS - 1 - m] = fma(-lam[2], lw, lf);
-  }
-  const double g4 = weno_rec_pair<R>(gp, gm, P.weno_eps);
-  // entropy
-#pragma unroll
-  for (int m = 0; m < NS; ++m) {
-    const double hr = 0.5 * ST(SF_RHO, m);
-    const double lw = fma(-2.0, A[m], hr), lf = fma(-2.0, FA[m], hr * ST(SF_U + D, m));
-    gp[m] = fma(lam[1], lw, lf);
-    gm[NS - 1 - m] = fma(-lam[1], lw, lf);
-  }
-  const double g1 = weno_rec_pair<R>(gp, gm, P.weno_eps);
-  // the two shear fields
-  double gs[2];
-#pragma unroll
-  for (int e = 0; e < 2; ++e) {
-    const int t = e == 0 ? T1 : T2;
-#pragma unroll
-    for (int m = 0; m < NS; ++m) {
-      const double lw = (0.5 * ST(SF_RHO, m)) * (ST(SF_U + t, m) - vb[t]);
-      const double lf = ST(SF_U + D, m) * lw;
-      gp[m] = fma(lam[1], lw, lf);
-      gm[NS - 1 - m] = fma(-lam[1], lw, lf);
-    }
-    gs[e] = weno_rec_pair<R>(gp, gm, P.weno_eps);
-  }
-  // f = sum over the fields of g r: r(u-+c) = (1, vbar -+ c e_D, H -+ un c), r(entropy) = (1, vbar, q^2/2), r(shear t) = (0, e_t, vbar_t)
-  const double gsum = (g0 + g4) + g1, gdc = (g4 - g0) * cb;
-  f[0] = gsum;
-#pragma unroll
-  for (int a = 0; a < 3; ++a) f[1 + a] = vb[a] * gsum;
-  f[1 + D] += gdc;
-  f[1 + T1] += gs[0];
-  f[1 + T2] += gs[1];
-  f[4] = fma(Hb, g0 + g4, fma(un, gdc, fma(qq, g1, fma(vb[T1], gs[0], vb[T2] * gs[1]))));
-}
-#undef ST
-
-// ---------------------------------------------------------------------------------------------
-// weno_kernel: blocks [0, nb0) work on x interfaces, [nb0, nb0 + nb1) on y, the rest on z.  A block owns
-// WCH consecutive interface slots of its direction (slot = interior extents with the D extent enlarged by
-// one; slot s along D is the interface between nodes s - 1 and s).  Hybrid mode: the flagged slots are
-// compacted into a shared-memory list (flag bits of flags_kernel: plus side of the left node, or minus side
-// of node 0 for the first interface of a pencil), then walked by all threads, so lanes stay converged on
-// WENO work whatever the activation pattern.  DENSE (full-WENO mode): every slot, WENO flux itself stored.
-// ---------------------------------------------------------------------------------------------
-template <int D, int L, int R, bool DENSE>
-__device__ __forceinline__ void weno_block(const DevP& P, long long chunk, int* s_list, int* s_count, double* s_st) {
-  const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
-  const int e0 = P.nx + (D == 0), e1 = P.ny + (D == 1), e2 = P.nz + (D == 2);
-  const int lane = threadIdx.x & 31;
-  if (threadIdx.x == 0) *s_count = 0;
-  __syncthreads();
-  // slot of this thread in round 0, decoded once; later rounds advance it by WTH
-  const long long t0 = chunk * WCH + threadIdx.x;
-  int i = (int)(t0 % e0);
-  const long long t1 = t0 / e0;
-  int j = (int)(t1 % e1), k = (int)(t1 / e1);
-  for (int rr = 0; rr < WCH / WTH; ++rr) {
-    bool want = false;
-    int n = 0;
-    if (k < e2) {
-      n = (int)pidx(P, i - (D == 0), j - (D == 1), k - (D == 2));       // left node of the interface
-      if (DENSE) want = true;
-      else {
-        const int a = D == 0 ? i : (D == 1 ? j : k);
-        want = a > 0 ? ((P.nflag[n] >> (2 * D + 1)) & 1) : ((P.nflag[n + s] >> (2 * D)) & 1);
-      }
-    }
-    const unsigned bal = __ballot_sync(0xffffffffu, want);
-    int pos = 0;
-    if (lane == 0 && bal) pos = atomicAdd(s_count, __popc(bal));
-    pos = __shfl_sync(0xffffffffu, pos, 0);
-    if (want) s_list[pos + __popc(bal & ((1u << lane) - 1u))] = n;
-    i += WTH;
-    while (i >= e0) { i -= e0; if (++j >= e1) { j = 0; ++k; } }
-  }
-  __syncthreads();
-  const int count = *s_count;
-  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs;
-  for (int e = threadIdx.x; e < count; e += WTH) {
-    const long long n = s_list[e];
-    double fw[5], lam[3];
-    weno_stencil<D, R>(P, n, s, s_st + threadIdx.x, lam);
-    weno_flux<D, R>(P, lam, fw, s_st + threadIdx.x);
-    if (!DENSE) {
-      double fc[5];
-      central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);
-#pragma unroll
-      for (int q = 0; q < 5; ++q) fw[q] -= fc[q];
-    }
-#pragma unroll
-    for (int q = 0; q < 5; ++q) out[q * P.fs + n] = fw[q];
-  }
-}
-
-#ifndef STREAMS_WENO_MINB
-#define STREAMS_WENO_MINB 4
-#endif
-template <int L, int R, bool DENSE>
-__global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_kernel(const DevP P, int nb0, int nb1) {
-  __shared__ int s_list[WCH];
-  __shared__ int s_count;
-  __shared__ double s_st[6 * 2 * R * WTH];
-  const int b = blockIdx.x;
-  if (b < nb0) weno_block<0, L, R, DENSE>(P, b, s_list, &s_count, s_st);
-  else if (b < nb0 + nb1) weno_block<1, L, R, DENSE>(P, b - nb0, s_list, &s_count, s_st);
-  else weno_block<2, L, R, DENSE>(P, b - nb0 - nb1, s_list, &s_count, s_st);
-}
-
-// ---------------------------------------------------------------------------------------------
-// weno_list_kernel (hybrid mode): the flagged interfaces of each direction were compacted into global work
-// lists by flags_kernel (DevP::ilist, counts in DevP::counters), so every warp here is full of WENO work
-// whatever the activation pattern.  Persistent blocks walk groups of WTH consecutive list entries
-// (consecutive entries are mostly consecutive nodes: coalesced stencil loads), directions one after the other.
-// ---------------------------------------------------------------------------------------------
-template <int D, int L, int R>
-__device__ __forceinline__ void weno_list_item(const DevP& P, long long n, double* s_st) {
-  const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
-  double fw[5], fc[5], lam[3];
-  weno_stencil<D, R>(P, n, s, s_st + threadIdx.x, lam);
-  central_flux_st<D, L, R>(P, fc, s_st + threadIdx.x);     // first: its registers are free before the WENO rows are live
-  weno_flux<D, R>(P, lam, fw, s_st + threadIdx.x);
-  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
-#pragma unroll
-  for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q] - fc[q];
-}
-
-template <int L, int R>
-__global__ void __launch_bounds__(WTH, STREAMS_WENO_MINB) weno_list_kernel(const DevP P) {
-  __shared__ double s_st[6 * 2 * R * WTH];
-  const int c0 = P.counters[C_NIFACE], c1 = P.counters[C_NIFACE + 1], c2 = P.counters[C_NIFACE + 2];
-  const int g0 = (c0 + WTH - 1) / WTH, g1 = (c1 + WTH - 1) / WTH, g2 = (c2 + WTH - 1) / WTH;
-#ifndef STREAMS_WENO_CHUNK
-#define STREAMS_WENO_CHUNK 4
-#endif
-  // blocks take chunks of consecutive groups round-robin: list neighbours are grid neighbours, so the stencil rows
-  // of a group are still in this SM's L1 when the next rows' interfaces need them, while all blocks advance through
-  // the lists together (one direction's code in the instruction cache at a time).  The list entry of the next item
-  // is fetched before the current item is evaluated, which takes one dependent memory latency off every item.
-  constexpr int CH = STREAMS_WENO_CHUNK;
-  const int gt = g0 + g1 + g2;
-  auto group_of = [&](int it) { return ((int)blockIdx.x + (it / CH) * (int)gridDim.x) * CH + (it % CH); };
-  auto fetch = [&](int g, int& d) {                    // padded index of the left node of this thread's item, or -1
-    d = 0;
-    if (g >= gt) return -1;
-    int e, cd;
-    if (g < g0) { e = g * WTH + threadIdx.x; cd = c0; }
-    else if (g < g0 + g1) { d = 1; e = (g - g0) * WTH + threadIdx.x; cd = c1; }
-    else { d = 2; e = (g - g0 - g1) * WTH + threadIdx.x; cd = c2; }
-    return e < cd ? P.ilist[(long long)d * P.lcap + e] : -1;
-  };
-  int d_cur, d_nxt;
-  int n_cur = fetch(group_of(0), d_cur);
-#pragma unroll 1
-  for (int it = 0; group_of(it) < gt; ++it) {
-    const int n_nxt = fetch(group_of(it + 1), d_nxt);
-    if (n_cur >= 0) {
-      if (d_cur == 0) weno_list_item<0, L, R>(P, n_cur, s_st);
-      else if (d_cur == 1) weno_list_item<1, L, R>(P, n_cur, s_st);
-      else weno_list_item<2, L, R>(P, n_cur, s_st);
-    }
-    n_cur = n_nxt; d_cur = d_nxt;
-  }
-}
-
 // -------------------------------------------------------------------------- launch
-template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY>
-static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st) {
-  using G = MarchGeom<TY>;
-  using SM = MarchSmem<TY, VISC, WENO>;
-  auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY>;
-  static int attr_dev = -1;                          // the opt-in is per device: redo it when the current device changes
-  int dev = 0;
-  cudaGetDevice(&dev);
-  if (attr_dev != dev) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) != cudaSuccess) return -2;
-    attr_dev = dev;
-  }
+// configure: only opt the instantiation in to its dynamic shared memory on the current device (streams_init).
+template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY, int NG>
+static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st, bool configure) {
+  using G = MarchGeom<TY, NG>;
+  using SM = MarchSmem<TY, NG, VISC, WENO>;
+  auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY, NG>;
+  if (configure)
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) == cudaSuccess ? 0 : -2;
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int tiles = nbx * nby;
   const int chunks = pick_chunks(tiles, P.nz, P.nsm * STREAMS_MARCH_MINB);
@@ -824,13 +442,13 @@ static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa,
   return 1;
 }
 
-template <int L, int LV, int R>
-static int launch_main_T(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st) {
+template <int M, int NG>
+static int launch_main_T(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st, bool configure) {
   const bool visc = P.visc_law != VISC_NONE;
   const bool conv = P.flux_mode != FLUX_WENO;
   const bool weno = P.flux_mode != FLUX_CENTRAL;
   constexpr int TY = STREAMS_MARCH_TY;
-#define STREAMS_MAIN(V, C, W) return launch_march<L, LV, V, C, W, TY>(P, mp, sa, st)
+#define STREAMS_MAIN(V, C, W) return launch_march<M, M, V, C, W, TY, NG>(P, mp, sa, st, configure)
   if (visc && conv && weno) STREAMS_MAIN(true, true, true);
   else if (visc && conv) STREAMS_MAIN(true, true, false);
   else if (visc) STREAMS_MAIN(true, false, true);
@@ -853,7 +471,7 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
       qres != cudaDriverEntryPointSuccess)
     return -1;
   const encode_fn encode = (encode_fn)fn;
-  constexpr int TY = STREAMS_MARCH_TY;
+  constexpr int TY = STREAMS_MARCH_TY, STY = STREAMS_SENSOR_TY;
   const cuuint32_t nf = P.visc_law != VISC_NONE ? 9 : 6;
   const cuuint64_t strides[3] = {(cuuint64_t)P.px * 8, (cuuint64_t)P.sz * 8, (cuuint64_t)P.fs * 8};
   const cuuint32_t ones[4] = {1, 1, 1, 1};
@@ -863,45 +481,30 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
     return encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   };
-  if (make(&maps->centre, P.q, nf, MarchGeom<TY>::ROW, MarchGeom<TY>::ROWS, nf) != CUDA_SUCCESS) return -2;
+  const cuuint32_t halo = 2 * (cuuint32_t)P.ng;        // MarchGeom<TY, NG>::ROW / ROWS with NG = DevP::ng
+  if (make(&maps->centre, P.q, nf, MTX + 8, TY + halo, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->w, P.w, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
   if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
-  constexpr int STY = STREAMS_SENSOR_TY;
-  if (make(&maps->s_centre, P.q, nf, MarchGeom<STY>::ROW, MarchGeom<STY>::ROWS, 3) != CUDA_SUCCESS) return -2;
+  if (make(&maps->s_centre, P.q, nf, MTX + 8, STY + halo, 3) != CUDA_SUCCESS) return -2;
   if (make(&maps->s_ring, P.q, nf, MTX, STY, 3) != CUDA_SUCCESS) return -2;
   return 0;
 }
 
-template <int L, int R>
-static int launch_weno_T(const DevP& P, cudaStream_t st) {
-  if (P.flux_mode == FLUX_CENTRAL) return 0;
-  const long long a = (long long)P.nx * P.ny * P.nz;
-  auto blocks = [&](long long extra) { return (int)((a + extra + WCH - 1) / WCH); };
-  const int nb0 = blocks((long long)P.ny * P.nz), nb1 = blocks((long long)P.nx * P.nz), nb2 = blocks((long long)P.nx * P.ny);
-  dim3 b(WTH), g((unsigned)(nb0 + nb1 + nb2));
-  if (P.flux_mode == FLUX_HYBRID) weno_list_kernel<L, R><<<P.nsm * STREAMS_WENO_MINB, b, 0, st>>>(P);
-  else weno_kernel<L, R, true><<<g, b, 0, st>>>(P, nb0, nb1);
-  return 1;
-}
+// Instantiated families: m = 1, 2, 3 on the three-layer layout, m = 4 (central 8 / viscous 8) on the four-layer
+// one.  A scheme runs on the smallest family that covers its central and viscous orders (and on m = 4 whenever the
+// layout has four ghost layers, e.g. for WENO 7 with a lower central order); the coefficient tables of DevP are
+// zero-padded, so the terms beyond the requested order are exact zeros (x + 0 = x): mixed orders give the same
+// numbers as an instantiation of their own would.
+int march_family(int L, int Lv, int ng) { return ng == 4 ? 4 : (L > Lv ? L : Lv); }
 
-// Instantiated scheme families: m = 1, 2, 3 with central order 2m, viscous order 2m and WENO order 2m - 1
-// (2/1/2, 4/3/4, 6/5/6); orders a mode does not use are ignored.  The layout always carries ng = 3 ghost layers.
-bool rhs_supported(int L, int Lv, int r, int flux_mode, int visc_law) {
-  return L >= 1 && L <= 3 && (visc_law == VISC_NONE || Lv == L) && (flux_mode == FLUX_CENTRAL || r == L);
-}
-
-int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, int r, const StageArgs& sa, cudaStream_t st) {
-  if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
-  if (L == 1) return launch_main_T<1, 1, 1>(P, mp, sa, st);
-  if (L == 2) return launch_main_T<2, 2, 2>(P, mp, sa, st);
-  return launch_main_T<3, 3, 3>(P, mp, sa, st);
-}
-int launch_weno(const DevP& P, int L, int Lv, int r, cudaStream_t st) {
-  if (!rhs_supported(L, Lv, r, P.flux_mode, P.visc_law)) return -1;
-  if (L == 1) return launch_weno_T<1, 1>(P, st);
-  if (L == 2) return launch_weno_T<2, 2>(P, st);
-  return launch_weno_T<3, 3>(P, st);
+int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, const StageArgs& sa, cudaStream_t st, bool configure) {
+  const int m = march_family(P.flux_mode != FLUX_WENO ? L : 1, P.visc_law != VISC_NONE ? Lv : 1, P.ng);
+  if (m < 1 || m > 4 || (P.ng != 3 && P.ng != 4)) return -1;
+  if (m == 1) return launch_main_T<1, 3>(P, mp, sa, st, configure);
+  if (m == 2) return launch_main_T<2, 3>(P, mp, sa, st, configure);
+  if (m == 3) return launch_main_T<3, 3>(P, mp, sa, st, configure);
+  return launch_main_T<4, 4>(P, mp, sa, st, configure);
 }
 
 }  // namespace streams

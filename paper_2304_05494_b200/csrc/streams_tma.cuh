@@ -65,12 +65,15 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, 
 
 constexpr int MTX = 32;
 
-template <int TY>
+// Tile geometry of the z-marching kernels: a block owns MTX x TY nodes of a plane; NG = ghost width of the layout
+// (DevP::ng: 3, or 4 when an order of the scheme needs four layers) = halo rows / ring depth of the tile.
+template <int TY, int NG>
 struct MarchGeom {
-  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (3 used), rows stay 32 B aligned
-  static constexpr int ROWS = TY + 6;
+  static constexpr int ROW = MTX + 8;            // row pitch: 4 halo columns each side (NG used), rows stay 32 B aligned
+  static constexpr int ROWS = TY + 2 * NG;
   static constexpr int PLANE = ROW * ROWS;       // doubles per field per buffer
   static constexpr int NT = MTX * TY;
+  static_assert(NG >= 1 && NG <= 4, "the halo columns of a row hold at most four ghost nodes");
 };
 
 // z chunks per tile: enough blocks to fill every SM slot in whole waves, long enough that the ring fill

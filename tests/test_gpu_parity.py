@@ -157,15 +157,124 @@ def test_order_family_full_weno_and_central(S, m):
     check_case(S, _with_orders(base.replace(flux_mode=W.FLUX_CENTRAL), m), 6)
 
 
-def test_unsupported_order_mix_is_rejected_at_init(S):
+# ---- order 8 / WENO 7 / viscous 8 (four ghost layers) and mixed orders
+def test_order_family_8_7_8_hybrid_viscous_periodic(S):
+    case = W.isotropic_turbulence(nx=40, ny=37, nz=35, mach_t=0.6, k0=3.0, kmax=8, seed=31, dilatational=0.5)
+    check_case(S, _with_orders(case, 4), 10, expect_activation=(0.002, 0.8))
+
+
+def test_order_family_8_7_8_channel_walls(S):
+    check_case(S, _with_orders(W.channel(40, 36, 34, seed=32), 4), 6)
+
+
+def test_order_family_8_7_8_boundary_layer(S):
+    check_case(S, _with_orders(W.boundary_layer(72, 40, 36, seed=34, nblobs=5), 4), 6, expect_activation=(0.0005, 0.5))
+
+
+def test_order_family_8_7_8_full_weno_and_central(S):
+    base = W.isotropic_turbulence(nx=34, ny=33, nz=36, mach_t=0.4, k0=3.0, kmax=8, seed=33, viscous=False,
+                                  flux_mode=W.FLUX_WENO)
+    check_case(S, _with_orders(base, 4), 6)
+    check_case(S, _with_orders(base.replace(flux_mode=W.FLUX_CENTRAL), 4), 6)
+    # ragged and narrow: extents that are not multiples of any tile, one of them below two ghost widths
+    small = W.isotropic_turbulence(nx=35, ny=7, nz=21, mach_t=0.4, k0=2.0, kmax=3, seed=35, dilatational=0.4)
+    check_case(S, _with_orders(small, 4), 4)
+
+
+@pytest.mark.parametrize("orders", [(6, 3, 4), (4, 5, 6), (2, 7, 2), (8, 3, 6), (6, 5, 8), (2, 1, 8), (8, 1, 2)])
+def test_mixed_orders_hybrid_viscous(S, orders):
+    """Any mix of central / WENO / viscous orders runs on the covering instance with zero-padded coefficients and
+    must give the oracle's numbers for exactly that mix."""
+    co, wo, vo = orders
+    case = W.isotropic_turbulence(nx=36, ny=34, nz=33, mach_t=0.6, k0=3.0, kmax=8, seed=36, dilatational=0.5)
+    check_case(S, case.replace(central_order=co, weno_order=wo, visc_order=vo, name=f"mix_{co}_{wo}_{vo}"), 6,
+               expect_activation=(0.002, 0.8))
+
+
+@pytest.mark.parametrize("orders", [(6, 3, 6), (4, 7, 4)])
+def test_mixed_orders_channel(S, orders):
+    co, wo, vo = orders
+    check_case(S, W.channel(40, 36, 34, seed=37).replace(central_order=co, weno_order=wo, visc_order=vo), 6)
+
+
+def test_invalid_orders_are_rejected_at_init(S):
     from paper_2304_05494_b200 import binding
-    case = W.config(0).replace(central_order=8)
+    for bad in (dict(central_order=10), dict(central_order=5), dict(weno_order=9), dict(visc_order=3)):
+        case = W.isotropic_turbulence(nx=16, ny=16, nz=16, mach_t=0.3, k0=2.0, kmax=4, seed=1).replace(**bad)
+        with pytest.raises(binding.StreamsError) as e:
+            S(case)
+        assert e.value.code == binding.STREAMS_EINVAL
+
+
+# ---- branches the round-1 suite did not reach on the GPU
+def test_power_law_viscosity(S):
+    """STREAMS_VISC_POWER with a non-zero exponent and T_ref != 1 (device pow vs the oracle's std::pow)."""
+    case = W.isotropic_turbulence(nx=40, ny=36, nz=34, mach_t=0.6, k0=3.0, kmax=8, seed=41, dilatational=0.5)
+    case = case.replace(visc_law=W.VISC_POWER, pow_exp=0.76, t_ref=0.8, mu_ref=4 * case.mu_ref, name="power_law")
+    check_case(S, case, 10, expect_activation=(0.002, 0.8))
+    ch = W.channel(40, 36, 34, seed=42)
+    check_case(S, ch.replace(visc_law=W.VISC_POWER, pow_exp=0.7, t_ref=1.3, name="power_law_channel"), 6)
+
+
+def test_wall_ghost_temperature_clamp(S):
+    """Fluid hotter than 1.9 T_w next to an isothermal wall: the ghost temperature is clamped at 0.1 T_w (O6 / S15)."""
+    case = W.channel(40, 36, 34, seed=43)
+    w0 = case.w0.copy()
+    g = case.gamma
+    rho, ru, rv, rw, E = w0
+    p = (g - 1) * (E - 0.5 * (ru ** 2 + rv ** 2 + rw ** 2) / rho)
+    T = p / (case.rgas * rho)
+    for j, fac in ((0, 2.5), (1, 2.0), (case.ny - 1, 2.2)):          # rows 0, 1 at the lower wall, the last row at the upper
+        Tn = fac * case.t_wall_lo * np.ones_like(T[:, j, :])
+        rn = p[:, j, :] / (case.rgas * Tn)
+        sc = rn / rho[:, j, :]
+        for q in range(4):
+            w0[q][:, j, :] *= sc                                       # same velocities, same pressure, hotter and lighter
+        w0[4][:, j, :] = p[:, j, :] / (g - 1) + 0.5 * (w0[1][:, j, :] ** 2 + w0[2][:, j, :] ** 2 + w0[3][:, j, :] ** 2) / rn
+    check_case(S, case.replace(w0=w0, name="hot_wall"), 4)
+
+
+@pytest.mark.parametrize("flux_mode", [W.FLUX_HYBRID, W.FLUX_WENO, W.FLUX_CENTRAL])
+def test_freestream_faces_in_x_y_and_z(S, flux_mode):
+    """STREAMS_BC_FREESTREAM on all six faces, hybrid + viscous: the x-column and z-slab segments of the ghost fill and
+    the constant extrapolation of div / mask beyond non-periodic x and z faces."""
+    base = W.isotropic_turbulence(nx=37, ny=35, nz=33, mach_t=0.5, k0=3.0, kmax=8, seed=44, dilatational=0.5)
+    w0 = base.w0
+    fs = tuple(float(w0[q].mean()) for q in range(5))
+    case = base.replace(bc_x=W.BC_FREESTREAM, bc_y_lo=W.BC_FREESTREAM, bc_y_hi=W.BC_FREESTREAM, bc_z=W.BC_FREESTREAM,
+                        y_wall_lo=0.0, y_wall_hi=base.ly, freestream=fs, flux_mode=flux_mode, name="freestream_box")
+    check_case(S, case, 6, expect_activation=(0.002, 0.9) if flux_mode == W.FLUX_HYBRID else None)
+    # periodic x, free-stream z only; and the reverse
+    check_case(S, case.replace(bc_x=W.BC_PERIODIC, name="fs_z"), 3)
+    check_case(S, case.replace(bc_z=W.BC_PERIODIC, name="fs_x"), 3)
+
+
+def test_blow_up_mid_run_is_reported(S):
+    """A state that goes non-finite in the middle of a multi-step call: STREAMS_ENAN, with the CFL time step (the rate
+    of the last stage's epilogue must keep a NaN) and with a fixed one (finiteness check of the updated state)."""
+    from paper_2304_05494_b200 import binding
+    base = W.isotropic_turbulence(nx=32, ny=32, nz=32, mach_t=0.6, k0=3.0, kmax=8, seed=45, dilatational=0.5)
+    gpu = S(base)
+    dt, _ = gpu.step(2)                                   # healthy
+    assert np.isfinite(gpu.get_fields()).all()
+    gpu.destroy()
+    for case in (base.replace(cfl=40.0, name="cfl40"), base.replace(dt_fixed=60 * dt, name="dtfixed")):
+        gpu = S(case)
+        with pytest.raises(binding.StreamsError) as e:
+            gpu.step(60)
+        assert e.value.code == binding.STREAMS_ENAN
+        gpu.destroy()
+    # one node with a negative pressure, reached after a healthy step: the sound speed of that node is NaN while every
+    # conserved value stays finite; the very next dt must not come from the healthy nodes alone
+    gpu = S(base)
+    gpu.step(1)
+    w = gpu.get_fields()
+    w[4, 5, 6, 7] = 0.4 * (w[1, 5, 6, 7] ** 2 + w[2, 5, 6, 7] ** 2 + w[3, 5, 6, 7] ** 2) / w[0, 5, 6, 7]   # E < kinetic energy
+    gpu.set_fields(w)
     with pytest.raises(binding.StreamsError) as e:
-        S(case)
-    assert e.value.code == binding.STREAMS_EINVAL
-    mixed = W.isotropic_turbulence(nx=16, ny=16, nz=16, mach_t=0.3, k0=2.0, kmax=4, seed=1).replace(weno_order=3)
-    with pytest.raises(binding.StreamsError):
-        S(mixed)
+        gpu.step(3)
+    assert e.value.code == binding.STREAMS_ENAN
+    gpu.destroy()
 
 
 # ---- uniform body acceleration (DESIGN.md S17; PAPER:377 forcing)
