@@ -351,7 +351,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.mu_ref = gas->mu_ref; P.t_ref = gas->t_ref; P.suth_s = gas->suth_s_over_tref; P.pow_exp = gas->pow_exp;
   const double rr = gas->u_ref / gas->l_ref;
   P.eps_s = rr * rr;
-  P.thr = scheme->sensor_threshold; P.weno_eps = scheme->weno_eps; P.cfl = scheme->cfl;
+  P.thr = scheme->sensor_threshold; P.thr2 = P.thr * P.thr; P.weno_eps = scheme->weno_eps; P.cfl = scheme->cfl;
   for (int q = 0; q < 5; ++q) P.fsw[q] = gas->freestream[q];
   for (int d = 0; d < 3; ++d) P.accel[d] = gas->accel[d];
   P.has_accel = gas->accel[0] != 0.0 || gas->accel[1] != 0.0 || gas->accel[2] != 0.0;

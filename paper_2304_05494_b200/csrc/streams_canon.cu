@@ -144,6 +144,18 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
   }
 
+  // this thread's column in the outputs, advanced plane by plane
+  double* __restrict__ div_p = P.div + ncol + (long long)kb * isz;
+  unsigned char* __restrict__ mask_p = P.mask + ncol + (long long)kb * isz;
+  const unsigned char* __restrict__ ovr_p = P.mask_ovr ? P.mask_ovr + ncol : nullptr;
+  // does this thread own x / y face ghosts (DevP::sown: the kernel writes them itself)?
+  const bool per_z = P.bc_z == BC_PERIODIC;
+  const bool zface = P.sown != 0;
+  const bool gplan = P.sown && active &&
+                     ((P.bc_x == BC_PERIODIC ? (i < NG || i >= P.nx - NG) : (i == 0 || i == P.nx - 1)) ||
+                      (j < NG && P.bc_y_lo == BC_PERIODIC) || (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) ||
+                      (j == 0 && P.bc_y_lo != BC_PERIODIC) || (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC));
+
   for (int k = kb; k < ke; ++k) {
     const int it = k - kb, b = it & 1;
     const unsigned par = (unsigned)(it >> 1) & 1u;
@@ -169,42 +181,56 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     }
     const double dv = (gx[0] + gy[1]) + gz[2];
     if (active) {
-      const long long n = ncol + (long long)k * isz;
-      P.div[n] = dv;
+      *div_p = dv;
       unsigned char mk = 0;
       if (MASK || THETA) {
         const double ox = gy[2] - gz[1], oy = gz[0] - gx[2], oz = gx[1] - gy[0];
         const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
-        double th = -dv / sqrt(s);
-        if (!(th > 0.0)) th = 0.0;
-        if (THETA) P.theta[iidx(P, i, j, k)] = th;
-        mk = (th > P.thr) ? 1 : 0;
-        if (MASK && P.mask_ovr) mk = P.mask_ovr[n];       // imposed mask (activation sweeps)
-        if (MASK) P.mask[n] = mk;
+        // mask = theta > thr with theta = max(-dv / sqrt(s), 0).  Without the theta output the decision is taken on
+        // the squares wherever it is clear by a margin far above the rounding of either form (1e-12 relative, the
+        // quotient is good to 2 ulp); only a node within that margin of the threshold evaluates the square root and
+        // the division -- the same operations as the definition, so the mask carries the bits of the definition.
+        const double a = -dv, a2 = a * a, t2 = P.thr2 * s;
+        bool clear_hi = a > 0.0 && a2 > t2 * (1.0 + 1e-12), clear_lo = !(a > 0.0) || a2 < t2 * (1.0 - 1e-12);
+        if (P.thr < 0.0) { clear_hi = true; clear_lo = false; }       // theta >= 0 > thr at every node
+        if (a != a) { clear_hi = false; clear_lo = true; }              // NaN: theta = 0, not above a threshold >= 0
+        if (THETA || !(clear_hi || clear_lo)) {
+          double th = -dv / sqrt(s);
+          if (!(th > 0.0)) th = 0.0;
+          if (THETA) P.theta[iidx(P, i, j, k)] = th;
+          mk = (th > P.thr) ? 1 : 0;
+        } else {
+          mk = clear_hi ? 1 : 0;
+        }
+        if (MASK && ovr_p) mk = ovr_p[(long long)k * isz];   // imposed mask (activation sweeps)
+        if (MASK) *mask_p = mk;
       }
       // face ghosts of div / mask (S6), written by the node they copy: its periodic image, or the NG ghost nodes
-      // beyond a non-periodic face (constant extrapolation)
-      if (P.sown) {
-        auto put = [&](long long m) { P.div[m] = dv; if (MASK) P.mask[m] = mk; };
+      // beyond a non-periodic face (constant extrapolation).  Which x / y ghosts a thread owns is fixed along the
+      // march (gplan), the z faces are a property of the plane.
+      if (gplan | (zface && (per_z ? (k < NG || k >= P.nz - NG) : (k == 0 || k == P.nz - 1)))) {
+        auto put = [&](long long m) { div_p[m] = dv; if (MASK) mask_p[m] = mk; };
         auto face = [&](int a, int na, bool per, long long st) {      // a: index along the direction, st: its stride
           if (per) {
-            if (a < NG) put(n + na * st);
-            else if (a >= na - NG) put(n - na * st);
+            if (a < NG) put(na * st);
+            else if (a >= na - NG) put(-na * st);
           } else {
-            if (a == 0) { for (int m = 1; m <= NG; ++m) put(n - m * st); }
-            if (a == na - 1) { for (int m = 1; m <= NG; ++m) put(n + m * st); }
+            if (a == 0) { for (int m = 1; m <= NG; ++m) put(-m * st); }
+            if (a == na - 1) { for (int m = 1; m <= NG; ++m) put(m * st); }
           }
         };
         face(i, P.nx, P.bc_x == BC_PERIODIC, 1);
         if (j < NG || j >= P.ny - NG) {
-          if (j < NG && P.bc_y_lo == BC_PERIODIC) put(n + P.ny * P.sy);
-          if (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) put(n - P.ny * P.sy);
-          if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(n - m * P.sy); }
-          if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(n + m * P.sy); }
+          if (j < NG && P.bc_y_lo == BC_PERIODIC) put(P.ny * P.sy);
+          if (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) put(-P.ny * P.sy);
+          if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(-m * P.sy); }
+          if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(m * P.sy); }
         }
-        face(k, P.nz, P.bc_z == BC_PERIODIC, P.sz);
+        face(k, P.nz, per_z, P.sz);
       }
     }
+    div_p += isz;
+    mask_p += isz;
     mbar_wait(&full_r[b], par);
     const double* __restrict__ rn = ring + (size_t)b * 3 * G::NT + tid;
     // (register moves: renaming the ring through a phase switch measured slower, here and in rhs_march_kernel;

@@ -164,6 +164,9 @@ __device__ __forceinline__ void viscous_close(const DevP& P, const double c0[6],
 // One thread issues the TMA copies after a split barrier (bar.arrive by the other warps, bar.sync by
 // its warp), so no warp but that one waits for the slowest.  Completion is tracked by mbarriers.
 // ---------------------------------------------------------------------------------------------
+#ifndef STREAMS_MARCH_NSLOT
+#define STREAMS_MARCH_NSLOT 2
+#endif
 template <int TY, int NG, bool VISC, bool WENO>
 struct MarchSmem {
   using G = MarchGeom<TY, NG>;
@@ -172,8 +175,9 @@ struct MarchSmem {
   static constexpr size_t RING = (size_t)NF * G::NT * 8;       // one ring-plane slot
   static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[5]
   static constexpr size_t DFS = WENO ? (size_t)5 * G::NT * 8 : 0;
-  static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + 2 * RING, OFF_DFS = OFF_EPI + 2 * EPI,
-                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 32 + 8 * 32;   // 4 mbarriers, rate scratch
+  static constexpr int NSLOT = STREAMS_MARCH_NSLOT;            // ring-plane / RK-operand slots: loads run NSLOT - 1 planes ahead
+  static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + NSLOT * RING, OFF_DFS = OFF_EPI + NSLOT * EPI,
+                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 64 + 8 * 32;   // 2 + NSLOT mbarriers, rate scratch
   static_assert(BUF % 128 == 0 && RING % 128 == 0 && EPI % 128 == 0, "TMA destinations are 128-byte aligned");
   static_assert(TOTAL <= 227 * 1024, "shared memory of one block");
 };
@@ -181,10 +185,11 @@ struct MarchSmem {
 #ifndef STREAMS_MARCH_MINB
 #define STREAMS_MARCH_MINB 1
 #endif
-template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY, int NG>
+template <int L, int LV, bool VISC, bool CONV, bool WENO, bool UPD, int TY, int NG>
 __global__ void __launch_bounds__(MTX * TY, STREAMS_MARCH_MINB)
 rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
-                 const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r, const DevP P,
+                 const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r,
+                 const DevP P,
                  const StageArgs sa, int nbx, int nby, int kz) {
   using G = MarchGeom<TY, NG>;
   using SM = MarchSmem<TY, NG, VISC, WENO>;
@@ -192,12 +197,13 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   static_assert(L <= NG && LV <= NG, "ring depth");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][NF][PLANE]
-  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][NF][NT]
-  double* const epi = reinterpret_cast<double*>(smem_raw + SM::OFF_EPI);    // [2][10][NT]
+  constexpr int NSLOT = SM::NSLOT;
+  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [NSLOT][NF][NT]
+  double* const epi = reinterpret_cast<double*>(smem_raw + SM::OFF_EPI);    // [NSLOT][10][NT]
   double* const dfs = reinterpret_cast<double*>(smem_raw + SM::OFF_DFS);    // [5][NT]
   unsigned long long* const bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
   unsigned long long* const full_c = bars;        // [2] centre plane landed
-  unsigned long long* const full_e = bars + 2;    // [2] ring plane + RK operands landed
+  unsigned long long* const full_e = bars + 2;    // [NSLOT] ring plane + RK operands landed
 
   const int tid = threadIdx.x;
   const int tx = tid & 31, ty = tid >> 5;
@@ -216,7 +222,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const int s0 = (ty + NG) * G::ROW + tx + 4;          // this node in a shared-memory plane
 
   const unsigned bytes_c = (unsigned)SM::BUF;
-  const unsigned bytes_e = (unsigned)SM::RING + (sa.update_w ? 5u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
+  const unsigned bytes_e = (unsigned)SM::RING + (UPD ? 5u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
   const int cx0 = i0 + P.ox, cy0 = j0 + NG;            // tile origin in padded coordinates
 
   auto issue_centre = [&](int k, int b) {              // thread 0 only
@@ -227,7 +233,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     mbar_expect_tx(&full_e[b], bytes_e);
     tma_load_4d(ring + (size_t)b * NF * G::NT, &tm_ring, &full_e[b], cx0, cy0, k + NG + 1 + NG, 0);
     if (sa.read_prev) tma_load_4d(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + NG, 0);
-    if (sa.update_w) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + NG, 0);
+    if (UPD) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + NG, 0);
   };
 
 #ifndef STREAMS_MARCH_PF
@@ -245,21 +251,24 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     if (PF > 0 && k < ke) {
       tma_prefetch_4d(&tm_ring, cx0, cy0, k + NG + 1 + NG, 0);
       if (sa.read_prev) tma_prefetch_4d(&tm_r, cx0, cy0, k + NG, 0);
-      if (sa.update_w) tma_prefetch_4d(&tm_w, cx0, cy0, k + NG, 0);
+      if (UPD) tma_prefetch_4d(&tm_w, cx0, cy0, k + NG, 0);
     }
   };
   if (tid == 0) {
     mbar_init(&full_c[0], 1); mbar_init(&full_c[1], 1);
-    mbar_init(&full_e[0], 1); mbar_init(&full_e[1], 1);
+#pragma unroll
+    for (int a = 0; a < NSLOT; ++a) mbar_init(&full_e[a], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   if (tid == 0) {
     issue_centre(kb, 0);
     if (kb + 1 < ke) issue_centre(kb + 1, 1);
-    issue_ring_epi(kb, 0);
 #pragma unroll
-    for (int a = 1; a <= PF; ++a) prefetch_ring_epi(kb + a);
+    for (int a = 0; a < NSLOT - 1; ++a)
+      if (kb + a < ke) issue_ring_epi(kb + a, a);
+#pragma unroll
+    for (int a = 1; a <= PF; ++a) prefetch_ring_epi(kb + NSLOT - 2 + a);
   }
 
   // metrics of this row (constant along the march)
@@ -272,7 +281,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     ym.eyy = P.eta_yy_v[min(j, P.ny - 1)];
   }
   const double sb2 = fma(-2.0 * P.sbv, ym.eyv2, P.sb2xz);
-  const double dt = sa.update_w ? P.scal[S_DT] : 0.0;
+  const double dt = UPD ? P.scal[S_DT] : 0.0;
 
   // ring = planes kb-NG .. kb+NG of this thread's column
   double zr[NF][2 * NG + 1];
@@ -290,17 +299,54 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   unsigned fl_next = 0;
   if (WENO && CONV && active) fl_next = ld_u8_now(P.nflag + ncol + (long long)kb * P.sz);
 
+  // a2 / a1 / a9 of the next stage for the node just updated (state wn of plane kk): its primitives go to the other q
+  // buffer (stencils of this stage still read the current one), also at the node's periodic images in the ghost layers
+  // (the owner writes them; the next stage only fills the non-periodic ghost shell), then the time-step rate and the
+  // finiteness check of the last stage.  DEFER: evaluated one plane late, inside the stencil phase of the next plane,
+  // so that its long dependent chain (reciprocal, square roots, Newton steps) overlaps the wide stencil arithmetic
+  // instead of running alone between two barriers.
+#ifndef STREAMS_MARCH_DEFER
+#define STREAMS_MARCH_DEFER 1
+#endif
+  constexpr bool DEFER = STREAMS_MARCH_DEFER != 0;
+  double wn[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
+  // (no branch around the arithmetic: `ok` only predicates the stores, so the chain sits in the stencil phase's block)
+  auto finish_node = [&](int kk, bool ok) {
+    double mu, cc, vel[3], o[NQ];
+    prims_from_state<VISC, WENO>(P, wn, sa.want_rate != 0, o, mu, cc, vel);
+    double* __restrict__ qo = sa.q_out + (ncol + kk * isz);
+    if (ok) store_prims<VISC, WENO>(P, qo, o);
+    const int zoff = !P.own_z ? 0 : (kk < NG ? P.nz * isz : (kk >= P.nz - NG ? -P.nz * isz : 0));
+    if (ok && xoff) store_prims<VISC, WENO>(P, qo + xoff, o);
+    if (ok && yoff) store_prims<VISC, WENO>(P, qo + yoff, o);
+    if (ok && zoff) store_prims<VISC, WENO>(P, qo + zoff, o);
+    if (ok && sa.want_rate) {                                // fmax drops a NaN operand: test the rate before the max
+      const double rr = dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc);
+      bad |= !(rr == rr);
+      rate = fmax(rate, rr);
+    }
+    if (ok && sa.check_state)                          // the step's last stage: Inf or NaN anywhere in the new state
+      bad |= !(fabs((wn[0] + wn[1]) + (wn[2] + wn[3]) + wn[4]) <= 1.7976931348623157e308);
+  };
+
   for (int k = kb; k < ke; ++k) {
     const int it = k - kb, b = it & 1;
     const unsigned par = (unsigned)(it >> 1) & 1u;
+    const int se = it % NSLOT;                            // ring / RK-operand slot of this plane
+    const unsigned par_e = (unsigned)(it / NSLOT) & 1u;
     const int n = ncol + k * isz;
-    if (tid == G::NT - 32) prefetch_ring_epi(k + 1 + PF);   // no shared-memory hazard: any thread, off the issuing warp's path
+    if (tid == G::NT - 32) prefetch_ring_epi(k + NSLOT - 1 + PF);   // no shared-memory hazard: any thread, off the issuing warp's path
     // does this node have a net WENO correction (an adjacent flagged interface)?  Flags of this plane were
     // prefetched, the next plane's are requested now; the five values are staged while the stencils run
     bool fl = false, any_fl = false;
     if (WENO) {
+      unsigned fl_new = 0;
+      if (CONV && active && k + 1 < ke) fl_new = ld_u8_now(P.nflag + n + isz);
+      // the byte loaded one plane ago is consumed only here: without this fence the compiler tests the byte it has
+      // just requested (and carries the predicate), which stalls every plane on the load
+      asm volatile("" : "+r"(fl_next));
       fl = CONV ? (fl_next != 0) : active;
-      if (CONV && active && k + 1 < ke) fl_next = ld_u8_now(P.nflag + n + isz);
+      fl_next = fl_new;
       any_fl = __any_sync(0xffffffffu, fl);
       if (any_fl) {
 #pragma unroll
@@ -310,6 +356,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
 
     // (C) the right-hand side of this node
     mbar_wait(&full_c[b], par);
+    if (DEFER && UPD) finish_node(k - 1, active && it > 0);
     const double* __restrict__ sc = buf + (size_t)b * NF * G::PLANE + s0;
     auto gx = [&](int f, int o2) { return sc[f * G::PLANE + o2]; };
     auto gy = [&](int f, int o2) { return sc[f * G::PLANE + o2 * G::ROW]; };
@@ -322,6 +369,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     for (int l = 0; l < 4; ++l) alr[l] = P.kc[l] * c0[F_RHO];
     double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     Visc V;
+#ifndef STREAMS_MARCH_SKELETON
     if (VISC) {
       double gT[3], lapT = 0.0;
       scalar_terms<0, LV>(P, gx, ym, gT, lapT, V);
@@ -335,12 +383,18 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       V.vm[0] = V.vm[1] = V.vm[2] = 0.0;
       V.dv = 0.0; V.ph = 0.0;
     }
+#endif
+#ifdef STREAMS_MARCH_SKELETON   // measurement build: the kernel's data movement without its stencil arithmetic
+    r[0] = gx(0, 1) + gy(1, -1); r[1] = gz(2, 1) + c0[3]; r[2] = gx(4, -2); r[3] = gy(5, 2); r[4] = gz(VISC ? 8 : 0, -3) + gx(VISC ? 7 : 1, 3) + gy(VISC ? 6 : 2, 3);
+#else
     dir_terms<0, L, LV, CONV, VISC>(P, gx, ym, c0, alr, r, V);
     dir_terms<1, L, LV, CONV, VISC>(P, gy, ym, c0, alr, r, V);
     dir_terms<2, L, LV, CONV, VISC>(P, gz, ym, c0, alr, r, V);
     if (VISC) viscous_close(P, c0, zr[VISC ? F_MU : 0][NG], sb2, r, V);
+#endif
 
-    // every warp is done with buf[b], ring[b^1], epi[b^1]: the issuing thread refills them
+    // every warp is done with buf[b] and with the ring / RK-operand slot of the previous plane: the issuing thread
+    // refills them
     // (two alternating barrier ids: a warp may run one iteration ahead of the slowest)
     if (tid >> 5) {
       if (b) asm volatile("bar.arrive 2, %0;" ::"n"(G::NT) : "memory");
@@ -349,14 +403,14 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
       else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
       if (tid == 0) {
-        if (k + 1 < ke) issue_ring_epi(k + 1, b ^ 1);   // needed one plane from now: ahead of the larger centre box
+        if (k + NSLOT - 1 < ke) issue_ring_epi(k + NSLOT - 1, (it + NSLOT - 1) % NSLOT);   // ahead of the larger centre box
         if (k + 2 < ke) issue_centre(k + 2, b);
       }
     }
 
     // (D) net correction of the flagged interfaces around the node, body force, RK update, stores
-    mbar_wait(&full_e[b], par);
-    const double* __restrict__ ep = epi + (size_t)b * 10 * G::NT + tid;
+    mbar_wait(&full_e[se], par_e);
+    const double* __restrict__ ep = epi + (size_t)se * 10 * G::NT + tid;
     if (WENO && any_fl) {
       cp_async_wait_all();
 #pragma unroll
@@ -368,38 +422,20 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       for (int a = 0; a < 3; ++a) r[1 + a] = fma(rho0, P.accel[a], r[1 + a]);
       r[4] = fma(rho0, fma(c0[F_U], P.accel[0], fma(c0[F_V], P.accel[1], c0[F_W] * P.accel[2])), r[4]);
     }
-    if (active) {
-      if (sa.update_w) {
-        double wn[5];
+    if (UPD) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          double inc = sa.gam * r[q];
-          if (sa.read_prev) inc = fma(sa.rhk, ep[q * G::NT], inc);
-          wn[q] = fma(dt, inc, ep[(5 + q) * G::NT]);
-          P.w[(long long)q * P.fs + n] = wn[q];
-        }
-        // a2 of the next stage: the primitives of the updated node go to the other q buffer (stencils of this
-        // stage still read the current one); the next stage only fills the ghost shell
-        double mu, cc, vel[3], o[NQ];
-        prims_from_state<VISC, WENO>(P, wn, sa.want_rate != 0, o, mu, cc, vel);
-        double* __restrict__ qo = sa.q_out + n;
-        store_prims<VISC, WENO>(P, qo, o);
-        // a1 of the next stage for the periodic directions: the owner also writes its images in the ghost layers
-        const int zoff = !P.own_z ? 0 : (k < NG ? P.nz * isz : (k >= P.nz - NG ? -P.nz * isz : 0));
-        if (xoff) store_prims<VISC, WENO>(P, qo + xoff, o);
-        if (yoff) store_prims<VISC, WENO>(P, qo + yoff, o);
-        if (zoff) store_prims<VISC, WENO>(P, qo + zoff, o);
-        if (sa.want_rate) {                            // fmax drops a NaN operand: test the rate before the max
-          const double rr = dt_rate<VISC>(P, vel, cc, mu, wn[0], ym.eyc);
-          bad |= !(rr == rr);
-          rate = fmax(rate, rr);
-        }
-        if (sa.check_state)                            // the step's last stage: Inf or NaN anywhere in the new state
-          bad |= !(fabs((wn[0] + wn[1]) + (wn[2] + wn[3]) + wn[4]) <= 1.7976931348623157e308);
+      for (int q = 0; q < 5; ++q) {
+        double inc = sa.gam * r[q];
+        if (sa.read_prev) inc = fma(sa.rhk, ep[q * G::NT], inc);
+        wn[q] = fma(dt, inc, ep[(5 + q) * G::NT]);
+        if (active) st_out(P.w + (long long)q * P.fs + n, wn[q]);
       }
+      if (!DEFER) finish_node(k, active);
+    }
+    if (active) {
       if (sa.write_r) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) P.R[(long long)q * P.fs + n] = r[q];
+        for (int q = 0; q < 5; ++q) st_out(P.R + (long long)q * P.fs + n, r[q]);
       }
       if (sa.r_dense) {
         const long long o = ((long long)k * P.ny + j) * P.nx + i;
@@ -409,7 +445,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     }
 
     // (E) shift the ring
-    const double* __restrict__ rn = ring + (size_t)b * NF * G::NT + tid;
+    const double* __restrict__ rn = ring + (size_t)se * NF * G::NT + tid;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
 #pragma unroll
@@ -417,21 +453,22 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       zr[f][2 * NG] = rn[f * G::NT];
     }
   }
+  if (DEFER && UPD) finish_node(ke - 1, active);
   if (bad) P.scal[S_NAN] = 1.0;                       // streams_step returns STREAMS_ENAN
   // a9 of the next step: one atomicMax per block on the bit pattern of the largest rate (a NaN wins)
   if (sa.want_rate) {
     if (bad) rate = __longlong_as_double(0x7ff8000000000000LL);
-    block_rate_max(P, rate, bars + 4);
+    block_rate_max(P, rate, bars + 8);
   }
 }
 
 // -------------------------------------------------------------------------- launch
 // configure: only opt the instantiation in to its dynamic shared memory on the current device (streams_init).
-template <int L, int LV, bool VISC, bool CONV, bool WENO, int TY, int NG>
+template <int L, int LV, bool VISC, bool CONV, bool WENO, bool UPD, int TY, int NG>
 static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa, cudaStream_t st, bool configure) {
   using G = MarchGeom<TY, NG>;
   using SM = MarchSmem<TY, NG, VISC, WENO>;
-  auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, TY, NG>;
+  auto kern = rhs_march_kernel<L, LV, VISC, CONV, WENO, UPD, TY, NG>;
   if (configure)
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) == cudaSuccess ? 0 : -2;
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
@@ -448,7 +485,16 @@ static int launch_main_T(const DevP& P, const MarchMaps& mp, const StageArgs& sa
   const bool conv = P.flux_mode != FLUX_WENO;
   const bool weno = P.flux_mode != FLUX_CENTRAL;
   constexpr int TY = STREAMS_MARCH_TY;
-#define STREAMS_MAIN(V, C, W) return launch_march<M, M, V, C, W, TY, NG>(P, mp, sa, st, configure)
+#define STREAMS_MAIN(V, C, W)                                                                              \
+  do {                                                                                                     \
+    if (configure) {                                                                                       \
+      const int a = launch_march<M, M, V, C, W, true, TY, NG>(P, mp, sa, st, true);                        \
+      const int b = launch_march<M, M, V, C, W, false, TY, NG>(P, mp, sa, st, true);                       \
+      return (a | b) ? -2 : 0;                                                                             \
+    }                                                                                                      \
+    if (sa.update_w) return launch_march<M, M, V, C, W, true, TY, NG>(P, mp, sa, st, false);               \
+    return launch_march<M, M, V, C, W, false, TY, NG>(P, mp, sa, st, false);                               \
+  } while (0)
   if (visc && conv && weno) STREAMS_MAIN(true, true, true);
   else if (visc && conv) STREAMS_MAIN(true, true, false);
   else if (visc) STREAMS_MAIN(true, false, true);
@@ -461,6 +507,9 @@ static int launch_main_T(const DevP& P, const MarchMaps& mp, const StageArgs& sa
 // TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point: libstreams does not link
 // libcuda).  All four tensors are 4-D (x, y, z, field) views of padded fields: the primitives + dilatation
 // (DevP::q, NF fields), w and R (5 fields each).
+#ifndef STREAMS_TMA_L2_PROMOTION
+#define STREAMS_TMA_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
 int make_march_maps(const DevP& P, MarchMaps* maps) {
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -479,7 +528,7 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
     const cuuint64_t dims[4] = {(cuuint64_t)P.px, (cuuint64_t)P.py, (cuuint64_t)P.pz, nfields};
     const cuuint32_t box[4] = {bx, by, 1, bf};
     return encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                  CU_TENSOR_MAP_SWIZZLE_NONE, STREAMS_TMA_L2_PROMOTION, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   };
   const cuuint32_t halo = 2 * (cuuint32_t)P.ng;        // MarchGeom<TY, NG>::ROW / ROWS with NG = DevP::ng
   if (make(&maps->centre, P.q, nf, MTX + 8, TY + halo, nf) != CUDA_SUCCESS) return -2;
@@ -501,10 +550,15 @@ int march_family(int L, int Lv, int ng) { return ng == 4 ? 4 : (L > Lv ? L : Lv)
 int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, const StageArgs& sa, cudaStream_t st, bool configure) {
   const int m = march_family(P.flux_mode != FLUX_WENO ? L : 1, P.visc_law != VISC_NONE ? Lv : 1, P.ng);
   if (m < 1 || m > 4 || (P.ng != 3 && P.ng != 4)) return -1;
+#ifdef STREAMS_ONLY_FAMILY3                            // development builds: the production family only
+  if (m != 3) return -1;
+  return launch_main_T<3, 3>(P, mp, sa, st, configure);
+#else
   if (m == 1) return launch_main_T<1, 3>(P, mp, sa, st, configure);
   if (m == 2) return launch_main_T<2, 3>(P, mp, sa, st, configure);
   if (m == 3) return launch_main_T<3, 3>(P, mp, sa, st, configure);
   return launch_main_T<4, 4>(P, mp, sa, st, configure);
+#endif
 }
 
 }  // namespace streams

@@ -23,6 +23,20 @@ __device__ __forceinline__ void cp_async8_zfill(void* smem_dst, const void* gsrc
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(n) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// 16 bytes (L2 only) when `take`, zeros otherwise; both addresses 16-byte aligned
+__device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool take) {
+  const unsigned n = take ? 16u : 0u;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// waits until at most N of this thread's most recent commit groups are still pending
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// this thread's arrival on `bar` (counted in the barrier's init count), performed when all its earlier cp.async have
+// landed; earlier shared-memory stores of the thread are ordered before it too
+__device__ __forceinline__ void cp_async_mbar_arrive(unsigned long long* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 // a load the compiler may not sink to its first use
 __device__ __forceinline__ unsigned ld_u8_now(const unsigned char* p) {
   unsigned v;

@@ -358,43 +358,48 @@ __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_list_kernel(const 
 // ---------------------------------------------------------------------------------------------
 // corr_gather_kernel: the net correction of a node, corr_q(n) = sum_d metric_d (dF_d,q(n) - dF_d,q(n - e_d)) over the
 // flagged interfaces around it (hybrid: the bits of DevP::nflag, bit 2d = minus side, 2d+1 = plus side; full WENO:
-// all six), directions in the order x, y, z.  One thread per 8 consecutive x nodes: the 8 flag bytes are one 64-bit
-// load, and a thread whose word is zero is done (most of the grid in hybrid mode).  dF holds stale values at
-// interfaces that are not flagged: they are never read.  HBM: 1 B per node + (<= 30 R + 5 W) x 8 B per flagged node.
+// all six), directions in the order x, y, z.  dF holds stale values at interfaces that are not flagged: they are
+// never read.  HBM: 1 B per node + (<= 30 R + 5 W) x 8 B per flagged node.
 // ---------------------------------------------------------------------------------------------
-template <bool DENSE>
-__global__ void __launch_bounds__(256) corr_gather_kernel(const DevP P, int nwx) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= (long long)nwx * P.ny * P.nz) return;
-  const int iw = (int)(t % nwx);
-  const long long t2 = t / nwx;
-  const int j = (int)(t2 % P.ny), k = (int)(t2 / P.ny);
-  const int i0 = iw * 8;
-  const long long n0 = pidx(P, i0, j, k);
-  unsigned long long word = DENSE ? 0x3f3f3f3f3f3f3f3full : *reinterpret_cast<const unsigned long long*>(P.nflag + n0);
-  const int nvalid = min(8, P.nx - i0);
-  if (nvalid < 8) word &= (1ull << (8 * nvalid)) - 1ull;
-  if (word == 0ull) return;
-  const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+__device__ __forceinline__ void corr_node(const DevP& P, long long n, unsigned fl, const double met[3]) {
   const long long st[3] = {1, P.sy, P.sz};
-  for (int b = 0; b < nvalid; ++b) {
-    const unsigned fl = (unsigned)(word >> (8 * b)) & 0x3fu;
-    if (!fl) continue;
-    const long long n = n0 + b;
-    double c[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  double c[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+  for (int d = 0; d < 3; ++d) {
+    const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+    const bool hp = (fl >> (2 * d + 1)) & 1u, hm = (fl >> (2 * d)) & 1u;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) {
-        const double fp = ((fl >> (2 * d + 1)) & 1u) ? f[q * P.fs] : 0.0;
-        const double fm = ((fl >> (2 * d)) & 1u) ? f[q * P.fs - st[d]] : 0.0;
-        c[q] = fma(met[d], fp - fm, c[q]);
-      }
+    for (int q = 0; q < 5; ++q) {
+      const double fp = hp ? f[q * P.fs] : 0.0;
+      const double fm = hm ? f[q * P.fs - st[d]] : 0.0;
+      c[q] = fma(met[d], fp - fm, c[q]);
     }
-#pragma unroll
-    for (int q = 0; q < 5; ++q) P.corr[q * P.fs + n] = c[q];
   }
+#pragma unroll
+  for (int q = 0; q < 5; ++q) P.corr[q * P.fs + n] = c[q];
+}
+
+// full-WENO mode: every node, one thread each
+__global__ void __launch_bounds__(128) corr_gather_dense_kernel(const DevP P) {
+  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= P.nx) return;
+  const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+  corr_node(P, pidx(P, i, j, k), 0x3fu, met);
+}
+
+// hybrid mode: one thread per node, x fastest (the flag bytes of a warp are one 32-byte segment), 128 nodes of a row
+// per block (measured: larger blocks and persistent row-walking blocks are 1.4-3x slower); a thread whose byte is
+// zero is done (most of the grid).  Flagged nodes come in clusters, so the warps that
+// have work are mostly full and their loads coalesced; the many resident threads hide the latency of the gather.
+// HBM: 1 B per node + the flagged nodes' values.
+__global__ void __launch_bounds__(128) corr_gather_kernel(const DevP P) {
+  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= P.nx) return;
+  const long long n = pidx(P, i, j, k);
+  const unsigned fl = P.nflag[n];
+  if (!fl) return;
+  const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+  corr_node(P, n, fl, met);
 }
 
 // -------------------------------------------------------------------------- launch
@@ -407,11 +412,13 @@ static int launch_weno_T(const DevP& P, cudaStream_t st) {
 
 int launch_corr(const DevP& P, cudaStream_t st) {
   if (P.flux_mode == FLUX_CENTRAL) return 0;
-  const int nwx = (P.nx + 7) / 8;
-  const long long nwords = (long long)nwx * P.ny * P.nz;
-  dim3 b(256), g((unsigned)((nwords + 255) / 256));
-  if (P.flux_mode == FLUX_HYBRID) corr_gather_kernel<false><<<g, b, 0, st>>>(P, nwx);
-  else corr_gather_kernel<true><<<g, b, 0, st>>>(P, nwx);
+  if (P.flux_mode == FLUX_HYBRID) {
+    dim3 b(128), g((unsigned)((P.nx + 127) / 128), (unsigned)P.ny, (unsigned)P.nz);
+    corr_gather_kernel<<<g, b, 0, st>>>(P);
+  } else {
+    dim3 b(128), g((unsigned)((P.nx + 127) / 128), (unsigned)P.ny, (unsigned)P.nz);
+    corr_gather_dense_kernel<<<g, b, 0, st>>>(P);
+  }
   return 1;
 }
 
