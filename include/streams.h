@@ -158,8 +158,12 @@ int streams_set_body_force(streams_ctx* ctx, const double* accel3);
 enum { STREAMS_SUM_STATE = 0, STREAMS_SUM_RESIDUAL = 1 };
 int streams_get_sums(streams_ctx* ctx, int kind, double* out5);
 
-/* Number of kernels the library has launched on this context since streams_init. */
+/* Number of kernels the library has launched on this context since streams_init (kernels replayed from a CUDA graph
+ * count one by one), and the number of graph submissions among them: streams_step captures the launches of one RK3
+ * step once per variant of its launch sequence and replays them afterwards (small grids cannot hide the
+ * launch latency).  Profiling (streams_profile) and the environment variable STREAMS_NO_GRAPH=1 switch the graphs off. */
 long long streams_kernel_launches(const streams_ctx* ctx);
+long long streams_graph_launches(const streams_ctx* ctx);
 
 /* Per-kernel device timing, the measurement of BASELINE metric part 2 ("per-kernel % of roofline";
  * the paper's analogue is its per-kernel table).  Kernel classes: */

@@ -55,6 +55,8 @@ def load(kind: str = "omp"):
         lib.oracle_get_fields.argtypes = [C.c_void_p, _c_double_p]
         lib.oracle_rhs.argtypes = [C.c_void_p, C.c_int, _c_double_p]
         lib.oracle_step.argtypes = [C.c_void_p, C.c_int, _c_double_p, _c_double_p]
+        lib.oracle_step_forced.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _c_double_p, _c_double_p, _c_double_p]
+        lib.oracle_bulk_sums.argtypes = [C.c_void_p, C.c_int, _c_double_p, _c_double_p]
         lib.oracle_compute_dt.restype = C.c_double
         lib.oracle_compute_dt.argtypes = [C.c_void_p]
         lib.oracle_get_sensor.argtypes = [C.c_void_p, _c_double_p, _c_ubyte_p, _c_double_p]
@@ -143,6 +145,21 @@ class Oracle:
         if rc:
             raise RuntimeError(f"oracle_step rc={rc}")
         return dt.value, t.value
+
+    def step_forced(self, nsteps: int, direction: int = 0, target: float = float("nan")):
+        """nsteps steps under the bulk-flow controller (S18); returns (dt, time, [g_x, g_y, g_z])."""
+        dt, t = C.c_double(), C.c_double()
+        g = (C.c_double * 3)()
+        rc = self.lib.oracle_step_forced(self.h, nsteps, direction, C.c_double(target), C.byref(dt), C.byref(t),
+                                         C.cast(g, _c_double_p))
+        if rc:
+            raise RuntimeError(f"oracle_step_forced rc={rc}")
+        return dt.value, t.value, list(g)
+
+    def bulk_sums(self, direction: int = 0):
+        m, p = C.c_double(), C.c_double()
+        self.lib.oracle_bulk_sums(self.h, direction, C.byref(m), C.byref(p))
+        return m.value, p.value
 
     def compute_dt(self):
         return self.lib.oracle_compute_dt(self.h)

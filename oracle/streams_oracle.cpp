@@ -34,6 +34,8 @@
 //                        manufactured Navier-Stokes terms with n = 0.76 at design order
 //   S17 body force     : uniform state => R = (0, rho g, rho u.g) exactly; momentum budget of a periodic box;
 //                        Poiseuille flow driven by g instead of a pressure gradient
+//   S18 flow control   : deadbeat on a frictionless uniform flow (P reaches its target in one step and stays), holds
+//                        a laminar channel against its wall friction
 // Unpinned against the real STREAmS code (not in the container): S1, S2, S4, S5,
 // S6, S7, S8, S9, S10, S12, S13, S15, S16 -- "parity unpinned vs STREAmS"; the
 // oracle's reading is the definition for this build.
@@ -812,6 +814,51 @@ struct Solver {
     }
     return 0;
   }
+
+  // ---------------------------------------------------------------------------
+  // S18 bulk-flow control of a forced channel ("forcing term evaluations (sum reduction)"
+  // force_rhs): after every step the volume integrals M = sum rho dV and P = sum (rho u_d) dV are taken
+  // (dV = dx dz / eta_y(j), nodes in index order) and the uniform acceleration along d is reset so that P returns to
+  // its target over the next step: a force g acting for dt changes P by g M dt, hence
+  //   g <- [g - (P - P_prev) / (M dt)] + (P_target - P) / (M dt),
+  // the first bracket being the force that would have kept P constant over the step just taken (the running estimate
+  // of the wall friction).  The paper prints no controller formula: this reading is pinned by its defining property
+  // (deadbeat on a frictionless uniform flow, tests/test_oracle_force.py), not against STREAmS.
+  // ---------------------------------------------------------------------------
+  bool ctrl_started = false;
+  double ctrl_prev = 0.0, ctrl_target = 0.0;
+  void bulk_sums(int d, double& mass, double& mom) const {
+    mass = 0.0; mom = 0.0;
+    const double dxdz = 1.0 / (inv_dx * inv_dz);
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          const size_t n = idx(i, j, k);
+          const double dV = dxdz / eta_y_c[j];
+          mass += w[0][n] * dV;
+          mom += w[1 + d][n] * dV;
+        }
+  }
+  int step_forced(int nsteps, int d, double target) {
+    double mass, mom;
+    if (!ctrl_started) {
+      bulk_sums(d, mass, mom);
+      ctrl_prev = mom;
+      ctrl_target = std::isnan(target) ? mom : target;
+      ctrl_started = true;
+    } else if (!std::isnan(target)) {
+      ctrl_target = target;
+    }
+    for (int s = 0; s < nsteps; ++s) {
+      const int rc = step(1);
+      if (rc) return rc;
+      bulk_sums(d, mass, mom);
+      const double g_balance = P.accel[d] - (mom - ctrl_prev) / (mass * dt);
+      P.accel[d] = g_balance + (ctrl_target - mom) / (mass * dt);
+      ctrl_prev = mom;
+    }
+    return 0;
+  }
 };
 
 }  // namespace
@@ -871,6 +918,19 @@ int oracle_step(void* h, int nsteps, double* dt_last, double* time) {
   return rc;
 }
 double oracle_compute_dt(void* h) { return static_cast<Solver*>(h)->compute_dt(); }
+// S18: nsteps steps under the bulk-flow controller along direction d; target NaN = hold the current bulk momentum.
+// accel3_out (nullable) receives the acceleration after the last update.
+int oracle_step_forced(void* h, int nsteps, int d, double target, double* dt_last, double* time, double* accel3_out) {
+  Solver* s = static_cast<Solver*>(h);
+  if (!s->have_fields) return -4;
+  if (d < 0 || d > 2) return -1;
+  const int rc = s->step_forced(nsteps, d, target);
+  if (dt_last) *dt_last = s->dt;
+  if (time) *time = s->time;
+  if (accel3_out) for (int a = 0; a < 3; ++a) accel3_out[a] = s->P.accel[a];
+  return rc;
+}
+void oracle_bulk_sums(void* h, int d, double* mass, double* mom) { static_cast<Solver*>(h)->bulk_sums(d, *mass, *mom); }
 
 // theta / mask / div of the last rhs() (interior, [nz][ny][nx]).
 int oracle_get_sensor(void* h, double* theta_out, unsigned char* mask_out, double* div_out) {

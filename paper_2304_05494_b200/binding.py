@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
 STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
            "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
-           "streams_kernel_launches",
+           "streams_kernel_launches", "streams_graph_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
            "streams_measure_fp64_scratch_bytes",
            "streams_last_error", "streams_destroy")
@@ -76,6 +76,8 @@ def load_library(path: str = LIB_PATH):
     lib.streams_get_activation_totals.argtypes = [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4
     lib.streams_kernel_launches.restype = C.c_longlong
     lib.streams_kernel_launches.argtypes = [C.c_void_p]
+    lib.streams_graph_launches.restype = C.c_longlong
+    lib.streams_graph_launches.argtypes = [C.c_void_p]
     lib.streams_profile.argtypes = [C.c_void_p, C.c_int, C.c_int]
     lib.streams_get_profile.argtypes = [C.c_void_p, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.streams_measure_fp64_scratch_bytes.restype = C.c_size_t
@@ -154,7 +156,10 @@ class Streams:
             raise StreamsError(STREAMS_EINVAL, self.lib.streams_last_error(None).decode())
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # a stream of the context's own unless the caller brings one: the legacy default stream cannot be captured
+            # into the CUDA graphs streams_step replays.  Device tensors that cross this boundary are ordered against
+            # torch's current stream explicitly (_after_torch / _before_torch).
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         ptr = (self.workspace.data_ptr() + 255) // 256 * 256
         h = C.c_void_p()
         rc = self.lib.streams_init(C.byref(h), C.byref(g), C.byref(a), C.byref(s), C.c_void_p(ptr), nbytes,
@@ -180,19 +185,31 @@ class Streams:
         assert x.is_contiguous()
         return C.c_void_p(x.data_ptr()), int(x.is_cuda)
 
+    def _after_torch(self):
+        """The library's stream waits for what torch has enqueued (a device tensor is about to be read)."""
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))
+
+    def _before_torch(self):
+        """torch's current stream waits for the library's (a device tensor has just been written)."""
+        self.torch.cuda.current_stream(self.device).wait_stream(self.stream)
+
     # -- C ABI
     def set_fields(self, w):
         if isinstance(w, np.ndarray):
             w = np.ascontiguousarray(w, dtype=np.float64)
         assert tuple(w.shape) == (5,) + self.shape
         p, dev = self._ptr(w)
+        if dev:
+            self._after_torch()
         self._check(self.lib.streams_set_fields(self.h, p, dev))
 
     def rhs(self, out=None):
         if out is None:
             out = self.torch.empty((5,) + self.shape, dtype=self.torch.float64, device=self.device)
         assert out.is_cuda
+        self._after_torch()
         self._check(self.lib.streams_rhs(self.h, C.c_void_p(out.data_ptr())))
+        self._before_torch()
         return out
 
     def step(self, nsteps):
@@ -204,7 +221,11 @@ class Streams:
         if out is None:
             out = np.empty((5,) + self.shape, dtype=np.float64)
         p, dev = self._ptr(out)
+        if dev:
+            self._after_torch()
         self._check(self.lib.streams_get_fields(self.h, p, dev))
+        if dev:
+            self._before_torch()
         return out
 
     def get_sensor(self):
@@ -222,6 +243,8 @@ class Streams:
             mask = np.ascontiguousarray(mask, dtype=np.uint8)
         assert tuple(mask.shape) == self.shape
         p, dev = self._ptr(mask)
+        if dev:
+            self._after_torch()
         self._check(self.lib.streams_set_mask_override(self.h, p, dev))
 
     def set_body_force(self, accel):
@@ -250,6 +273,9 @@ class Streams:
 
     def kernel_launches(self):
         return int(self.lib.streams_kernel_launches(self.h))
+
+    def graph_launches(self):
+        return int(self.lib.streams_graph_launches(self.h))
 
     def profile(self, enable=True, max_records=0):
         self._check(self.lib.streams_profile(self.h, int(bool(enable)), int(max_records)))

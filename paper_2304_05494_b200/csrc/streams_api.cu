@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -136,6 +137,12 @@ struct streams_ctx {
   double prof_ms[STREAMS_K_COUNT];
   long long prof_n[STREAMS_K_COUNT];
   long long prof_dropped;
+  // CUDA graphs of one RK3 step (streams_step): the launches of a step are captured once per variant
+  // (primitive buffer the step starts from, dt recomputed at its start, rate reduced at its end) and replayed
+  bool graphs_on;
+  cudaGraphExec_t step_graph[8];
+  int step_graph_launches[8];
+  long long graph_launches;
 };
 
 namespace {
@@ -266,6 +273,13 @@ void use_qbuf(streams_ctx* ctx, int b) {
   ctx->P.div = ctx->qbuf[b] + (size_t)Q_DIV * ctx->S.fs;
 }
 
+void drop_step_graphs(streams_ctx* ctx) {            // kernel arguments baked into the graphs have changed
+  for (int g = 0; g < 8; ++g) {
+    if (ctx->step_graph[g]) cudaGraphExecDestroy(ctx->step_graph[g]);
+    ctx->step_graph[g] = nullptr;
+  }
+}
+
 // the RHS (+ update) of one stage: the WENO flux corrections of the flagged interfaces first (they read the
 // primitives only), then the fused central / viscous / correction / update pass over all nodes
 int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
@@ -278,6 +292,28 @@ int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   }
   const int a = timed(ctx, STREAMS_K_RHS_MAIN, [&] { return launch_rhs_main(P, ctx->maps[ctx->cur], ctx->S.L, ctx->S.Lv, sa, st, false); });
   return a < 0 ? a : (b < 0 ? b : (c < 0 ? c : a + b + c));
+}
+
+// the launches of one RK3 step: three stages of (ghost fill, step scalars, sensor, flags, WENO, gather, fused RHS + update)
+int enqueue_step(streams_ctx* ctx, bool want_dt, bool want_rate) {
+  // Wray's low-storage RK3 (DESIGN.md O5 / S12)
+  const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+  const double rhk[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+  for (int l = 0; l < 3; ++l) {
+    int rc = enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
+    if (rc < 0) return rc;
+    StageArgs sa;
+    sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
+    sa.r_dense = nullptr;
+    sa.q_out = ctx->qbuf[ctx->cur ^ 1];
+    sa.want_rate = (l == 2 && want_rate) ? 1 : 0;
+    sa.check_state = (l == 2);
+    if ((rc = enqueue_rhs(ctx, sa)) < 0) return rc;
+    use_qbuf(ctx, ctx->cur ^ 1);                     // the updated state's primitives are in the other buffer
+    ctx->prims_interior = true;
+    if (sa.want_rate) ctx->rate_ready = true;
+  }
+  return 0;
 }
 
 }  // namespace
@@ -310,6 +346,12 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   ctx->base = (char*)workspace_dev;
   ctx->have_fields = false; ctx->step_count = 0; ctx->launches = 0; ctx->err[0] = 0;
   ctx->prof_on = false; ctx->prof_used = 0; ctx->prof_dropped = 0;
+  {
+    const char* ng = std::getenv("STREAMS_NO_GRAPH");   // debugging aid: launch every kernel of a step individually
+    ctx->graphs_on = !(ng && ng[0] && ng[0] != '0');
+  }
+  for (int g = 0; g < 8; ++g) { ctx->step_graph[g] = nullptr; ctx->step_graph_launches[g] = 0; }
+  ctx->graph_launches = 0;
   for (int k = 0; k < STREAMS_K_COUNT; ++k) { ctx->prof_ms[k] = 0.0; ctx->prof_n[k] = 0; }
   if (ctx->scheme.dt_every < 1) ctx->scheme.dt_every = 1;
   DevP& P = ctx->P;
@@ -475,26 +517,52 @@ int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
   if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_step before streams_set_fields");
   if (nsteps < 0) return fail(ctx, STREAMS_EINVAL, "nsteps must be non-negative");
-  // Wray's low-storage RK3 (DESIGN.md O5 / S12)
-  const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
-  const double rhk[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
   if (nsteps > 0) ctx->r_valid = false;              // R becomes the low-storage scheme's previous-stage register
   for (int s = 0; s < nsteps; ++s) {
     const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
-    for (int l = 0; l < 3; ++l) {
-      int rc = enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
+    // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
+    const bool want_rate = !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0;
+    // A step whose launch sequence is the steady one (primitives of the state already in place, the rate for its dt
+    // already reduced) is replayed from a CUDA graph: the 10-16 launches of a step become one submission, which is
+    // what a small grid needs (grids below ~2 M points cannot hide the launch latency).
+    const bool steady = ctx->prims_interior && (!want_dt || ctx->scheme.dt_fixed > 0.0 || ctx->rate_ready);
+    if (ctx->graphs_on && !ctx->prof_on && steady) {
+      const int key = ctx->cur | (want_dt ? 2 : 0) | (want_rate ? 4 : 0);
+      if (!ctx->step_graph[key]) {
+        const long long l0 = ctx->launches;
+        const int cur0 = ctx->cur;
+        const bool rr0 = ctx->rate_ready;
+        if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+          cudaGetLastError();                          // e.g. the legacy default stream cannot be captured: launch directly
+          ctx->graphs_on = false;
+          const int rd = enqueue_step(ctx, want_dt, want_rate);
+          if (rd < 0) return launch_fail(ctx, rd);
+          ctx->step_count += 1;
+          continue;
+        }
+        const int rc = enqueue_step(ctx, want_dt, want_rate);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t ee = cudaStreamEndCapture(ctx->stream, &graph);
+        if (rc < 0) { if (graph) cudaGraphDestroy(graph); return launch_fail(ctx, rc); }
+        if (ee != cudaSuccess) return cuda_fail(ctx, ee, "cudaStreamEndCapture");
+        const cudaError_t ei = cudaGraphInstantiate(&ctx->step_graph[key], graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) { ctx->step_graph[key] = nullptr; return cuda_fail(ctx, ei, "cudaGraphInstantiate"); }
+        ctx->step_graph_launches[key] = (int)(ctx->launches - l0);
+        // nothing ran during the capture: rewind the host state it advanced, the replay below advances it again
+        ctx->launches = l0;
+        use_qbuf(ctx, cur0);
+        ctx->rate_ready = rr0;
+      }
+      CU(cudaGraphLaunch(ctx->step_graph[key], ctx->stream));
+      ctx->graph_launches += 1;
+      ctx->launches += ctx->step_graph_launches[key];
+      use_qbuf(ctx, ctx->cur ^ 1);                   // three stages, three swaps of the primitive buffers
+      if (want_dt) ctx->rate_ready = false;
+      if (want_rate) ctx->rate_ready = true;
+    } else {
+      const int rc = enqueue_step(ctx, want_dt, want_rate);
       if (rc < 0) return launch_fail(ctx, rc);
-      StageArgs sa;
-      sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
-      sa.r_dense = nullptr;
-      sa.q_out = ctx->qbuf[ctx->cur ^ 1];
-      // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
-      sa.want_rate = (l == 2 && !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0) ? 1 : 0;
-      sa.check_state = (l == 2);
-      if ((rc = enqueue_rhs(ctx, sa)) < 0) return launch_fail(ctx, rc);
-      use_qbuf(ctx, ctx->cur ^ 1);                   // the updated state's primitives are in the other buffer
-      ctx->prims_interior = true;
-      if (sa.want_rate) ctx->rate_ready = true;
     }
     ctx->step_count += 1;
   }
@@ -568,6 +636,7 @@ int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int s
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
   if (ctx->scheme.flux_mode != STREAMS_FLUX_HYBRID) return fail(ctx, STREAMS_EINVAL, "a node mask exists in hybrid mode only");
   DevP& P = ctx->P;
+  drop_step_graphs(ctx);
   if (!mask) { P.mask_ovr = nullptr; return STREAMS_OK; }
   unsigned char* dst = (unsigned char*)(ctx->base + ctx->S.off_movr);
   cudaMemcpy3DParms p;
@@ -591,6 +660,7 @@ int streams_set_body_force(streams_ctx* ctx, const double* accel3) {
     ctx->gas.accel[d] = accel3[d];
   }
   ctx->P.has_accel = accel3[0] != 0.0 || accel3[1] != 0.0 || accel3[2] != 0.0;
+  drop_step_graphs(ctx);
   ctx->r_valid = false;                              // R no longer is the right-hand side under the new force
   return STREAMS_OK;
 }
@@ -611,6 +681,7 @@ int streams_get_sums(streams_ctx* ctx, int kind, double* out5) {
 }
 
 long long streams_kernel_launches(const streams_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long long streams_graph_launches(const streams_ctx* ctx) { return ctx ? ctx->graph_launches : 0; }
 
 int streams_profile(streams_ctx* ctx, int enable, int max_records) {
   if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
@@ -662,6 +733,7 @@ const char* streams_last_error(const streams_ctx* ctx) { return ctx ? ctx->err :
 int streams_destroy(streams_ctx* ctx) {
   if (!ctx) return STREAMS_EINVAL;
   cudaStreamSynchronize(ctx->stream);
+  drop_step_graphs(ctx);
   for (cudaEvent_t ev : ctx->prof_pool) cudaEventDestroy(ev);
   delete ctx;
   return STREAMS_OK;

@@ -4,6 +4,7 @@ import numpy as np
 import pytest
 
 import workloads as W
+from tests import helpers
 from tests.helpers import field_err, natural_scales
 
 pytestmark = pytest.mark.gpu
@@ -28,10 +29,11 @@ def check_case(S, case, nsteps, tol_rhs=TOL_RHS, tol_step=TOL_STEP, expect_activ
     gpu = S(case)
     ora = _oracle(case)
     floor_w, floor_r = natural_scales(case)
+    hits0 = len(helpers.FLOOR_HITS)
     # one RHS
     r_gpu = gpu.rhs().cpu().numpy()
     r_ora = ora.rhs()
-    errs = [field_err(r_gpu[q], r_ora[q], floor_r[q]) for q in range(5)]
+    errs = [field_err(r_gpu[q], r_ora[q], floor_r[q], "rhs", q, tol_rhs) for q in range(5)]
     assert max(errs) <= tol_rhs, ("rhs", case.name, errs)
     # streams_rhs must not change the interior
     assert np.array_equal(gpu.get_fields(), case.w0)
@@ -53,8 +55,9 @@ def check_case(S, case, nsteps, tol_rhs=TOL_RHS, tol_step=TOL_STEP, expect_activ
     dt_o, t_o = ora.step(nsteps)
     assert abs(dt_g - dt_o) <= 1e-12 * dt_o and abs(t_g - t_o) <= 1e-12 * t_o
     w_g, w_o = gpu.get_fields(), ora.get_fields()
-    errs = [field_err(w_g[q], w_o[q], floor_w[q]) for q in range(5)]
+    errs = [field_err(w_g[q], w_o[q], floor_w[q], "state", q, tol_step) for q in range(5)]
     assert max(errs) <= tol_step, ("step", case.name, errs)
+    helpers.check_floor_hits(case, hits0)        # the floor was used only where DESIGN.md says a field is at round-off
     # mask of the evolved state (S14): may differ only at nodes whose theta sits within 1e-10 of the
     # threshold, because the two states now differ by round-off
     if case.flux_mode == W.FLUX_HYBRID:

@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 import workloads as W
+from tests import helpers
 from tests.helpers import field_err, natural_scales
 
 pytestmark = pytest.mark.gpu

@@ -65,3 +65,54 @@ def test_poiseuille_flow_is_held_steady_by_its_force():
     # without the force the same nodes decelerate at -2 mu U
     R0 = O.Oracle(case.replace(accel=(0.0, 0.0, 0.0))).rhs()
     assert np.allclose(R0[1][:, inner, :], -2 * mu * U, rtol=1e-4)
+
+
+# ---- S18: the bulk-flow controller (PAPER:377, 386 force_rhs); the paper prints no formula, the pins are its properties
+def test_controller_is_deadbeat_on_a_frictionless_uniform_flow():
+    """Uniform state in a periodic inviscid box: the right-hand side is the body force alone, so a force g acting for
+    one step changes the bulk momentum P by exactly g M dt.  Started 10 % below its target, P is on target after the
+    first controlled step (to round-off), the force that brought it there was (P_target - P0) / (M dt), and from then on
+    the force returns to zero and P stays put."""
+    n = 8
+    one = np.ones((n, n, n))
+    rho0, u0, p0 = 1.3, 0.5, 1.1
+    case = W.Case(name="ctrl", nx=n, ny=n, nz=n, lx=1.0, ly=1.0, lz=1.0, dt_fixed=1e-2,
+                  w0=W.conserved_from_primitive(rho0 * one, u0 * one, 0 * one, 0 * one, p0 * one, 1.4))
+    o = O.Oracle(case, kind="serial")
+    mass, mom0 = o.bulk_sums(0)
+    assert np.isclose(mass, rho0, rtol=1e-14) and np.isclose(mom0, rho0 * u0, rtol=1e-14)      # unit volume
+    target = 1.1 * mom0
+    dt, t, g = o.step_forced(1, 0, target)           # step 1 runs unforced, then the controller sets g
+    assert np.isclose(o.bulk_sums(0)[1], mom0, rtol=1e-14)
+    assert np.isclose(g[0], (target - mom0) / (mass * dt), rtol=1e-12) and g[1] == 0.0 and g[2] == 0.0
+    dt, t, g = o.step_forced(1, 0)                   # step 2 under that force lands on the target
+    assert np.isclose(o.bulk_sums(0)[1], target, rtol=1e-13)
+    assert abs(g[0]) <= 1e-10 * abs(target - mom0) / (mass * dt)
+    for _ in range(3):
+        dt, t, g = o.step_forced(1, 0)
+        assert np.isclose(o.bulk_sums(0)[1], target, rtol=1e-13)
+    # the energy integral has grown by the work of the force, the mass is untouched
+    assert np.isclose(o.bulk_sums(0)[0], mass, rtol=1e-14)
+
+
+def test_controller_holds_a_laminar_channel_against_wall_friction():
+    """Poiseuille-like profile between isothermal walls: without a force the bulk momentum decays (wall friction);
+    under the controller it is back on target after every step to 1e-6 of the drift an unforced step leaves, and the
+    force settles near the friction it balances, tau_w * wall area / mass."""
+    case = W.channel(24, 24, 12, seed=3)
+    case = case.replace(flux_mode=W.FLUX_CENTRAL, dt_fixed=0.0)
+    free = O.Oracle(case, kind="serial")
+    m0, p0 = free.bulk_sums(0)
+    free.step(6)
+    drift = p0 - free.bulk_sums(0)[1]
+    assert drift > 0
+    o = O.Oracle(case, kind="serial")
+    gs = []
+    for _ in range(6):
+        dt, t, g = o.step_forced(1, 0)
+        gs.append(g[0])
+    # P one step after an update: the controller corrected the previous deviation; what remains is the change of the
+    # friction over one step, far below the unforced drift
+    o.step_forced(1, 0)
+    assert abs(o.bulk_sums(0)[1] - p0) < 0.05 * drift / 6
+    assert gs[-1] > 0 and abs(gs[-1] - gs[-2]) < 0.2 * abs(gs[-1])
