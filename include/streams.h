@@ -44,6 +44,7 @@ enum { STREAMS_OK = 0, STREAMS_EINVAL = -1, STREAMS_ENOMEM = -2, STREAMS_ECUDA =
 enum { STREAMS_BC_PERIODIC = 0, STREAMS_BC_WALL_ISOTHERMAL = 1, STREAMS_BC_FREESTREAM = 2 };
 enum { STREAMS_VISC_NONE = 0, STREAMS_VISC_POWER = 1, STREAMS_VISC_SUTHERLAND = 2 };
 enum { STREAMS_FLUX_CENTRAL = 0, STREAMS_FLUX_WENO = 1, STREAMS_FLUX_HYBRID = 2 };
+enum { STREAMS_WENO_JS = 0, STREAMS_WENO_Z = 1 };
 
 /* Grid ("Cartesian coordinates", "evaluation of grid metrics").
  * Uniform directions: spacing l/n, node i at i*l/n.  y is stretched when y_nodes != NULL. */
@@ -87,6 +88,7 @@ typedef struct {
   double cfl;                 /* dt = cfl / max rate                                            */
   double dt_fixed;            /* > 0 overrides the CFL time step                                */
   int dt_every;               /* recompute dt every dt_every steps (10 in production)*/
+  int weno_variant;           /* STREAMS_WENO_JS (Jiang-Shu weights) or STREAMS_WENO_Z (WENO-Z, S19) */
 } streams_scheme;
 
 /* Bytes of DEVICE workspace streams_init needs for this grid/gas/scheme; 0 on invalid input. */
@@ -142,10 +144,21 @@ int streams_get_activation_totals(streams_ctx* ctx, long long* flagged_sum, long
  * WENO forced on a chosen fraction of the points).  STREAMS_EINVAL unless flux_mode == STREAMS_FLUX_HYBRID. */
 int streams_set_mask_override(streams_ctx* ctx, const unsigned char* mask, int src_is_device);
 
-/* Replaces the uniform body acceleration streams_gas.accel (3 HOST doubles, copied) from the next evaluation on.
- * With streams_get_sums(STREAMS_SUM_STATE) this is what a bulk-flow controller needs (the forcing term is
- * re-evaluated from sum reductions every step); the controller itself is host logic (paper_2304_05494_b200/forcing.py). */
+/* Replaces the uniform body acceleration streams_gas.accel (3 HOST doubles, copied) from the next evaluation on, and
+ * takes it back from the bulk-flow controller if streams_step_forced had been used. */
 int streams_set_body_force(streams_ctx* ctx, const double* accel3);
+
+/* nsteps RK3 steps of a forced flow under the bulk-flow controller ("forcing term evaluations (sum
+ * reduction)", PAPER:386 force_rhs; reading S18 of DESIGN.md): after every step the volume integrals of mass M and of
+ * the momentum P along `direction` (0, 1, 2) are reduced on the device in a fixed order and a one-thread kernel resets
+ * the acceleration along `direction`,  g <- [g - (P - P_prev) / (M dt)] + (P_target - P) / (M dt):  the force that would
+ * have kept P constant over the step just taken plus what returns P to its target over the next one.  The kernels of
+ * the following step read g from device memory; nothing is synchronised with the host between the steps.
+ * target: the bulk momentum integral to hold, NaN = keep the one in force (at the first call: the current P).
+ * dt_last, time, accel3_out (the acceleration after the last update): HOST, nullable.  Errors as streams_step.
+ * A later streams_step keeps the last g; streams_set_body_force returns the acceleration to the host. */
+int streams_step_forced(streams_ctx* ctx, int nsteps, int direction, double target, double* dt_last,
+                        double* time, double* accel3_out);
 
 /* Sum reductions over the interior nodes (PAPER:218-236 compute_residual; Table 2 "forcing term evaluations (sum
  * reduction)"), in a fixed order: the five doubles of out5 (HOST) are reproducible bit for bit.

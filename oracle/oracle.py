@@ -37,6 +37,7 @@ class OracleParams(C.Structure):
         ("sensor_threshold", C.c_double), ("weno_eps", C.c_double),
         ("cfl", C.c_double), ("dt_fixed", C.c_double),
         ("accel", C.c_double * 3),
+        ("weno_variant", C.c_int),
     ]
 
 
@@ -68,6 +69,8 @@ def load(kind: str = "omp"):
         lib.oracle_fd_coeffs.argtypes = [C.c_int, _c_double_p, _c_double_p]
         lib.oracle_weno_reconstruct.restype = C.c_double
         lib.oracle_weno_reconstruct.argtypes = [_c_double_p, C.c_int, C.c_double, C.c_int, _c_double_p]
+        lib.oracle_weno_reconstruct_variant.restype = C.c_double
+        lib.oracle_weno_reconstruct_variant.argtypes = [_c_double_p, C.c_int, C.c_double, C.c_int]
         lib.oracle_eigenvectors.argtypes = [C.c_int, _c_double_p, C.c_double, C.c_double, _c_double_p, _c_double_p]
         lib.oracle_num_threads.restype = C.c_int
         _libs[kind] = lib
@@ -92,6 +95,7 @@ def params_from_case(case, dbg_flags: int = 0) -> OracleParams:
         p.freestream[q] = case.freestream[q]
     for a in range(3):
         p.accel[a] = case.accel[a]
+    p.weno_variant = case.weno_variant
     return p
 
 
@@ -217,6 +221,12 @@ def weno_reconstruct(v, r: int, eps: float = 1e-6, linear: bool = False, kind: s
     beta = np.zeros(4)
     val = load(kind).oracle_weno_reconstruct(_dp(v), r, eps, int(linear), _dp(beta))
     return val, beta[:r].copy()
+
+
+def weno_reconstruct_variant(v, r: int, eps: float = 1e-6, variant: int = 1, kind: str = "serial"):
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert v.size == 2 * r - 1
+    return load(kind).oracle_weno_reconstruct_variant(_dp(v), r, eps, variant)
 
 
 def eigenvectors(d: int, vel, H: float, gamma: float, kind: str = "serial"):

@@ -34,6 +34,8 @@
 //                        manufactured Navier-Stokes terms with n = 0.76 at design order
 //   S17 body force     : uniform state => R = (0, rho g, rho u.g) exactly; momentum budget of a periodic box;
 //                        Poiseuille flow driven by g instead of a pressure gradient
+//   S19 WENO-Z         : design order 2r-1 at a first-order critical point (Jiang-Shu: lower), weights within
+//                        O(dx^4) of the linear ones on smooth data, the smooth side at a jump
 //   S18 flow control   : deadbeat on a frictionless uniform flow (P reaches its target in one step and stays), holds
 //                        a laminar channel against its wall friction
 // Unpinned against the real STREAmS code (not in the container): S1, S2, S4, S5,
@@ -77,6 +79,7 @@ extern "C" struct oracle_params {
   double sensor_threshold, weno_eps;
   double cfl, dt_fixed;
   double accel[3];              // uniform body acceleration g (S17)
+  int weno_variant;             // 0: Jiang-Shu weights, 1: WENO-Z (S19)
 };
 
 namespace {
@@ -115,7 +118,7 @@ void fd2_coeffs(int L, double* b) {
 // tests/test_oracle_weno.py by exact rational derivation).
 // beta_out (optional) receives the r smoothness indicators.
 // -----------------------------------------------------------------------------
-double weno_reconstruct(const double* v, int r, double eps, bool linear, double* beta_out) {
+double weno_reconstruct(const double* v, int r, double eps, bool linear, double* beta_out, int variant = 0) {
   double q[4], beta[4], d[4];
   if (r == 1) {
     if (beta_out) beta_out[0] = 0.0;
@@ -166,9 +169,17 @@ double weno_reconstruct(const double* v, int r, double eps, bool linear, double*
   }
   if (beta_out) for (int k = 0; k < r; ++k) beta_out[k] = beta[k];
   double alpha[4], asum = 0.0;
+  // S19 (variant 1, WENO-Z of Borges et al. 2008 / Castro et al. 2011): the global indicator
+  // tau = |beta_0 - beta_{r-1}| (r = 2, 3), |beta_0 - beta_1 - beta_2 + beta_3| (r = 4) measures the smoothness of the
+  // whole stencil; alpha_k = d_k (1 + (tau / (eps + beta_k))^2) keeps the weights within O(dx^(2r-2))... of the linear
+  // ones wherever the data are smooth, critical points included (Jiang-Shu weights drop to order r there).
+  double tau = 0.0;
+  if (variant == 1 && r >= 2) tau = std::fabs(r == 4 ? ((beta[0] - beta[1]) - beta[2]) + beta[3] : beta[0] - beta[r - 1]);
   for (int k = 0; k < r; ++k) {
-    // alpha_k = d_k / (eps + beta_k)^2 ; debug switch: omega_k = d_k (linear limit, O3 pin ii)
-    alpha[k] = linear ? d[k] : d[k] / ((eps + beta[k]) * (eps + beta[k]));
+    // Jiang-Shu: alpha_k = d_k / (eps + beta_k)^2 ; debug switch: omega_k = d_k (linear limit, O3 pin ii)
+    if (linear) alpha[k] = d[k];
+    else if (variant == 1) { const double t = tau / (eps + beta[k]); alpha[k] = d[k] * (1.0 + t * t); }
+    else alpha[k] = d[k] / ((eps + beta[k]) * (eps + beta[k]));
     asum += alpha[k];
   }
   double res = 0.0;
@@ -606,8 +617,8 @@ struct Solver {
         gp[m] = 0.5 * sp;
         gm[m] = 0.5 * sm;
       }
-      ghat[s] = weno_reconstruct(gp, r, P.weno_eps, linear, nullptr) +
-                weno_reconstruct(gm, r, P.weno_eps, linear, nullptr);
+      ghat[s] = weno_reconstruct(gp, r, P.weno_eps, linear, nullptr, P.weno_variant) +
+                weno_reconstruct(gm, r, P.weno_eps, linear, nullptr, P.weno_variant);
     }
     // 5. project back on the right eigenvectors
     for (int q = 0; q < 5; ++q) {
@@ -874,6 +885,7 @@ void* oracle_create(const oracle_params* p, const double* y_nodes) {
   const int L = p->central_order / 2;
   if (p->central_order % 2 || L < 1 || L > 4) return nullptr;
   if (p->flux_mode != FLUX_CENTRAL && (p->weno_order % 2 == 0 || p->weno_order < 1 || p->weno_order > 7)) return nullptr;
+  if (p->weno_variant < 0 || p->weno_variant > 1) return nullptr;
   if (p->visc_law != VISC_NONE && (p->visc_order % 2 || p->visc_order < 2 || p->visc_order > 8)) return nullptr;
   return new Solver(*p, y_nodes);
 }
@@ -997,6 +1009,9 @@ int oracle_get_metrics(void* h, double* eta_y_c, double* eta_y_v, double* eta_yy
 void oracle_fd_coeffs(int order, double* a, double* b) { fd1_coeffs(order / 2, a); fd2_coeffs(order / 2, b); }
 double oracle_weno_reconstruct(const double* v, int r, double eps, int linear, double* beta_out) {
   return weno_reconstruct(v, r, eps, linear != 0, beta_out);
+}
+double oracle_weno_reconstruct_variant(const double* v, int r, double eps, int variant) {
+  return weno_reconstruct(v, r, eps, false, nullptr, variant);
 }
 void oracle_eigenvectors(int d, const double* vel, double H, double gamma, double* Lm, double* Rm) {
   euler_eigenvectors(d, vel, H, gamma, Lm, Rm);

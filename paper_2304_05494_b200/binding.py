@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
 
 STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
-           "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
+           "streams_step_forced", "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches", "streams_graph_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
            "streams_measure_fp64_scratch_bytes",
@@ -45,7 +45,7 @@ class streams_gas(C.Structure):
 class streams_scheme(C.Structure):
     _fields_ = [("central_order", C.c_int), ("weno_order", C.c_int), ("visc_order", C.c_int),
                 ("flux_mode", C.c_int), ("sensor_threshold", C.c_double), ("weno_eps", C.c_double),
-                ("cfl", C.c_double), ("dt_fixed", C.c_double), ("dt_every", C.c_int)]
+                ("cfl", C.c_double), ("dt_fixed", C.c_double), ("dt_every", C.c_int), ("weno_variant", C.c_int)]
 
 
 _lib = None
@@ -67,6 +67,7 @@ def load_library(path: str = LIB_PATH):
     lib.streams_set_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_rhs.argtypes = [C.c_void_p, C.c_void_p]
     lib.streams_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
+    lib.streams_step_forced.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp, _dp, _dp]
     lib.streams_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_set_mask_override.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -109,7 +110,7 @@ def structs_from_case(case):
     for d in range(3):
         a.accel[d] = case.accel[d]
     for n in ("central_order", "weno_order", "visc_order", "flux_mode", "sensor_threshold", "weno_eps", "cfl",
-              "dt_fixed", "dt_every"):
+              "dt_fixed", "dt_every", "weno_variant"):
         setattr(s, n, getattr(case, n))
     return g, a, s, keep
 
@@ -217,6 +218,14 @@ class Streams:
         self._check(self.lib.streams_step(self.h, int(nsteps), C.byref(dt), C.byref(t)))
         return dt.value, t.value
 
+    def step_forced(self, nsteps, direction=0, target=float("nan")):
+        """nsteps steps under the device-side bulk-flow controller; returns (dt, time, [g_x, g_y, g_z])."""
+        dt, t = C.c_double(), C.c_double()
+        g = (C.c_double * 3)()
+        self._check(self.lib.streams_step_forced(self.h, int(nsteps), int(direction), C.c_double(target), C.byref(dt),
+                                                 C.byref(t), C.cast(g, _dp)))
+        return dt.value, t.value, list(g)
+
     def get_fields(self, out=None):
         if out is None:
             out = np.empty((5,) + self.shape, dtype=np.float64)
@@ -291,8 +300,9 @@ class Streams:
 
     def destroy(self):
         if getattr(self, "h", None):
-            self.lib.streams_destroy(self.h)
+            self.lib.streams_destroy(self.h)         # synchronises the stream
             self.h = None
+        self.workspace = None                        # the device memory goes back to torch's allocator
 
     def __del__(self):
         try:

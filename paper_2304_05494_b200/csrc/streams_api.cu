@@ -60,6 +60,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   if (g->bc_y_lo != STREAMS_BC_PERIODIC && !(g->y_wall_hi > g->y_wall_lo)) return "y_wall_hi must exceed y_wall_lo";
   if (sc->central_order < 2 || sc->central_order > 8 || sc->central_order % 2) return "central_order must be 2, 4, 6 or 8";
   if (sc->flux_mode < 0 || sc->flux_mode > 2) return "bad flux_mode";
+  if (sc->weno_variant != STREAMS_WENO_JS && sc->weno_variant != STREAMS_WENO_Z) return "bad weno_variant";
   if (gas->visc_law < 0 || gas->visc_law > 2) return "bad visc_law";
   if (sc->flux_mode != STREAMS_FLUX_CENTRAL && (sc->weno_order < 1 || sc->weno_order > 7 || sc->weno_order % 2 == 0))
     return "weno_order must be 1, 3, 5 or 7";
@@ -396,10 +397,11 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.thr = scheme->sensor_threshold; P.thr2 = P.thr * P.thr; P.weno_eps = scheme->weno_eps; P.cfl = scheme->cfl;
   for (int q = 0; q < 5; ++q) P.fsw[q] = gas->freestream[q];
   for (int d = 0; d < 3; ++d) P.accel[d] = gas->accel[d];
-  P.has_accel = gas->accel[0] != 0.0 || gas->accel[1] != 0.0 || gas->accel[2] != 0.0;
+  P.has_accel = (gas->accel[0] != 0.0 || gas->accel[1] != 0.0 || gas->accel[2] != 0.0) ? 1 : 0;
   P.t_wall_lo = grid->t_wall_lo; P.t_wall_hi = grid->t_wall_hi;
   P.bc_x = grid->bc_x; P.bc_y_lo = grid->bc_y_lo; P.bc_y_hi = grid->bc_y_hi; P.bc_z = grid->bc_z;
   P.visc_law = gas->visc_law; P.flux_mode = scheme->flux_mode;
+  P.weno_z = scheme->weno_variant == STREAMS_WENO_Z;
   P.own_x = grid->bc_x == STREAMS_BC_PERIODIC && grid->nx >= 2 * S.ng;
   P.own_y = grid->bc_y_lo == STREAMS_BC_PERIODIC && grid->ny >= 2 * S.ng;
   P.own_z = grid->bc_z == STREAMS_BC_PERIODIC && grid->nz >= 2 * S.ng;
@@ -469,7 +471,7 @@ int streams_set_fields(streams_ctx* ctx, const double* w, int src_is_device) {
     p.kind = kind;
     CU(cudaMemcpy3DAsync(&p, ctx->stream));
   }
-  CU(cudaMemsetAsync(P.scal, 0, S_COUNT * 8, ctx->stream));
+  CU(cudaMemsetAsync(P.scal, 0, S_ACC * 8, ctx->stream));   // step scalars; the controller's (S_ACC ..) are kept
   CU(cudaMemsetAsync(P.counters, 0, C_COUNT * 4, ctx->stream));
   if (!src_is_device) CU(cudaStreamSynchronize(ctx->stream));   // the host buffer may be reused on return
   ctx->have_fields = true;
@@ -513,68 +515,112 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev) {
   return STREAMS_OK;
 }
 
-int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
-  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
-  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_step before streams_set_fields");
-  if (nsteps < 0) return fail(ctx, STREAMS_EINVAL, "nsteps must be non-negative");
-  if (nsteps > 0) ctx->r_valid = false;              // R becomes the low-storage scheme's previous-stage register
-  for (int s = 0; s < nsteps; ++s) {
-    const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
-    // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
-    const bool want_rate = !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0;
-    // A step whose launch sequence is the steady one (primitives of the state already in place, the rate for its dt
-    // already reduced) is replayed from a CUDA graph: the 10-16 launches of a step become one submission, which is
-    // what a small grid needs (grids below ~2 M points cannot hide the launch latency).
-    const bool steady = ctx->prims_interior && (!want_dt || ctx->scheme.dt_fixed > 0.0 || ctx->rate_ready);
-    if (ctx->graphs_on && !ctx->prof_on && steady) {
-      const int key = ctx->cur | (want_dt ? 2 : 0) | (want_rate ? 4 : 0);
-      if (!ctx->step_graph[key]) {
-        const long long l0 = ctx->launches;
-        const int cur0 = ctx->cur;
-        const bool rr0 = ctx->rate_ready;
-        if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
-          cudaGetLastError();                          // e.g. the legacy default stream cannot be captured: launch directly
-          ctx->graphs_on = false;
-          const int rd = enqueue_step(ctx, want_dt, want_rate);
-          if (rd < 0) return launch_fail(ctx, rd);
-          ctx->step_count += 1;
-          continue;
-        }
-        const int rc = enqueue_step(ctx, want_dt, want_rate);
-        cudaGraph_t graph = nullptr;
-        const cudaError_t ee = cudaStreamEndCapture(ctx->stream, &graph);
-        if (rc < 0) { if (graph) cudaGraphDestroy(graph); return launch_fail(ctx, rc); }
-        if (ee != cudaSuccess) return cuda_fail(ctx, ee, "cudaStreamEndCapture");
-        const cudaError_t ei = cudaGraphInstantiate(&ctx->step_graph[key], graph, 0);
-        cudaGraphDestroy(graph);
-        if (ei != cudaSuccess) { ctx->step_graph[key] = nullptr; return cuda_fail(ctx, ei, "cudaGraphInstantiate"); }
-        ctx->step_graph_launches[key] = (int)(ctx->launches - l0);
-        // nothing ran during the capture: rewind the host state it advanced, the replay below advances it again
-        ctx->launches = l0;
-        use_qbuf(ctx, cur0);
-        ctx->rate_ready = rr0;
+// One RK3 step on the stream: replayed from its CUDA graph when its launch sequence is the steady one, launched kernel
+// by kernel otherwise.  Returns STREAMS_OK or an error code (message set).
+static int run_one_step(streams_ctx* ctx) {
+  const bool want_dt = (ctx->step_count % ctx->scheme.dt_every) == 0;
+  // the last stage also reduces the time-step rate of the state it produces if the next step recomputes dt
+  const bool want_rate = !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0;
+  // A step whose launch sequence is the steady one (primitives of the state already in place, the rate for its dt
+  // already reduced) is replayed from a CUDA graph: the 10-16 launches of a step become one submission, which is
+  // what a small grid needs (grids below ~2 M points cannot hide the launch latency).
+  const bool steady = ctx->prims_interior && (!want_dt || ctx->scheme.dt_fixed > 0.0 || ctx->rate_ready);
+  if (ctx->graphs_on && !ctx->prof_on && steady) {
+    const int key = ctx->cur | (want_dt ? 2 : 0) | (want_rate ? 4 : 0);
+    if (!ctx->step_graph[key]) {
+      const long long l0 = ctx->launches;
+      const int cur0 = ctx->cur;
+      const bool rr0 = ctx->rate_ready;
+      if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();                          // e.g. the legacy default stream cannot be captured: launch directly
+        ctx->graphs_on = false;
+        const int rd = enqueue_step(ctx, want_dt, want_rate);
+        if (rd < 0) return launch_fail(ctx, rd);
+        ctx->step_count += 1;
+        return STREAMS_OK;
       }
-      CU(cudaGraphLaunch(ctx->step_graph[key], ctx->stream));
-      ctx->graph_launches += 1;
-      ctx->launches += ctx->step_graph_launches[key];
-      use_qbuf(ctx, ctx->cur ^ 1);                   // three stages, three swaps of the primitive buffers
-      if (want_dt) ctx->rate_ready = false;
-      if (want_rate) ctx->rate_ready = true;
-    } else {
       const int rc = enqueue_step(ctx, want_dt, want_rate);
-      if (rc < 0) return launch_fail(ctx, rc);
+      cudaGraph_t graph = nullptr;
+      const cudaError_t ee = cudaStreamEndCapture(ctx->stream, &graph);
+      if (rc < 0) { if (graph) cudaGraphDestroy(graph); return launch_fail(ctx, rc); }
+      if (ee != cudaSuccess) return cuda_fail(ctx, ee, "cudaStreamEndCapture");
+      const cudaError_t ei = cudaGraphInstantiate(&ctx->step_graph[key], graph, 0);
+      cudaGraphDestroy(graph);
+      if (ei != cudaSuccess) { ctx->step_graph[key] = nullptr; return cuda_fail(ctx, ei, "cudaGraphInstantiate"); }
+      ctx->step_graph_launches[key] = (int)(ctx->launches - l0);
+      // nothing ran during the capture: rewind the host state it advanced, the replay below advances it again
+      ctx->launches = l0;
+      use_qbuf(ctx, cur0);
+      ctx->rate_ready = rr0;
     }
-    ctx->step_count += 1;
+    CU(cudaGraphLaunch(ctx->step_graph[key], ctx->stream));
+    ctx->graph_launches += 1;
+    ctx->launches += ctx->step_graph_launches[key];
+    use_qbuf(ctx, ctx->cur ^ 1);                   // three stages, three swaps of the primitive buffers
+    if (want_dt) ctx->rate_ready = false;
+    if (want_rate) ctx->rate_ready = true;
+  } else {
+    const int rc = enqueue_step(ctx, want_dt, want_rate);
+    if (rc < 0) return launch_fail(ctx, rc);
   }
+  ctx->step_count += 1;
+  return STREAMS_OK;
+}
+
+// reads the step scalars back (synchronises the stream) and maps a non-finite state or time step to STREAMS_ENAN
+static int finish_steps(streams_ctx* ctx, double* dt_last, double* time, double* accel3_out) {
   CU(cudaGetLastError());
   double h[S_COUNT];
   CU(cudaMemcpyAsync(h, ctx->P.scal, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   if (dt_last) *dt_last = h[S_DT];
   if (time) *time = h[S_TIME];
+  if (accel3_out) for (int a = 0; a < 3; ++a) accel3_out[a] = ctx->P.has_accel == 2 ? h[S_ACC + a] : ctx->P.accel[a];
   if (h[S_NAN] != 0.0 || !std::isfinite(h[S_DT]) || !std::isfinite(h[S_TIME]) || !std::isfinite(h[S_RATE]))
     return fail(ctx, STREAMS_ENAN, "the state or the time step became non-finite");
   return STREAMS_OK;
+}
+
+int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_step before streams_set_fields");
+  if (nsteps < 0) return fail(ctx, STREAMS_EINVAL, "nsteps must be non-negative");
+  if (nsteps > 0) ctx->r_valid = false;              // R becomes the low-storage scheme's previous-stage register
+  for (int s = 0; s < nsteps; ++s) {
+    const int rc = run_one_step(ctx);
+    if (rc != STREAMS_OK) return rc;
+  }
+  return finish_steps(ctx, dt_last, time, nullptr);
+}
+
+int streams_step_forced(streams_ctx* ctx, int nsteps, int direction, double target, double* dt_last, double* time,
+                        double* accel3_out) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "streams_step_forced before streams_set_fields");
+  if (nsteps < 0 || direction < 0 || direction > 2) return fail(ctx, STREAMS_EINVAL, "bad nsteps or direction");
+  double* scratch = (double*)(ctx->base + ctx->S.off_sums);
+  double* sums_dev = scratch + (sums_scratch_doubles() - 8);
+  cudaStream_t st = ctx->stream;
+  if (ctx->P.has_accel != 2) {
+    // the controller takes the acceleration over: its current value moves to the device scalars, the kernels read it
+    // there from now on (until streams_set_body_force hands it back to the host)
+    CU(cudaMemcpyAsync(ctx->P.scal + S_ACC, ctx->P.accel, 3 * sizeof(double), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));                   // P.accel is host memory of the context
+    ctx->P.has_accel = 2;
+    drop_step_graphs(ctx);
+    timed(ctx, STREAMS_K_MISC, [&] { return launch_sums(ctx->P, STREAMS_SUM_STATE, scratch, sums_dev, st); });
+    timed(ctx, STREAMS_K_MISC, [&] { return launch_controller(ctx->P, sums_dev, direction, target, true, st); });
+    target = std::nan("");                           // recorded; later updates keep it
+  }
+  if (nsteps > 0) ctx->r_valid = false;
+  for (int s = 0; s < nsteps; ++s) {
+    const int rc = run_one_step(ctx);
+    if (rc != STREAMS_OK) return rc;
+    timed(ctx, STREAMS_K_MISC, [&] { return launch_sums(ctx->P, STREAMS_SUM_STATE, scratch, sums_dev, st); });
+    timed(ctx, STREAMS_K_MISC, [&] { return launch_controller(ctx->P, sums_dev, direction, target, false, st); });
+    target = std::nan("");
+  }
+  return finish_steps(ctx, dt_last, time, accel3_out);
 }
 
 int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_out, int dst_is_device) {
@@ -659,7 +705,7 @@ int streams_set_body_force(streams_ctx* ctx, const double* accel3) {
     ctx->P.accel[d] = accel3[d];
     ctx->gas.accel[d] = accel3[d];
   }
-  ctx->P.has_accel = accel3[0] != 0.0 || accel3[1] != 0.0 || accel3[2] != 0.0;
+  ctx->P.has_accel = (accel3[0] != 0.0 || accel3[1] != 0.0 || accel3[2] != 0.0) ? 1 : 0;   // host-owned again
   drop_step_graphs(ctx);
   ctx->r_valid = false;                              // R no longer is the right-hand side under the new force
   return STREAMS_OK;

@@ -505,6 +505,27 @@ __global__ void sum_final_kernel(const double* __restrict__ partial, double* __r
   }
 }
 
+// S18: bulk-flow controller, one thread after the state sums of a step.  A force g acting for dt changes
+// the bulk momentum P = sums[1 + d] by g M dt (M = sums[0]): g <- [g - (P - P_prev) / (M dt)] + (P_target - P) / (M dt).
+// init: the first call records P (and takes it as the target when none was given, target = NaN) and leaves g alone.
+__global__ void controller_kernel(const DevP P, const double* __restrict__ sums, int d, double target, int init) {
+  const double mass = sums[0], mom = sums[1 + d];
+  if (init) {
+    P.scal[S_PPREV] = mom;
+    P.scal[S_PTARGET] = (target != target) ? mom : target;
+    return;
+  }
+  if (target == target) P.scal[S_PTARGET] = target;
+  const double dt = P.scal[S_DT];
+  const double g_balance = P.scal[S_ACC + d] - (mom - P.scal[S_PPREV]) / (mass * dt);
+  P.scal[S_ACC + d] = g_balance + (P.scal[S_PTARGET] - mom) / (mass * dt);
+  P.scal[S_PPREV] = mom;
+}
+int launch_controller(const DevP& P, const double* sums, int d, double target, bool init, cudaStream_t st) {
+  controller_kernel<<<1, 1, 0, st>>>(P, sums, d, target, init ? 1 : 0);
+  return 1;
+}
+
 // partial: 5 * SUM_BLOCKS doubles of scratch, out: 5 doubles (device)
 int launch_sums(const DevP& P, int kind, double* partial, double* out, cudaStream_t st) {
   if (kind == 0) sum_partial_kernel<0><<<SUM_BLOCKS, SUM_THREADS, 0, st>>>(P, partial);

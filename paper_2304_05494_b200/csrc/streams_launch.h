@@ -42,6 +42,7 @@ int launch_rhs_main(const DevP& P, const MarchMaps& maps, int L, int Lv, const S
 int march_family(int L, int Lv, int ng);
 int launch_sums(const DevP& P, int kind, double* partial, double* out, cudaStream_t st);   // streams_get_sums
 int sums_scratch_doubles();
+int launch_controller(const DevP& P, const double* sums, int d, double target, bool init, cudaStream_t st);   // S18
 size_t measure_fp64_scratch_bytes();
 double measure_fp64(cudaStream_t st, int kind, int repeats, double* scratch, size_t scratch_bytes);   // streams_measure_fp64
 

@@ -282,6 +282,8 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   }
   const double sb2 = fma(-2.0 * P.sbv, ym.eyv2, P.sb2xz);
   const double dt = UPD ? P.scal[S_DT] : 0.0;
+  double acc[3] = {P.accel[0], P.accel[1], P.accel[2]};   // S17; owned by the device-side controller when has_accel == 2
+  if (P.has_accel == 2) { acc[0] = P.scal[S_ACC]; acc[1] = P.scal[S_ACC + 1]; acc[2] = P.scal[S_ACC + 2]; }
 
   // ring = planes kb-NG .. kb+NG of this thread's column
   double zr[NF][2 * NG + 1];
@@ -419,8 +421,8 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     if (P.has_accel) {                               // S17: uniform body acceleration and its work
       const double rho0 = c0[F_RHO];
 #pragma unroll
-      for (int a = 0; a < 3; ++a) r[1 + a] = fma(rho0, P.accel[a], r[1 + a]);
-      r[4] = fma(rho0, fma(c0[F_U], P.accel[0], fma(c0[F_V], P.accel[1], c0[F_W] * P.accel[2])), r[4]);
+      for (int a = 0; a < 3; ++a) r[1 + a] = fma(rho0, acc[a], r[1 + a]);
+      r[4] = fma(rho0, fma(c0[F_U], acc[0], fma(c0[F_V], acc[1], c0[F_W] * acc[2])), r[4]);
     }
     if (UPD) {
 #pragma unroll

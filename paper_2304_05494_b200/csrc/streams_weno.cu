@@ -19,36 +19,49 @@ namespace streams {
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double sq(double x) { return x * x; }
 
-template <int R>
+// Z: WENO-Z weights (S19) alpha_k = d_k (1 + (tau / s_k)^2) with s_k = eps + beta_k and the global indicator
+// tau of the whole stencil; scaled by prod_j s_j^2 like the Jiang-Shu ones: a_k = d_k (s_k^2 + tau^2) prod_{j != k} s_j^2.
+template <int R, bool Z>
 __device__ __forceinline__ double weno_rec(const double* v, double eps);
 
 template <>
-__device__ __forceinline__ double weno_rec<1>(const double* v, double) { return v[0]; }
+__device__ __forceinline__ double weno_rec<1, false>(const double* v, double) { return v[0]; }
+template <>
+__device__ __forceinline__ double weno_rec<1, true>(const double* v, double) { return v[0]; }
 
 // The Jiang-Shu weights alpha_k = d_k / (eps + beta_k)^2 are scaled by prod_j (eps + beta_j)^2, which leaves
 // omega_k = alpha_k / sum(alpha) unchanged and needs one division per reconstruction instead of R + 1.
-template <>
-__device__ __forceinline__ double weno_rec<2>(const double* v, double eps) {
+template <bool Z>
+__device__ __forceinline__ double weno_rec2(const double* v, double eps) {
   const double q0 = 0.5 * (3.0 * v[1] - v[0]), q1 = 0.5 * (v[1] + v[2]);
   const double s0 = eps + sq(v[1] - v[0]), s1 = eps + sq(v[2] - v[1]);
-  const double a0 = (1.0 / 3.0) * sq(s1), a1 = (2.0 / 3.0) * sq(s0);
+  const double t2 = Z ? sq(s0 - s1) : 0.0;            // tau^2, tau = |beta_0 - beta_1|
+  const double a0 = (1.0 / 3.0) * (Z ? (sq(s0) + t2) * sq(s1) : sq(s1)), a1 = (2.0 / 3.0) * (Z ? (sq(s1) + t2) * sq(s0) : sq(s0));
   return (a0 * q0 + a1 * q1) * rcp_pos(a0 + a1);
 }
+template <> __device__ __forceinline__ double weno_rec<2, false>(const double* v, double eps) { return weno_rec2<false>(v, eps); }
+template <> __device__ __forceinline__ double weno_rec<2, true>(const double* v, double eps) { return weno_rec2<true>(v, eps); }
 
-template <>
-__device__ __forceinline__ double weno_rec<3>(const double* v, double eps) {
+template <bool Z>
+__device__ __forceinline__ double weno_rec3(const double* v, double eps) {
   const double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) * (1.0 / 6.0);
   const double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) * (1.0 / 6.0);
   const double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) * (1.0 / 6.0);
   const double s0 = eps + ((13.0 / 12.0) * sq(v[0] - 2.0 * v[1] + v[2]) + 0.25 * sq(v[0] - 4.0 * v[1] + 3.0 * v[2]));
   const double s1 = eps + ((13.0 / 12.0) * sq(v[1] - 2.0 * v[2] + v[3]) + 0.25 * sq(v[1] - v[3]));
   const double s2 = eps + ((13.0 / 12.0) * sq(v[2] - 2.0 * v[3] + v[4]) + 0.25 * sq(3.0 * v[2] - 4.0 * v[3] + v[4]));
-  const double a0 = 0.1 * sq(s1 * s2), a1 = 0.6 * sq(s0 * s2), a2 = 0.3 * sq(s0 * s1);
+  double a0 = 0.1 * sq(s1 * s2), a1 = 0.6 * sq(s0 * s2), a2 = 0.3 * sq(s0 * s1);
+  if (Z) {
+    const double t2 = sq(s0 - s2);                    // tau^2, tau = |beta_0 - beta_2|
+    a0 *= sq(s0) + t2; a1 *= sq(s1) + t2; a2 *= sq(s2) + t2;
+  }
   return (a0 * q0 + a1 * q1 + a2 * q2) * rcp_pos((a0 + a1) + a2);
 }
+template <> __device__ __forceinline__ double weno_rec<3, false>(const double* v, double eps) { return weno_rec3<false>(v, eps); }
+template <> __device__ __forceinline__ double weno_rec<3, true>(const double* v, double eps) { return weno_rec3<true>(v, eps); }
 
-template <>
-__device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
+template <bool Z>
+__device__ __forceinline__ double weno_rec4(const double* v, double eps) {
   const double q0 = (-3.0 * v[0] + 13.0 * v[1] - 23.0 * v[2] + 25.0 * v[3]) * (1.0 / 12.0);
   const double q1 = (v[1] - 5.0 * v[2] + 13.0 * v[3] + 3.0 * v[4]) * (1.0 / 12.0);
   const double q2 = (-v[2] + 7.0 * v[3] + 7.0 * v[4] - v[5]) * (1.0 / 12.0);
@@ -70,27 +83,33 @@ __device__ __forceinline__ double weno_rec<4>(const double* v, double eps) {
   const double s2 = eps + (cU * sq(U2) + cS * sq(S1) + cT * sq(T2));
   const double s3 = eps + (cU * sq(U3) + cS * sq(S3) + cT * sq(T3));
   const double p01 = s0 * s1, p23 = s2 * s3;
-  const double a0 = (1.0 / 35.0) * sq(s1 * p23), a1 = (12.0 / 35.0) * sq(s0 * p23);
-  const double a2 = (18.0 / 35.0) * sq(p01 * s3), a3 = (4.0 / 35.0) * sq(p01 * s2);
+  double a0 = (1.0 / 35.0) * sq(s1 * p23), a1 = (12.0 / 35.0) * sq(s0 * p23);
+  double a2 = (18.0 / 35.0) * sq(p01 * s3), a3 = (4.0 / 35.0) * sq(p01 * s2);
+  if (Z) {
+    const double t2 = sq(((s0 - s1) - s2) + s3);      // tau^2, tau = |beta_0 - beta_1 - beta_2 + beta_3|
+    a0 *= sq(s0) + t2; a1 *= sq(s1) + t2; a2 *= sq(s2) + t2; a3 *= sq(s3) + t2;
+  }
   return (a0 * q0 + a1 * q1 + a2 * q2 + a3 * q3) * rcp_pos(((a0 + a1) + a2) + a3);
 }
+template <> __device__ __forceinline__ double weno_rec<4, false>(const double* v, double eps) { return weno_rec4<false>(v, eps); }
+template <> __device__ __forceinline__ double weno_rec<4, true>(const double* v, double eps) { return weno_rec4<true>(v, eps); }
 
 // Both reconstructions of a characteristic field (upwind and mirrored stencil) as ONE call with the arguments by
 // value, in registers: the five fields of an interface then share one copy of the code instead of ten inlined
 // reconstructions (instruction-cache footprint: the list kernel's straight-line code shrinks by 30 %), while the two
 // reconstructions of a field still interleave.  STREAMS_WENO_REC_INLINE restores the inlined form.
-template <int R>
+template <int R, bool Z>
 __device__ __forceinline__ double weno_rec_pair(const double* gp, const double* gm, double eps) {
-  return weno_rec<R>(gp, eps) + weno_rec<R>(gm, eps);
+  return weno_rec<R, Z>(gp, eps) + weno_rec<R, Z>(gm, eps);
 }
 #ifndef STREAMS_WENO_REC_INLINE
 __device__ __noinline__ double weno_rec5_pair_call(double p0, double p1, double p2, double p3, double p4, double m0, double m1,
                                                   double m2, double m3, double m4, double eps) {
   const double gp[5] = {p0, p1, p2, p3, p4}, gm[5] = {m0, m1, m2, m3, m4};
-  return weno_rec<3>(gp, eps) + weno_rec<3>(gm, eps);
+  return weno_rec<3, false>(gp, eps) + weno_rec<3, false>(gm, eps);
 }
 template <>
-__device__ __forceinline__ double weno_rec_pair<3>(const double* gp, const double* gm, double eps) {
+__device__ __forceinline__ double weno_rec_pair<3, false>(const double* gp, const double* gm, double eps) {
   return weno_rec5_pair_call(gp[0], gp[1], gp[2], gp[3], gp[4], gm[0], gm[1], gm[2], gm[3], gm[4], eps);
 }
 #endif
@@ -175,7 +194,7 @@ __device__ __forceinline__ void weno_stencil(const DevP& P, long long n, long lo
   }
 }
 
-template <int D, int M, int R>
+template <int D, int M, int R, bool Z>
 __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], double f[5], const double* __restrict__ st) {
   constexpr int NS = 2 * M;                        // column pitch (the ST macro)
   constexpr int NW = 2 * R;                        // WENO stencil nodes, column slots O .. O + NW - 1
@@ -217,7 +236,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[0], lw, lf);
     gm[NW - 1 - m] = fma(-lam[0], lw, lf);          // mirrored: gm[0] is node n+R
   }
-  const double g0 = weno_rec_pair<R>(gp, gm, P.weno_eps);
+  const double g0 = weno_rec_pair<R, Z>(gp, gm, P.weno_eps);
   // u + c
 #pragma unroll
   for (int m = 0; m < NW; ++m) {
@@ -225,7 +244,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[2], lw, lf);
     gm[NW - 1 - m] = fma(-lam[2], lw, lf);
   }
-  const double g4 = weno_rec_pair<R>(gp, gm, P.weno_eps);
+  const double g4 = weno_rec_pair<R, Z>(gp, gm, P.weno_eps);
   // entropy
 #pragma unroll
   for (int m = 0; m < NW; ++m) {
@@ -234,7 +253,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
     gp[m] = fma(lam[1], lw, lf);
     gm[NW - 1 - m] = fma(-lam[1], lw, lf);
   }
-  const double g1 = weno_rec_pair<R>(gp, gm, P.weno_eps);
+  const double g1 = weno_rec_pair<R, Z>(gp, gm, P.weno_eps);
   // the two shear fields
   double gs[2];
 #pragma unroll
@@ -247,7 +266,7 @@ __device__ __forceinline__ void weno_flux(const DevP& P, const double lam[3], do
       gp[m] = fma(lam[1], lw, lf);
       gm[NW - 1 - m] = fma(-lam[1], lw, lf);
     }
-    gs[e] = weno_rec_pair<R>(gp, gm, P.weno_eps);
+    gs[e] = weno_rec_pair<R, Z>(gp, gm, P.weno_eps);
   }
   // f = sum over the fields of g r: r(u-+c) = (1, vbar -+ c e_D, H -+ un c), r(entropy) = (1, vbar, q^2/2), r(shear t) = (0, e_t, vbar_t)
   const double gsum = (g0 + g4) + g1, gdc = (g4 - g0) * cb;
@@ -272,7 +291,7 @@ template <int R> struct WenoOcc { static constexpr int MINB = R >= 4 ? 2 : STREA
 // node's index.  Flat index over the interface slots of the three directions (slot = interior extents with the D
 // extent enlarged by one; slot s along D is the interface between nodes s - 1 and s), grid-stride.
 // ---------------------------------------------------------------------------------------------
-template <int D, int M, int R>
+template <int D, int M, int R, bool Z>
 __device__ __forceinline__ void weno_dense_item(const DevP& P, long long t, double* s_st) {
   const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
   const int e0 = P.nx + (D == 0), e1 = P.ny + (D == 1);
@@ -282,21 +301,21 @@ __device__ __forceinline__ void weno_dense_item(const DevP& P, long long t, doub
   const long long n = pidx(P, i - (D == 0), j - (D == 1), k - (D == 2));       // left node of the interface
   double fw[5], lam[3];
   weno_stencil<D, M, R>(P, n, s, s_st + threadIdx.x, lam);
-  weno_flux<D, M, R>(P, lam, fw, s_st + threadIdx.x);
+  weno_flux<D, M, R, Z>(P, lam, fw, s_st + threadIdx.x);
   double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
 #pragma unroll
   for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q];
 }
 
-template <int M, int R>
+template <int M, int R, bool Z>
 __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_kernel(const DevP P) {
   __shared__ double s_st[6 * 2 * M * WTH];
   const long long a = (long long)P.nx * P.ny * P.nz;
   const long long n0 = a + (long long)P.ny * P.nz, n1 = a + (long long)P.nx * P.nz, n2 = a + (long long)P.nx * P.ny;
   const long long stride = (long long)gridDim.x * WTH;
-  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n0; t += stride) weno_dense_item<0, M, R>(P, t, s_st);
-  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n1; t += stride) weno_dense_item<1, M, R>(P, t, s_st);
-  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n2; t += stride) weno_dense_item<2, M, R>(P, t, s_st);
+  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n0; t += stride) weno_dense_item<0, M, R, Z>(P, t, s_st);
+  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n1; t += stride) weno_dense_item<1, M, R, Z>(P, t, s_st);
+  for (long long t = (long long)blockIdx.x * WTH + threadIdx.x; t < n2; t += stride) weno_dense_item<2, M, R, Z>(P, t, s_st);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -305,19 +324,19 @@ __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_kernel(const DevP 
 // whatever the activation pattern.  Persistent blocks walk groups of WTH consecutive list entries
 // (consecutive entries are mostly consecutive nodes: coalesced stencil loads), directions one after the other.
 // ---------------------------------------------------------------------------------------------
-template <int D, int M, int R>
+template <int D, int M, int R, bool Z>
 __device__ __forceinline__ void weno_list_item(const DevP& P, long long n, double* s_st) {
   const long long s = D == 0 ? 1 : (D == 1 ? P.sy : P.sz);
   double fw[5], fc[5], lam[3];
   weno_stencil<D, M, R>(P, n, s, s_st + threadIdx.x, lam);
   central_flux_st<D, M>(P, fc, s_st + threadIdx.x);        // first: its registers are free before the WENO rows are live
-  weno_flux<D, M, R>(P, lam, fw, s_st + threadIdx.x);
+  weno_flux<D, M, R, Z>(P, lam, fw, s_st + threadIdx.x);
   double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
 #pragma unroll
   for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q] - fc[q];
 }
 
-template <int M, int R>
+template <int M, int R, bool Z>
 __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_list_kernel(const DevP P) {
   __shared__ double s_st[6 * 2 * M * WTH];
   const int c0 = P.counters[C_NIFACE], c1 = P.counters[C_NIFACE + 1], c2 = P.counters[C_NIFACE + 2];
@@ -347,9 +366,9 @@ __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_list_kernel(const 
   for (int it = 0; group_of(it) < gt; ++it) {
     const int n_nxt = fetch(group_of(it + 1), d_nxt);
     if (n_cur >= 0) {
-      if (d_cur == 0) weno_list_item<0, M, R>(P, n_cur, s_st);
-      else if (d_cur == 1) weno_list_item<1, M, R>(P, n_cur, s_st);
-      else weno_list_item<2, M, R>(P, n_cur, s_st);
+      if (d_cur == 0) weno_list_item<0, M, R, Z>(P, n_cur, s_st);
+      else if (d_cur == 1) weno_list_item<1, M, R, Z>(P, n_cur, s_st);
+      else weno_list_item<2, M, R, Z>(P, n_cur, s_st);
     }
     n_cur = n_nxt; d_cur = d_nxt;
   }
@@ -403,11 +422,16 @@ __global__ void __launch_bounds__(128) corr_gather_kernel(const DevP P) {
 }
 
 // -------------------------------------------------------------------------- launch
+template <int M, int R, bool Z>
+static int launch_weno_Z(const DevP& P, cudaStream_t st) {
+  if (P.flux_mode == FLUX_HYBRID) weno_list_kernel<M, R, Z><<<P.nsm * WenoOcc<R>::MINB, WTH, 0, st>>>(P);
+  else weno_kernel<M, R, Z><<<P.nsm * WenoOcc<R>::MINB * 4, WTH, 0, st>>>(P);
+  return 1;
+}
 template <int M, int R>
 static int launch_weno_T(const DevP& P, cudaStream_t st) {
-  if (P.flux_mode == FLUX_HYBRID) weno_list_kernel<M, R><<<P.nsm * WenoOcc<R>::MINB, WTH, 0, st>>>(P);
-  else weno_kernel<M, R><<<P.nsm * WenoOcc<R>::MINB * 4, WTH, 0, st>>>(P);
-  return 1;
+  if (P.weno_z && R > 1) return launch_weno_Z<M, R, true>(P, st);     // (first order has no weights)
+  return launch_weno_Z<M, R, false>(P, st);
 }
 
 int launch_corr(const DevP& P, cudaStream_t st) {

@@ -209,6 +209,19 @@ def test_invalid_orders_are_rejected_at_init(S):
         assert e.value.code == binding.STREAMS_EINVAL
 
 
+# ---- WENO-Z weights (S19)
+@pytest.mark.parametrize("m", [2, 3, 4])
+def test_weno_z_hybrid_and_full_weno(S, m):
+    case = W.isotropic_turbulence(nx=40, ny=37, nz=35, mach_t=0.6, k0=3.0, kmax=8, seed=81, dilatational=0.5)
+    case = _with_orders(case, m).replace(weno_variant=1)
+    check_case(S, case, 8, expect_activation=(0.002, 0.8))
+    check_case(S, case.replace(flux_mode=W.FLUX_WENO, visc_law=W.VISC_NONE, name=case.name + "_dense"), 4)
+
+
+def test_weno_z_channel_mixed_orders(S):
+    check_case(S, W.channel(40, 36, 34, seed=82).replace(weno_variant=1, central_order=6, weno_order=3), 6)
+
+
 # ---- branches the round-1 suite did not reach on the GPU
 def test_power_law_viscosity(S):
     """STREAMS_VISC_POWER with a non-zero exponent and T_ref != 1 (device pow vs the oracle's std::pow)."""

@@ -195,25 +195,47 @@ def test_discrete_conservation_on_the_gpu(S):
         gpu.destroy()
 
 
-def test_bulk_flow_controller_holds_the_channel_flow_rate(S):
-    """paper_2304_05494_b200.forcing: the unforced channel loses bulk momentum to wall friction; with the controller
-    (library sums + streams_set_body_force every step) it stays at its target and the force settles at the friction level."""
-    from paper_2304_05494_b200.forcing import BulkFlowController
+def test_bulk_flow_controller_against_the_oracle(S):
+    """streams_step_forced (device-side sums + one-thread controller, no host round trip per step) against the oracle's
+    controller (reading S18) on a channel: same fields, same force, step by step and in one multi-step call."""
     case = W.channel(48, 40, 36, seed=61)
     free = S(case)
     p0 = free.get_sums(0)[1]
-    free.step(30)
+    free.step(20)
     loss = 1.0 - free.get_sums(0)[1] / p0
     free.destroy()
     assert loss > 1e-4                                   # friction is at work
+    gpu, ora = S(case), _oracle(case)
+    for n in (1, 1, 3, 15):
+        dt_g, t_g, g_g = gpu.step_forced(n)
+        dt_o, t_o, g_o = ora.step_forced(n)
+        assert abs(dt_g - dt_o) <= 1e-12 * dt_o and abs(t_g - t_o) <= 1e-12 * t_o
+        assert abs(g_g[0] - g_o[0]) <= 1e-8 * abs(g_o[0]) and g_g[1] == 0.0 and g_g[2] == 0.0, (g_g, g_o)
+    _cmp_fields(gpu, ora, case)
+    assert g_g[0] > 0.0
+    assert abs(gpu.get_sums(0)[1] / p0 - 1.0) < 0.02 * loss            # held at its target
+    # a target given later moves the bulk momentum there within a step (deadbeat up to the change of the friction)
+    gpu.step_forced(1, 0, 1.01 * p0); ora.step_forced(1, 0, 1.01 * p0)
+    gpu.step_forced(2); ora.step_forced(2)
+    assert abs(gpu.get_sums(0)[1] / (1.01 * p0) - 1.0) < 1e-4
+    _cmp_fields(gpu, ora, case)
+    # streams_set_body_force takes the acceleration back to the host
+    gpu.set_body_force((0.0, 0.0, 0.0)); ora.close()
+    gpu.step(1)
+    gpu.destroy()
+
+
+def test_bulk_flow_controller_is_deadbeat_without_friction(S):
+    """Uniform flow in an inviscid periodic box: on target one step after the controller saw the deviation."""
+    one = np.ones((16, 16, 16))
+    case = W.Case(name="ctrl", nx=16, ny=16, nz=16, lx=1.0, ly=1.0, lz=1.0, dt_fixed=1e-2,
+                  w0=W.conserved_from_primitive(1.3 * one, 0.5 * one, 0 * one, 0 * one, 1.1 * one, 1.4))
     gpu = S(case)
-    ctl = BulkFlowController(gpu)
-    ratios = []
-    for _ in range(30):
-        _, _, g, ratio = ctl.step(1)
-        ratios.append(ratio)
-    assert max(abs(r - 1.0) for r in ratios[2:]) < 0.02 * loss, (loss, ratios[-5:])
-    assert g[0] > 0.0 and g[1] == 0.0 and g[2] == 0.0
+    p0 = gpu.get_sums(0)[1]
+    gpu.step_forced(1, 0, 1.1 * p0)
+    assert abs(gpu.get_sums(0)[1] / p0 - 1.0) < 1e-13
+    _, _, g = gpu.step_forced(1)
+    assert abs(gpu.get_sums(0)[1] / (1.1 * p0) - 1.0) < 1e-12 and abs(g[0]) < 1e-8
     gpu.destroy()
 
 

@@ -311,3 +311,66 @@ def test_sod_in_z_matches_sod_in_x():
     e_x, line_x, _ = _run_sod(100, 0)
     e_z, line_z, _ = _run_sod(100, 2)
     assert np.allclose(line_x, line_z, atol=1e-12)
+
+
+# ---- S19: WENO-Z weights (Borges et al. 2008, Castro et al. 2011)
+def _critical_point_derivative_error(r, variant, h, eps=1e-40):
+    """|(fhat_{i+1/2} - fhat_{i-1/2}) / h - f'(x_i)| at a node x_i where f' = 0 (point values = cell averages of the flux
+    primitive, so the difference of the two reconstructions is the finite-volume derivative)."""
+    from scipy.optimize import brentq
+    f = lambda x: np.sin(x) + 0.2 * np.cos(2 * x)
+    x0 = brentq(lambda x: np.cos(x) - 0.4 * np.sin(2 * x), 1.0, 1.6)
+    v = f(x0 + h * np.arange(-r, r))
+    if variant < 0:
+        R = lambda vals: O.weno_reconstruct(vals, r, eps, linear=True)[0]
+    else:
+        R = lambda vals: O.weno_reconstruct_variant(vals, r, eps, variant)
+    return abs((R(v[1:2 * r]) - R(v[0:2 * r - 1])) / h)
+
+
+@pytest.mark.parametrize("r", [3, 4])
+def test_weno_z_keeps_the_linear_accuracy_at_a_critical_point(r):
+    """Where f' = 0 the Jiang-Shu weights leave the linear ones by O(dx) and the scheme loses accuracy (error constant
+    10x, r = 3) or order (5 instead of 7, r = 4); the Z weights stay within O(dx^(2r-4))... of the linear ones: the error of
+    the derivative is that of the linear (2r-1)-order scheme.  (Checked by mutation: a missing square of tau / (eps + beta) fails here, a tau taken
+    over part of the stencil fails the right-hand-side comparison below.)"""
+    for h in (0.05, 0.025):
+        lin = _critical_point_derivative_error(r, -1, h)
+        z = _critical_point_derivative_error(r, 1, h)
+        js = _critical_point_derivative_error(r, 0, h)
+        assert z <= 1.5 * lin, (r, h, z, lin)
+        assert js >= 5.0 * lin, (r, h, js, lin)
+    if r == 4:
+        e = [_critical_point_derivative_error(4, 1, h) for h in (0.1, 0.05)]
+        ej = [_critical_point_derivative_error(4, 0, h) for h in (0.1, 0.05)]
+        assert np.log2(e[0] / e[1]) > 6.5 and np.log2(ej[0] / ej[1]) < 5.6
+
+
+@pytest.mark.parametrize("r", [2, 3, 4])
+def test_weno_z_is_a_convex_essentially_non_oscillatory_reconstruction(r):
+    """Constants and polynomials of degree < r are reproduced (the weights sum to one); next to a jump the value comes
+    from the smooth side."""
+    rng = np.random.default_rng(60 + r)
+    assert O.weno_reconstruct_variant(np.full(2 * r - 1, 0.7), r) == pytest.approx(0.7, rel=1e-15)
+    x = sp.symbols("x")
+    for deg in range(r):
+        co = rng.uniform(-1, 1, deg + 1)
+        hpoly = sum(sp.Float(float(co[n])) * x ** n for n in range(deg + 1))
+        vals = [float(sp.integrate(hpoly, (x, int(j) - sp.Rational(1, 2), int(j) + sp.Rational(1, 2)))) for j in range(-(r - 1), r)]
+        assert abs(O.weno_reconstruct_variant(np.array(vals), r) - float(hpoly.subs(x, sp.Rational(1, 2)))) < 1e-12
+    left = np.ones(2 * r - 1)
+    left[r:] = 0.0                                   # jump just right of the interface: the upwind cells are all 1
+    assert abs(O.weno_reconstruct_variant(left, r) - 1.0) < 1e-6
+    right = np.zeros(2 * r - 1)
+    right[: r - 1] = 1.0                             # jump left of cell 0: only the rightmost sub-stencil is smooth
+    assert abs(O.weno_reconstruct_variant(right, r) - 0.0) < 1e-6
+
+
+def test_weno_z_changes_the_flux_only_where_the_weights_matter():
+    """Full-WENO right-hand side of a smooth field: Z and Jiang-Shu agree to the size of the nonlinear-weight error
+    (both are fifth-order schemes there), and differ next to a steep gradient."""
+    case = W.isotropic_turbulence(nx=24, ny=24, nz=24, mach_t=0.3, k0=2.0, kmax=3, seed=7, viscous=False, flux_mode=W.FLUX_WENO)
+    r_js = O.Oracle(case).rhs()
+    r_z = O.Oracle(case.replace(weno_variant=1)).rhs()
+    rel = np.max(np.abs(r_z - r_js)) / np.max(np.abs(r_js))
+    assert 1e-9 < rel < 5e-2, rel

@@ -64,6 +64,7 @@ class Case:
     flux_mode: int = FLUX_CENTRAL
     sensor_threshold: float = 0.2
     weno_eps: float = 1e-6
+    weno_variant: int = 0                    # 0: Jiang-Shu weights, 1: WENO-Z
     cfl: float = 0.5
     dt_fixed: float = 0.0
     dt_every: int = 1
