@@ -308,6 +308,18 @@ def run_ours(args):
         gpu.set_mask_override(imposed)
     state_bytes = 5 * N * 8
 
+    if args.ignore_nan:                         # measurement builds (STREAMS_LIB=...) do not produce the solution
+        _step = gpu.step
+
+        def step_anyway(n):
+            try:
+                return _step(n)
+            except binding.StreamsError as e:
+                if e.code != binding.STREAMS_ENAN:
+                    raise
+                return float("nan"), float("nan")
+        gpu.step = step_anyway
+
     rep = replicas.Replicas(dist, dev)          # barrier + max over ranks (tests/test_replicas_gloo.py)
     max_over_ranks = rep.max_over_ranks
 
@@ -329,14 +341,14 @@ def run_ours(args):
         gpu.set_fields(w_start)                 # resets the activation totals too
         if profile:
             gpu.profile(True, max_records=10 * 3 * args.steps + 64)
-        l0 = gpu.kernel_launches()
+        l0, g0 = gpu.kernel_launches(), gpu.graph_launches()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         sync_all()
         e0.record(gpu.stream)
         gpu.step(args.steps)
         e1.record(gpu.stream)
         sync_all()
-        return max_over_ranks(e0.elapsed_time(e1)), gpu.kernel_launches() - l0
+        return max_over_ranks(e0.elapsed_time(e1)), (gpu.kernel_launches() - l0, gpu.graph_launches() - g0)
 
     # ---- device-resident throughput: inputs already in HBM, K steps in one streams_step call.  Two timed regions
     # of the same K steps from the same state: (1) the product path as a user runs it -> `value`; (2) the same with
@@ -380,7 +392,7 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
     e2e_value = world * N * n_e2e / (e2e_ms * 1e-3)
-    assert np.isfinite(h_a.numpy()).all()
+    assert args.ignore_nan or np.isfinite(h_a.numpy()).all()
 
     if rank != 0:
         gpu.destroy()
@@ -468,7 +480,9 @@ def run_ours(args):
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
                 "steps": n_e2e, "ms_per_step": e2e_ms / n_e2e},
-        "gpu_launches": launches,
+        "gpu_launches": launches[0],
+        "graph_launches": launches[1],
+        "library": os.environ.get("STREAMS_LIB") or "paper_2304_05494_b200/lib/libstreams.so",
         "roofline": roofline,
         "cpu_baseline": cpu,
         "point_stages_per_s": 3 * value,
@@ -494,6 +508,8 @@ def main():
     ap.add_argument("--repeats", type=int, default=5, help="timed regions from the same state; value = median")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ignore-nan", action="store_true",
+                    help="keep timing when the state goes non-finite (measurement builds selected with STREAMS_LIB)")
     ap.add_argument("--order-family", type=int, default=3, choices=[1, 2, 3, 4],
                     help="m: central order 2m / WENO order 2m-1 / viscous order 2m (default 3 = 6/5/6)")
     ap.add_argument("--flux-mode", default=None, choices=["central", "weno", "hybrid"], help="override the config's flux mode")

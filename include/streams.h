@@ -41,7 +41,8 @@ typedef struct streams_ctx streams_ctx; /* opaque, owned by the library */
 
 enum { STREAMS_OK = 0, STREAMS_EINVAL = -1, STREAMS_ENOMEM = -2, STREAMS_ECUDA = -3,
        STREAMS_ESTATE = -4, STREAMS_ENAN = -5 };
-enum { STREAMS_BC_PERIODIC = 0, STREAMS_BC_WALL_ISOTHERMAL = 1, STREAMS_BC_FREESTREAM = 2 };
+enum { STREAMS_BC_PERIODIC = 0, STREAMS_BC_WALL_ISOTHERMAL = 1, STREAMS_BC_FREESTREAM = 2,
+       STREAMS_BC_HALO = 3 /* bc_z only: ghost planes delivered by the caller's halo exchange (sharded stepping) */ };
 enum { STREAMS_VISC_NONE = 0, STREAMS_VISC_POWER = 1, STREAMS_VISC_SUTHERLAND = 2 };
 enum { STREAMS_FLUX_CENTRAL = 0, STREAMS_FLUX_WENO = 1, STREAMS_FLUX_HYBRID = 2 };
 enum { STREAMS_WENO_JS = 0, STREAMS_WENO_Z = 1 };
@@ -56,6 +57,8 @@ typedef struct {
                               /* the plane lies midway between the last node and the first ghost)*/
   int bc_x, bc_y_lo, bc_y_hi, bc_z; /* STREAMS_BC_*; walls are supported in y only              */
   double t_wall_lo, t_wall_hi;/* isothermal wall temperatures                                   */
+  int nz_global;              /* bc_z == STREAMS_BC_HALO: z nodes of the whole domain, of which this context holds  */
+                              /* nz planes (lz is the whole domain's length: dz = lz / nz_global); else 0 (= nz)    */
 } streams_grid;
 
 /* Gas and flow parameters (PAPER:36 ideal gas; PAPER:40 calorically perfect branch). */
@@ -116,6 +119,33 @@ int streams_rhs(streams_ctx* ctx, double* rhs_out_dev);
  * updated state for Inf / NaN, and the time-step rate of every node keeps a NaN (a negative pressure); the error
  * is reported when the call returns (the remaining steps of the call still run). */
 int streams_step(streams_ctx* ctx, int nsteps, double* dt_last, double* time);
+
+/* Sharded stepping (PAPER:85 GPU-aware halo communication, PAPER:507 synchronous mode): the domain is cut
+ * into z slabs, one context per slab (one process per GPU), each created with bc_z = STREAMS_BC_HALO and its own nz.
+ * A slab's z ghost planes then hold its neighbours' first / last `ng` interior planes and are written by the CALLER
+ * (a peer copy or an NCCL send / receive of the slabs below), never by the library.  One RK3 step of a slab is, for
+ * stage = 0, 1, 2:
+ *     streams_shard_fill(ctx, stage, &rate_is_local)   ghost fill of the other directions, primitives
+ *       [stage 0, *rate_is_local != 0: max-reduce the double at STREAMS_HALO_RATE over all slabs, in place]
+ *       [exchange STREAMS_HALO_PRIMS]
+ *     streams_shard_sensor(ctx, stage)                 step scalars (stage 0), sensor, dilatation
+ *       [exchange STREAMS_HALO_DIV and STREAMS_HALO_MASK]
+ *     streams_shard_rhs(ctx, stage)                    flags, WENO fluxes, fused RHS + update; primitive buffers swap
+ * and streams_shard_finish after the last step of a batch (synchronises; dt, time, STREAMS_ENAN as streams_step).
+ * Every node is computed by the same arithmetic as in a single context, so a sharded run reproduces the single-GPU
+ * run bit for bit (tests/test_gpu_sharded.py).  Only z is cut; x and y keep their boundary conditions.
+ * streams_halo_slabs(what): DEVICE pointers of the slabs to exchange for the CURRENT state (call it after every
+ * streams_shard_rhs: the primitive buffers swap): *lo_send = this slab's first ng interior planes (they become the
+ * upper ghosts of the slab below), *lo_recv = its lower ghost planes, *hi_send / *hi_recv likewise at the upper end;
+ * each is `nfields` pieces of `slab_bytes` contiguous bytes, `field_stride_bytes` apart (whole padded planes: the x / y
+ * ghosts travel with them).  STREAMS_HALO_RATE: *lo_send = the local time-step rate (8 bytes), nothing else. */
+enum { STREAMS_HALO_PRIMS = 0, STREAMS_HALO_DIV = 1, STREAMS_HALO_MASK = 2, STREAMS_HALO_RATE = 3 };
+int streams_shard_fill(streams_ctx* ctx, int stage, int* rate_is_local);
+int streams_shard_sensor(streams_ctx* ctx, int stage);
+int streams_shard_rhs(streams_ctx* ctx, int stage);
+int streams_shard_finish(streams_ctx* ctx, double* dt_last, double* time);
+int streams_halo_slabs(streams_ctx* ctx, int what, void** lo_send, void** lo_recv, void** hi_send, void** hi_recv,
+                       size_t* slab_bytes, int* nfields, size_t* field_stride_bytes);
 
 /* Copy the conserved state out, w_out[5][nz][ny][nx].  dst_is_device: 0 = HOST, 1 = DEVICE. */
 int streams_get_fields(streams_ctx* ctx, double* w_out, int dst_is_device);

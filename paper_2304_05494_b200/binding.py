@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "lib", "libstreams.so")
 
 STREAMS_OK, STREAMS_EINVAL, STREAMS_ENOMEM, STREAMS_ECUDA, STREAMS_ESTATE, STREAMS_ENAN = 0, -1, -2, -3, -4, -5
 EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "streams_rhs", "streams_step",
-           "streams_step_forced", "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
+           "streams_step_forced", "streams_shard_fill", "streams_shard_sensor", "streams_shard_rhs",
+           "streams_shard_finish", "streams_halo_slabs", "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches", "streams_graph_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
            "streams_measure_fp64_scratch_bytes",
@@ -31,7 +32,7 @@ class streams_grid(C.Structure):
                 ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
                 ("y_nodes", _dp), ("y_wall_lo", C.c_double), ("y_wall_hi", C.c_double),
                 ("bc_x", C.c_int), ("bc_y_lo", C.c_int), ("bc_y_hi", C.c_int), ("bc_z", C.c_int),
-                ("t_wall_lo", C.c_double), ("t_wall_hi", C.c_double)]
+                ("t_wall_lo", C.c_double), ("t_wall_hi", C.c_double), ("nz_global", C.c_int)]
 
 
 class streams_gas(C.Structure):
@@ -51,11 +52,14 @@ class streams_scheme(C.Structure):
 _lib = None
 
 
-def load_library(path: str = LIB_PATH):
-    """dlopen libstreams.so and declare the prototypes of include/streams.h."""
+def load_library(path: str = None):
+    """dlopen libstreams.so and declare the prototypes of include/streams.h.  STREAMS_LIB=<path> selects another
+    build of the same library (measurement builds of paper_2304_05494_b200.build --tag)."""
     global _lib
     if _lib is not None:
         return _lib
+    if path is None:
+        path = os.environ.get("STREAMS_LIB") or LIB_PATH
     if not os.path.exists(path):
         raise RuntimeError(f"{path} is missing: build it with `python -m paper_2304_05494_b200.build` "
                            "(there is no CPU fallback)")
@@ -69,6 +73,11 @@ def load_library(path: str = LIB_PATH):
     lib.streams_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
     lib.streams_step_forced.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp, _dp, _dp]
     lib.streams_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+    lib.streams_shard_fill.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int)]
+    lib.streams_shard_sensor.argtypes = [C.c_void_p, C.c_int]
+    lib.streams_shard_rhs.argtypes = [C.c_void_p, C.c_int]
+    lib.streams_shard_finish.argtypes = [C.c_void_p, _dp, _dp]
+    lib.streams_halo_slabs.argtypes = [C.c_void_p, C.c_int] + [C.POINTER(C.c_void_p)] * 4 + [C.POINTER(C.c_size_t), C.POINTER(C.c_int), C.POINTER(C.c_size_t)]
     lib.streams_get_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_set_mask_override.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
     lib.streams_get_sums.argtypes = [C.c_void_p, C.c_int, _dp]
@@ -97,7 +106,7 @@ def structs_from_case(case):
     """workloads.Case -> (streams_grid, streams_gas, streams_scheme, keepalive)."""
     g, a, s = streams_grid(), streams_gas(), streams_scheme()
     for n in ("nx", "ny", "nz", "lx", "ly", "lz", "y_wall_lo", "y_wall_hi", "bc_x", "bc_y_lo", "bc_y_hi", "bc_z",
-              "t_wall_lo", "t_wall_hi"):
+              "t_wall_lo", "t_wall_hi", "nz_global"):
         setattr(g, n, getattr(case, n))
     keep = None
     if case.y_nodes is not None:
@@ -225,6 +234,40 @@ class Streams:
         self._check(self.lib.streams_step_forced(self.h, int(nsteps), int(direction), C.c_double(target), C.byref(dt),
                                                  C.byref(t), C.cast(g, _dp)))
         return dt.value, t.value, list(g)
+
+    # -- sharded stepping (one context per z slab; paper_2304_05494_b200/sharded.py drives these)
+    def shard_fill(self, stage):
+        flag = C.c_int()
+        self._check(self.lib.streams_shard_fill(self.h, int(stage), C.byref(flag)))
+        return bool(flag.value)
+
+    def shard_sensor(self, stage):
+        self._check(self.lib.streams_shard_sensor(self.h, int(stage)))
+
+    def shard_rhs(self, stage):
+        self._check(self.lib.streams_shard_rhs(self.h, int(stage)))
+
+    def shard_finish(self):
+        dt, t = C.c_double(), C.c_double()
+        self._check(self.lib.streams_shard_finish(self.h, C.byref(dt), C.byref(t)))
+        return dt.value, t.value
+
+    def halo_slabs(self, what):
+        """Torch views (no copies) of the slabs to exchange: dict lo_send / lo_recv / hi_send / hi_recv, each a list of
+        one 1-D uint8 tensor per field, aliasing the workspace."""
+        ptrs = [C.c_void_p() for _ in range(4)]
+        nbytes, nf, stride = C.c_size_t(), C.c_int(), C.c_size_t()
+        self._check(self.lib.streams_halo_slabs(self.h, int(what), *[C.byref(p) for p in ptrs], C.byref(nbytes), C.byref(nf),
+                                                C.byref(stride)))
+        base = self.workspace.data_ptr()
+        out = {}
+        for name, p in zip(("lo_send", "lo_recv", "hi_send", "hi_recv"), ptrs):
+            if not p.value:
+                out[name] = []
+                continue
+            off = p.value - base
+            out[name] = [self.workspace[off + f * stride.value: off + f * stride.value + nbytes.value] for f in range(nf.value)]
+        return out
 
     def get_fields(self, out=None):
         if out is None:

@@ -1,6 +1,10 @@
 """Build libstreams.so (sm_100a) in-tree with nvcc.
 
-    python -m paper_2304_05494_b200.build [--force] [--verbose]
+    python -m paper_2304_05494_b200.build [--force] [--verbose] [--define NAME[=VALUE] ...] [--tag TAG]
+
+--define adds -DNAME[=VALUE] to every translation unit and --tag TAG writes the result to lib_TAG/libstreams.so instead
+of lib/ (measurement builds, e.g. --define STREAMS_MARCH_SKELETON --tag skeleton: the data movement of the fused RHS
+kernel without its stencil arithmetic; select it at run time with STREAMS_LIB=<path>).
 
 streams_canon.cu is compiled with -fmad=false (canonical, contraction-free evaluation of the
 sensor path); the other translation units use the default FMA contraction.
@@ -30,16 +34,18 @@ def _newest_source() -> float:
     return t
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    os.makedirs(OUT, exist_ok=True)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
-        return LIB
+def build(force: bool = False, verbose: bool = False, defines=(), tag: str = "") -> str:
+    out_dir = OUT if not tag else os.path.join(HERE, "lib_" + tag)
+    lib = os.path.join(out_dir, "libstreams.so")
+    os.makedirs(out_dir, exist_ok=True)
+    if not force and not defines and os.path.exists(lib) and os.path.getmtime(lib) >= _newest_source():
+        return lib
     nvcc = os.environ.get("NVCC", "nvcc")
     objs = []
     procs = []
     for src, extra in UNITS:
-        obj = os.path.join(OUT, src.replace(".cu", ".o"))
-        cmd = [nvcc, *COMMON, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(out_dir, src.replace(".cu", ".o"))
+        cmd = [nvcc, *COMMON, *extra, *["-D" + d for d in defines], "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd))
@@ -48,9 +54,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for cmd, p in procs:
         if p.wait() != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    subprocess.check_call([nvcc, "-shared", *ARCH, "-o", LIB, *objs])
-    return LIB
+    subprocess.check_call([nvcc, "-shared", *ARCH, "-o", lib, *objs])
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    argv = sys.argv[1:]
+    defs = [argv[i + 1] for i, a in enumerate(argv) if a == "--define" and i + 1 < len(argv)]
+    tags = [argv[i + 1] for i, a in enumerate(argv) if a == "--tag" and i + 1 < len(argv)]
+    print(build(force="--force" in argv, verbose="--verbose" in argv, defines=defs, tag=tags[0] if tags else ""))

@@ -45,6 +45,7 @@ void fd2(int L, double* b) {
 }
 
 bool valid_bc(int b) { return b == STREAMS_BC_PERIODIC || b == STREAMS_BC_WALL_ISOTHERMAL || b == STREAMS_BC_FREESTREAM; }
+bool valid_bc_z(int b) { return valid_bc(b) || b == STREAMS_BC_HALO; }
 
 // Validates the problem and lays out the workspace.  Returns NULL on success, else a message.
 const char* plan(const streams_grid* g, const streams_gas* gas, const streams_scheme* sc, Sizes& S) {
@@ -53,7 +54,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   if (((long long)g->nx + 48) * ((long long)g->ny + 8) * ((long long)g->nz + 8) > 2000000000LL)
     return "grid too large for 32-bit node indices";
   if (!(g->lx > 0) || !(g->lz > 0)) return "lx, lz must be positive";
-  if (!valid_bc(g->bc_x) || !valid_bc(g->bc_y_lo) || !valid_bc(g->bc_y_hi) || !valid_bc(g->bc_z)) return "bad bc code";
+  if (!valid_bc(g->bc_x) || !valid_bc(g->bc_y_lo) || !valid_bc(g->bc_y_hi) || !valid_bc_z(g->bc_z)) return "bad bc code";
   if (g->bc_x == STREAMS_BC_WALL_ISOTHERMAL || g->bc_z == STREAMS_BC_WALL_ISOTHERMAL) return "walls are supported in y only";
   if ((g->bc_y_lo == STREAMS_BC_PERIODIC) != (g->bc_y_hi == STREAMS_BC_PERIODIC)) return "y periodic on one side only";
   if (g->bc_y_lo == STREAMS_BC_PERIODIC && !(g->ly > 0)) return "ly must be positive";
@@ -76,6 +77,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   // three ghost layers, four when an order of the scheme reaches further (central / viscous 8, WENO 7)
   S.ng = std::max(3, std::max(S.L, std::max(S.Lv, S.r)));
   if (g->nx < S.ng || g->ny < S.ng || g->nz < S.ng) return "each extent must be at least the ghost width";
+  if (g->bc_z == STREAMS_BC_HALO && g->nz_global != 0 && g->nz_global < g->nz) return "nz_global must be at least nz";
   if (g->ny + 2 * S.ng > 65535 || g->nz + 2 * S.ng > 65535) return "ny and nz (with ghosts) must not exceed 65535";
   S.ox = 16;                                              // interior i = 0 starts a 128-byte line
   S.px = (int)align_up((size_t)S.ox + g->nx + S.ng, 16);
@@ -242,22 +244,42 @@ cudaError_t prof_drain(streams_ctx* ctx) {
 // After an updating stage the fused RHS kernel has already written the primitives of every interior node of the
 // new state (and, on request, reduced its time-step rate): only the ghost shell is left.  Otherwise (first
 // evaluation after streams_set_fields, or a dt wanted that no stage prepared) the full pass runs.
-int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta, bool step_start = false) {
+// The three parts of what a stage needs before its RHS kernels (a sharded run exchanges halo planes between them,
+// streams_shard_*): (1) ghost fill + primitives (+ the local time-step rate when no stage prepared it) ...
+int prepare_fill(streams_ctx* ctx, bool want_dt) {
   const DevP& P = ctx->P;
   cudaStream_t st = ctx->stream;
   const bool reduce_dt = want_dt && !(ctx->scheme.dt_fixed > 0.0) && !ctx->rate_ready;
+  int n;
+  if (ctx->prims_interior && !reduce_dt) n = timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
+  else n = timed(ctx, STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
+  ctx->prims_interior = true;
+  return n < 0 ? n : 0;
+}
+// ... (2) the step scalars at the start of a step (dt = CFL / rate, time, step count), then sensor / dilatation ...
+int prepare_sensor(streams_ctx* ctx, bool want_dt, bool theta, bool step_start) {
+  const DevP& P = ctx->P;
+  cudaStream_t st = ctx->stream;
   int rc = 0;
   auto run = [&](int kind, auto&& launch) { const int n = timed(ctx, kind, launch); if (n < 0 && rc == 0) rc = n; };
-  if (ctx->prims_interior && !reduce_dt) run(STREAMS_K_FILL_PRIM, [&] { return launch_fill_ghosts(P, st); });
-  else run(STREAMS_K_FILL_PRIM, [&] { return launch_fill_prim(P, reduce_dt, st); });
-  ctx->prims_interior = true;
   if (step_start) run(STREAMS_K_DT, [&] { return launch_dt(P, ctx->scheme.dt_fixed, want_dt, st); });
   if (want_dt) ctx->rate_ready = false;             // dt_finalize consumed (and zeroed) the rate
   const bool hyb = ctx->scheme.flux_mode == STREAMS_FLUX_HYBRID;
   const bool visc = ctx->gas.visc_law != STREAMS_VISC_NONE;
   if (hyb || visc || theta)
     run(STREAMS_K_SENSOR, [&] { return launch_sensor(P, ctx->maps[ctx->cur], ctx->S.L, hyb || theta, theta, st, false); });
-  if (hyb) run(STREAMS_K_FLAGS, [&] { return launch_flags(P, ctx->S.r, st); });
+  return rc;
+}
+// ... (3) interface flags and work lists from the node mask.
+int prepare_flags(streams_ctx* ctx) {
+  if (ctx->scheme.flux_mode != STREAMS_FLUX_HYBRID) return 0;
+  const int n = timed(ctx, STREAMS_K_FLAGS, [&] { return launch_flags(ctx->P, ctx->S.r, ctx->stream); });
+  return n < 0 ? n : 0;
+}
+int enqueue_prepare(streams_ctx* ctx, bool want_dt, bool theta, bool step_start = false) {
+  int rc = prepare_fill(ctx, want_dt);
+  if (rc == 0) rc = prepare_sensor(ctx, want_dt, theta, step_start);
+  if (rc == 0) rc = prepare_flags(ctx);
   return rc;
 }
 
@@ -295,24 +317,31 @@ int enqueue_rhs(streams_ctx* ctx, const StageArgs& sa) {
   return a < 0 ? a : (b < 0 ? b : (c < 0 ? c : a + b + c));
 }
 
-// the launches of one RK3 step: three stages of (ghost fill, step scalars, sensor, flags, WENO, gather, fused RHS + update)
-int enqueue_step(streams_ctx* ctx, bool want_dt, bool want_rate) {
+// the RHS kernels and the update of stage l (0, 1, 2); the primitive buffers swap
+int enqueue_stage_rhs(streams_ctx* ctx, int l, bool want_rate) {
   // Wray's low-storage RK3 (O5 / S12)
   const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
   const double rhk[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+  StageArgs sa;
+  sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
+  sa.r_dense = nullptr;
+  sa.q_out = ctx->qbuf[ctx->cur ^ 1];
+  sa.want_rate = (l == 2 && want_rate) ? 1 : 0;
+  sa.check_state = (l == 2);
+  const int rc = enqueue_rhs(ctx, sa);
+  if (rc < 0) return rc;
+  use_qbuf(ctx, ctx->cur ^ 1);                       // the updated state's primitives are in the other buffer
+  ctx->prims_interior = true;
+  if (sa.want_rate) ctx->rate_ready = true;
+  return 0;
+}
+
+// the launches of one RK3 step: three stages of (ghost fill, step scalars, sensor, flags, WENO, gather, fused RHS + update)
+int enqueue_step(streams_ctx* ctx, bool want_dt, bool want_rate) {
   for (int l = 0; l < 3; ++l) {
     int rc = enqueue_prepare(ctx, want_dt && l == 0, false, l == 0);
     if (rc < 0) return rc;
-    StageArgs sa;
-    sa.gam = gam[l]; sa.rhk = rhk[l]; sa.update_w = 1; sa.read_prev = (l > 0); sa.write_r = (l < 2);
-    sa.r_dense = nullptr;
-    sa.q_out = ctx->qbuf[ctx->cur ^ 1];
-    sa.want_rate = (l == 2 && want_rate) ? 1 : 0;
-    sa.check_state = (l == 2);
-    if ((rc = enqueue_rhs(ctx, sa)) < 0) return rc;
-    use_qbuf(ctx, ctx->cur ^ 1);                     // the updated state's primitives are in the other buffer
-    ctx->prims_interior = true;
-    if (sa.want_rate) ctx->rate_ready = true;
+    if ((rc = enqueue_stage_rhs(ctx, l, want_rate)) < 0) return rc;
   }
   return 0;
 }
@@ -378,7 +407,7 @@ int streams_init(streams_ctx** out, const streams_grid* grid, const streams_gas*
   P.eta_y_c = met; P.eta_y_v = met + grid->ny; P.eta_yy_v = met + 2 * (size_t)grid->ny;
   P.scal = (double*)(ctx->base + S.off_scal);
   P.inv_dx = (double)grid->nx / grid->lx;
-  P.inv_dz = (double)grid->nz / grid->lz;
+  P.inv_dz = (double)(grid->bc_z == STREAMS_BC_HALO && grid->nz_global > 0 ? grid->nz_global : grid->nz) / grid->lz;
   fd1(S.L, P.a1); fd1(S.Lv, P.a1v); fd2(S.Lv, P.b2v);
   P.sbv = 0.0;
   for (int l = 0; l < 4; ++l) {
@@ -621,6 +650,85 @@ int streams_step_forced(streams_ctx* ctx, int nsteps, int direction, double targ
     target = std::nan("");
   }
   return finish_steps(ctx, dt_last, time, accel3_out);
+}
+
+// ---- sharded stepping: one context per z slab, the caller exchanges halo planes between the phases
+static bool shard_want_dt(const streams_ctx* ctx) { return (ctx->step_count % ctx->scheme.dt_every) == 0; }
+static bool shard_want_rate(const streams_ctx* ctx) {
+  return !(ctx->scheme.dt_fixed > 0.0) && ((ctx->step_count + 1) % ctx->scheme.dt_every) == 0;
+}
+static int shard_check(streams_ctx* ctx, int stage) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (!ctx->have_fields) return fail(ctx, STREAMS_ESTATE, "no fields set");
+  if (stage < 0 || stage > 2) return fail(ctx, STREAMS_EINVAL, "stage must be 0, 1 or 2");
+  return STREAMS_OK;
+}
+
+int streams_shard_fill(streams_ctx* ctx, int stage, int* rate_is_local) {
+  int rc = shard_check(ctx, stage);
+  if (rc != STREAMS_OK) return rc;
+  if (stage == 0) ctx->r_valid = false;
+  const bool want_dt = stage == 0 && shard_want_dt(ctx);
+  if (rate_is_local) *rate_is_local = (want_dt && !(ctx->scheme.dt_fixed > 0.0)) ? 1 : 0;
+  if ((rc = prepare_fill(ctx, want_dt)) < 0) return launch_fail(ctx, rc);
+  CU(cudaGetLastError());
+  return STREAMS_OK;
+}
+
+int streams_shard_sensor(streams_ctx* ctx, int stage) {
+  int rc = shard_check(ctx, stage);
+  if (rc != STREAMS_OK) return rc;
+  if ((rc = prepare_sensor(ctx, stage == 0 && shard_want_dt(ctx), false, stage == 0)) < 0) return launch_fail(ctx, rc);
+  CU(cudaGetLastError());
+  return STREAMS_OK;
+}
+
+int streams_shard_rhs(streams_ctx* ctx, int stage) {
+  int rc = shard_check(ctx, stage);
+  if (rc != STREAMS_OK) return rc;
+  if ((rc = prepare_flags(ctx)) < 0) return launch_fail(ctx, rc);
+  if ((rc = enqueue_stage_rhs(ctx, stage, shard_want_rate(ctx))) < 0) return launch_fail(ctx, rc);
+  if (stage == 2) ctx->step_count += 1;
+  CU(cudaGetLastError());
+  return STREAMS_OK;
+}
+
+int streams_shard_finish(streams_ctx* ctx, double* dt_last, double* time) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  return finish_steps(ctx, dt_last, time, nullptr);
+}
+
+int streams_halo_slabs(streams_ctx* ctx, int what, void** lo_send, void** lo_recv, void** hi_send, void** hi_recv,
+                       size_t* slab_bytes, int* nfields, size_t* field_stride_bytes) {
+  if (!ctx) return fail(ctx, STREAMS_EINVAL, "null context");
+  if (what != STREAMS_HALO_PRIMS && what != STREAMS_HALO_DIV && what != STREAMS_HALO_MASK && what != STREAMS_HALO_RATE)
+    return fail(ctx, STREAMS_EINVAL, "bad halo selector");
+  const DevP& P = ctx->P;
+  char* base;
+  size_t elem = 8, fstride = (size_t)P.fs * 8;
+  int nf = 1;
+  if (what == STREAMS_HALO_RATE) {                   // the local time-step rate (one double): max-reduce it over the ranks
+    if (lo_send) *lo_send = P.scal + S_RATE;
+    if (lo_recv) *lo_recv = nullptr;
+    if (hi_send) *hi_send = nullptr;
+    if (hi_recv) *hi_recv = nullptr;
+    if (slab_bytes) *slab_bytes = 8;
+    if (nfields) *nfields = 1;
+    if (field_stride_bytes) *field_stride_bytes = 0;
+    return STREAMS_OK;
+  }
+  if (what == STREAMS_HALO_PRIMS) { base = (char*)P.q; nf = NQ; }
+  else if (what == STREAMS_HALO_DIV) { base = (char*)P.div; }
+  else { base = (char*)P.mask; elem = 1; fstride = 0; }
+  const size_t plane = (size_t)P.sz * elem, slab = (size_t)P.ng * plane;
+  if (lo_recv) *lo_recv = base;                                        // ghost planes k = -ng .. -1
+  if (lo_send) *lo_send = base + slab;                                 // interior planes 0 .. ng-1
+  if (hi_send) *hi_send = base + (size_t)P.nz * plane;                 // interior planes nz-ng .. nz-1
+  if (hi_recv) *hi_recv = base + (size_t)(P.nz + P.ng) * plane;        // ghost planes nz .. nz+ng-1
+  if (slab_bytes) *slab_bytes = slab;
+  if (nfields) *nfields = nf;
+  if (field_stride_bytes) *field_stride_bytes = fstride;
+  return STREAMS_OK;
 }
 
 int streams_get_sensor(streams_ctx* ctx, double* theta_out, unsigned char* mask_out, int dst_is_device) {

@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) scalar_ghost_kernel(const DevP P) {
     j = m < g ? m - g : P.ny + (m - g);
     if (j < 0) js = P.bc_y_lo == BC_PERIODIC ? j + P.ny : 0;
     else js = P.bc_y_hi == BC_PERIODIC ? j - P.ny : P.ny - 1;
-  } else if ((t -= nY) < nZ) {
+  } else if ((t -= nY) < nZ && P.bc_z != BC_HALO) {
     i = is = (int)(t % P.nx);
     const long long t2 = t / P.nx;
     j = js = (int)(t2 % P.ny);
@@ -150,7 +150,7 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
   const unsigned char* __restrict__ ovr_p = P.mask_ovr ? P.mask_ovr + ncol : nullptr;
   // does this thread own x / y face ghosts (DevP::sown: the kernel writes them itself)?
   const bool per_z = P.bc_z == BC_PERIODIC;
-  const bool zface = P.sown != 0;
+  const bool zface = P.sown != 0 && P.bc_z != BC_HALO;    // (halo planes in z come from the neighbouring slab)
   const bool gplan = P.sown && active &&
                      ((P.bc_x == BC_PERIODIC ? (i < NG || i >= P.nx - NG) : (i == 0 || i == P.nx - 1)) ||
                       (j < NG && P.bc_y_lo == BC_PERIODIC) || (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) ||

@@ -93,7 +93,8 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   const int i = ip - P.ox, j = (int)blockIdx.y - P.ng, k = (int)blockIdx.z - P.ng;
   double rmax = 0.0;
-  if (i >= -P.ng && i < P.nx + P.ng) rmax = fill_node<VISC, STORE_C, DT>(P, i, j, k);
+  const bool halo_plane = P.bc_z == BC_HALO && (k < 0 || k >= P.nz);      // a neighbour's planes: not ours to fill
+  if (i >= -P.ng && i < P.nx + P.ng && !halo_plane) rmax = fill_node<VISC, STORE_C, DT>(P, i, j, k);
   if (DT) {
     __shared__ unsigned long long sm[4];
     block_rate_max(P, rmax, sm);
@@ -107,7 +108,7 @@ __global__ void __launch_bounds__(128) fill_prim_kernel(const DevP P) {
 template <bool VISC, bool STORE_C>
 __global__ void __launch_bounds__(128) fill_ghost_kernel(const DevP P) {
   const int g = P.ng, wx = P.nx + 2 * g;
-  const long long nZ = P.own_z ? 0 : 2LL * g * P.py * wx, nY = P.own_y ? 0 : (long long)P.nz * 2 * g * wx,
+  const long long nZ = (P.own_z || P.bc_z == BC_HALO) ? 0 : 2LL * g * P.py * wx, nY = P.own_y ? 0 : (long long)P.nz * 2 * g * wx,
                   nX = P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g;
   long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int i, j, k;
@@ -155,7 +156,7 @@ int launch_fill_prim(const DevP& P, bool with_dt, cudaStream_t st) {
 int launch_fill_ghosts(const DevP& P, cudaStream_t st) {
   const int g = P.ng;
   const long long wx = P.nx + 2 * g;
-  const long long total = (P.own_z ? 0 : 2LL * g * P.py * wx) + (P.own_y ? 0 : (long long)P.nz * 2 * g * wx) +
+  const long long total = ((P.own_z || P.bc_z == BC_HALO) ? 0 : 2LL * g * P.py * wx) + (P.own_y ? 0 : (long long)P.nz * 2 * g * wx) +
                           (P.own_x ? 0 : (long long)P.nz * P.ny * 2 * g);
   if (total == 0) return 0;
   dim3 b(128), gr((unsigned)((total + 127) / 128));

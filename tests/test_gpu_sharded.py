@@ -1,0 +1,71 @@
+"""The sharded step on ONE GPU: the z slabs of a run live in one process and are stepped in lockstep on one stream
+(nothing waits on anything else: the phases of all slabs are enqueued in order), their halo planes moved by device
+copies through the same exchange routine that moves them over NCCL between processes.  Every node is computed by the
+same arithmetic as in a single context, so the result must equal the single-context run BIT FOR BIT -- fields, time
+step and time -- whatever the number of slabs."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    from paper_2304_05494_b200 import build, binding, sharded
+    build.build()
+    return binding, sharded
+
+
+def _single(binding, case, nsteps):
+    g = binding.Streams(case)
+    dt, t = g.step(nsteps)
+    w = g.get_fields()
+    g.destroy()
+    return dt, t, w
+
+
+def _sharded(sharded, case, world, nsteps, chunks=(None,)):
+    s = sharded.ShardedStreams(case, world, list(range(world)))
+    dt = t = None
+    n = nsteps
+    for c in chunks:
+        k = n if c is None else c
+        dt, t = s.step(k)
+        n -= k
+    w = s.get_fields()
+    launches = s.kernel_launches()
+    s.destroy()
+    return dt, t, w, launches
+
+
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_hybrid_viscous_box_equals_the_single_context_run(mods, world):
+    binding, sharded = mods
+    case = W.isotropic_turbulence(nx=40, ny=36, nz=41, mach_t=0.6, k0=3.0, kmax=8, seed=91, dilatational=0.5)
+    dt0, t0, w0 = _single(binding, case, 6)
+    dt1, t1, w1, launches = _sharded(sharded, case, world, 6, chunks=(2, 1, 3))
+    assert launches > 0
+    assert dt1 == dt0 and t1 == t0
+    assert np.array_equal(w1, w0)
+
+
+def test_channel_with_walls_and_dt_every(mods):
+    """Walls in y (ghost fill of the other directions inside each slab), dt recomputed every third step."""
+    binding, sharded = mods
+    case = W.channel(48, 40, 36, seed=92).replace(dt_every=3)
+    dt0, t0, w0 = _single(binding, case, 7)
+    dt1, t1, w1, _ = _sharded(sharded, case, 3, 7)
+    assert dt1 == dt0 and t1 == t0 and np.array_equal(w1, w0)
+
+
+@pytest.mark.parametrize("mode", [W.FLUX_CENTRAL, W.FLUX_WENO])
+def test_other_flux_modes_and_four_ghost_layers(mods, mode):
+    binding, sharded = mods
+    case = W.isotropic_turbulence(nx=34, ny=33, nz=30, mach_t=0.4, k0=3.0, kmax=8, seed=93, flux_mode=mode,
+                                  viscous=(mode == W.FLUX_CENTRAL))
+    case = case.replace(central_order=8, weno_order=7, visc_order=8)
+    dt0, t0, w0 = _single(binding, case, 4)
+    dt1, t1, w1, _ = _sharded(sharded, case, 2, 4)
+    assert dt1 == dt0 and t1 == t0 and np.array_equal(w1, w0)

@@ -20,6 +20,7 @@ from typing import Optional
 import numpy as np
 
 BC_PERIODIC, BC_WALL_ISOTHERMAL, BC_FREESTREAM = 0, 1, 2
+BC_HALO = 3                                  # bc_z of a z slab of a sharded run: ghost planes come from the neighbours
 VISC_NONE, VISC_POWER, VISC_SUTHERLAND = 0, 1, 2
 FLUX_CENTRAL, FLUX_WENO, FLUX_HYBRID = 0, 1, 2
 
@@ -44,6 +45,7 @@ class Case:
     bc_z: int = BC_PERIODIC
     t_wall_lo: float = 1.0
     t_wall_hi: float = 1.0
+    nz_global: int = 0                       # z nodes of the whole domain when this case is a slab (bc_z = BC_HALO)
     # gas
     gamma: float = 1.4
     rgas: float = 1.0
