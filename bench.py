@@ -141,7 +141,7 @@ class ClockSampler:
 # (profiles/r1c_fp64_counts.md; static SASS counts overstate kernels with branches: the IEEE-divide slow paths and
 # the wall branch of fill_prim are rarely taken)
 FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 5, "corr_gather": 30,
-             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 115,
+             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 97,
              "prims": 60}      # prims: cons -> prim of the updated node in the fused RHS epilogue (shared reciprocal, no IEEE divide)
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
 
@@ -168,13 +168,14 @@ def work_model(case, act):
     I["fill_prim"] = (Np - N) * FP64_INST["fill_prim"]
     B["sensor"] = N * (24 + 8 + (1 if hyb else 0))             # read u v w, write div [mask]
     I["sensor"] = N * FP64_INST["sensor"]
-    B["flags"] = N * (1 + 1) + n_if * 4                        # read mask, write flags byte, append to the work lists
+    B["flags"] = N * (1 + 1) + (n_if + n_sh) * 4               # read mask, write flags byte, append to the four work lists
     I["flags"] = 0
     # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
     # read R_prev (stages 2, 3), write R (stages 1, 2)
     # (+ hybrid / WENO: the flag byte of every node and the 5 net corrections of every node next to a flagged interface)
     # + the primitives of the updated node (a2 of the next stage), written to the other q buffer
-    per_point = (48 if conv else 0) + (24 if visc else 0) + 40 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40 + 8 * nprim
+    # (w: four fields read -- the old density comes with the primitives --, five written)
+    per_point = (48 if conv else 0) + (24 if visc else 0) + 32 + 40 + (2.0 / 3.0) * 40 + (2.0 / 3.0) * 40 + 8 * nprim
     B["rhs_main"] = N * per_point + (N * 1 if hyb else 0) + n_sh * 40
     I["rhs_main"] = (N * FP64_INST["rhs_main_" + (("c" if conv else "") + ("v" if visc else "") or "0")]
                      + n_sh * FP64_INST["rhs_corr"] + N * (FP64_INST["prims"] + FP64_INST["fill_prim_dt"] / 3.0))
@@ -182,8 +183,8 @@ def work_model(case, act):
     # rest), a list entry, 5 flux values out
     B["weno"] = n_if * (56 + 4 + 40)                           # per timed group: the x, y and z launches of a stage
     I["weno"] = n_if * FP64_INST["weno_hybrid" if hyb else "weno_dense"]
-    # net correction per node: the flag byte of every node, every interface value once, 5 values out per flagged node
-    B["corr_gather"] = (N * 1 if hyb else 0) + n_if * 40 + n_sh * 40
+    # net correction per listed node: list entry + flag byte, every interface value once, 5 values out
+    B["corr_gather"] = (n_sh * 5 if hyb else 0) + n_if * 40 + n_sh * 40
     I["corr_gather"] = n_sh * FP64_INST["corr_gather"]
     B["dt"] = 0                                                # the rate is reduced inside fill_prim; this class is
     I["dt"] = 0                                                # the one-thread finalize (dt = CFL / rate)
@@ -498,6 +499,76 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------
+# sharded arm: ONE problem cut into z slabs, halo exchange per phase (strong scaling)
+# ------------------------------------------------------------------------------------------------
+def run_sharded(args):
+    """`--sharded`: the config's grid is cut into z slabs, one per rank (torchrun, NCCL point-to-point between
+    neighbours) or `--slabs S` slabs inside this process when there is one GPU (the copies are then device copies on one
+    stream; this measures what the phase structure and the exchange cost, not a speed-up).  value = points of the WHOLE
+    grid x K / max-over-ranks device time."""
+    import torch
+    from paper_2304_05494_b200 import build as kbuild, replicas, sharded
+
+    rank, world, local = replicas.rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libstreams has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        kbuild.build()
+    if dist is not None:
+        dist.barrier()
+    case = make_case(args.config)                   # every rank builds the same field and keeps its slab
+    nslabs = world if world > 1 else max(1, args.slabs)
+    ranks = [rank] if world > 1 else list(range(nslabs))
+    sh = sharded.ShardedStreams(case, nslabs, ranks, device=f"cuda:{local}", dist=dist)
+    rep = replicas.Replicas(dist, sh.device)
+    N = case.npoints
+    sh.step(args.warmup)
+    clocks = ClockSampler(local) if rank == 0 else None
+    reps = []
+    for _ in range(max(1, args.repeats)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        rep.barrier(); torch.cuda.synchronize(sh.device)
+        e0.record(sh.stream)
+        sh.step(args.steps)
+        e1.record(sh.stream)
+        rep.barrier(); torch.cuda.synchronize(sh.device)
+        reps.append(rep.max_over_ranks(e0.elapsed_time(e1)))
+    clk = clocks.stop() if clocks else None
+    ms = float(np.median(reps))
+    launches = sh.kernel_launches()
+    w = sh.get_fields()
+    ok = bool(np.isfinite(w).all())
+    sh.destroy()
+    if rank == 0:
+        ranges = sharded.slab_ranges(case.nz, nslabs)
+        halo_bytes = 2 * 3 * 3 * (case.nx + 32) * (case.ny + 6) * 8 * (9 + 1) + 2 * 3 * 3 * (case.nx + 32) * (case.ny + 6)
+        line = {
+            "metric": METRIC, "value": N * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "repeats": {"n": len(reps), "best_ms_per_step": min(reps) / args.steps, "median_ms_per_step": ms / args.steps},
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_TEXT[args.config], "grid": [case.nx, case.ny, case.nz], "points": N,
+                       "parallelism": (f"{nslabs} z slabs, one per GPU, halo exchange by NCCL send / receive" if world > 1 else
+                                       f"{nslabs} z slabs in one process on one GPU (exchange = device copies)"),
+                       "slab_planes": [b - a for a, b in ranges], "halo_bytes_per_slab_per_stage_approx": halo_bytes,
+                       "l2": "inputs larger than L2" if N * 400 > 4 * 126e6 else "L2-resident"},
+            "clocks": clk, "gpu_launches": launches, "state_finite": ok, "roofline": None, "cpu_baseline": None,
+            "e2e": None,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -513,6 +584,10 @@ def main():
     ap.add_argument("--order-family", type=int, default=3, choices=[1, 2, 3, 4],
                     help="m: central order 2m / WENO order 2m-1 / viscous order 2m (default 3 = 6/5/6)")
     ap.add_argument("--flux-mode", default=None, choices=["central", "weno", "hybrid"], help="override the config's flux mode")
+    ap.add_argument("--sharded", action="store_true",
+                    help="cut the grid into z slabs (one per rank under torchrun, --slabs in one process otherwise) "
+                         "and exchange halo planes every phase: strong scaling instead of independent replicas")
+    ap.add_argument("--slabs", type=int, default=2, help="--sharded on one GPU: number of slabs in this process")
     ap.add_argument("--activation", type=float, default=None,
                     help="hybrid mode: impose the node mask on this fraction of the z planes (PAPER:497-501 sweep)")
     args = ap.parse_args()
@@ -522,6 +597,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
     return run_ours(args)
 
 

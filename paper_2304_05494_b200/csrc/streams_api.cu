@@ -99,7 +99,7 @@ const char* plan(const streams_grid* g, const streams_gas* gas, const streams_sc
   {
     const size_t face = std::max(std::max((size_t)g->ny * g->nz, (size_t)g->nx * g->nz), (size_t)g->nx * g->ny);
     S.lcap = align_up(S.N + face, 64);
-    S.off_ilist = take(hyb ? 3 * S.lcap * 4 : 256);
+    S.off_ilist = take(hyb ? 4 * S.lcap * 4 : 256);     // interfaces x, y, z and the nodes next to one
   }
   S.off_dF = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 15 * S.fs * 8 : 256);
   S.off_corr = take(sc->flux_mode != STREAMS_FLUX_CENTRAL ? 5 * S.fs * 8 : 256);

@@ -121,7 +121,7 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
     // per-evaluation counters of flags_kernel (which runs after this kernel; their last readers ran before it)
     P.counters[C_NSHOCK] = 0;
     P.counters[C_NFLAGGED] = 0;
-    P.counters[C_NIFACE] = 0; P.counters[C_NIFACE + 1] = 0; P.counters[C_NIFACE + 2] = 0;
+    P.counters[C_NIFACE] = 0; P.counters[C_NIFACE + 1] = 0; P.counters[C_NIFACE + 2] = 0; P.counters[C_NIFACE + 3] = 0;
     reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[2] += 1ull;   // sensor evaluations since set_fields
   }
   if (tid == 0) {
@@ -270,8 +270,8 @@ template <int R>
 __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nwords = (long long)nwx * P.ny * P.nz;
-  int cnt[5] = {0, 0, 0, 0, 0};      // flagged nodes, shock nodes, interfaces x, y, z
-  unsigned long long hiw[3] = {0ull, 0ull, 0ull}, first[3] = {0ull, 0ull, 0ull};   // flagged interfaces named by their
+  int cnt[6] = {0, 0, 0, 0, 0, 0};   // flagged nodes, shock nodes, interfaces x, y, z, nodes next to a flagged interface
+  unsigned long long hiw[4] = {0ull, 0ull, 0ull, 0ull}, first[4] = {0ull, 0ull, 0ull, 0ull};   // flagged interfaces named by their
   int n0w = 0;                                                                    // left node: plus sides, pencil starts
   if (t < nwords) {
     const int iw = (int)(t % nwx);
@@ -322,10 +322,12 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
       hiw[d] = hi[d];
       cnt[2 + d] = __popcll(hi[d]) + __popcll(first[d]);
     }
+    hiw[3] = any;                                    // list 3: the nodes that receive a net correction (corr_gather_kernel)
+    cnt[5] = cnt[1];
   }
   // counters 0, 1: warp-shuffle sums, one atomic per block
   __shared__ int s_cnt[2];
-  __shared__ int s_wsum[3][8], s_base[3];
+  __shared__ int s_wsum[4][8], s_base[4];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0;
   // most blocks see no flagged node at all: nothing to count or to append (the barrier also publishes s_cnt)
@@ -339,9 +341,9 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   }
   // flagged interfaces: exclusive scan over the block, one atomic per direction per block reserves the
   // block's range of the direction's work list (DevP::ilist), every thread writes its own entries
-  int off[3];
+  int off[4];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
+  for (int d = 0; d < 4; ++d) {
     int v = cnt[2 + d];
 #pragma unroll
     for (int s = 1; s < 32; s <<= 1) {
@@ -352,7 +354,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
     off[d] = v - cnt[2 + d];
   }
   __syncthreads();
-  if (threadIdx.x < 3) {
+  if (threadIdx.x < 4) {
     const int d = threadIdx.x;
     int run = 0;
 #pragma unroll
@@ -360,7 +362,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
     int base = 0;
     if (run) {
       base = atomicAdd(&P.counters[C_NIFACE + d], run);
-      atomicAdd(&reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[3 + d], (unsigned long long)run);
+      if (d < 3) atomicAdd(&reinterpret_cast<unsigned long long*>(P.counters + C_TOTALS)[3 + d], (unsigned long long)run);
     }
     s_base[d] = base;
   } else if (threadIdx.x >= 32 && threadIdx.x < 34 && s_cnt[threadIdx.x - 32]) {
@@ -372,7 +374,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
   __syncthreads();
   if (t < nwords) {
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
+    for (int d = 0; d < 4; ++d) {
       if (cnt[2 + d] == 0) continue;
       int* __restrict__ Lst = P.ilist + (long long)d * P.lcap + s_base[d] + s_wsum[d][wid] + off[d];
       unsigned long long wl = first[d], wh = hiw[d];

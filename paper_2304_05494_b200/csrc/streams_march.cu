@@ -173,7 +173,7 @@ struct MarchSmem {
   static constexpr int NF = VISC ? 9 : 6;
   static constexpr size_t BUF = (size_t)NF * G::PLANE * 8;     // one centre-plane buffer
   static constexpr size_t RING = (size_t)NF * G::NT * 8;       // one ring-plane slot
-  static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[5]
+  static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[1..4] (+ one spare field)
   static constexpr size_t DFS = WENO ? (size_t)5 * G::NT * 8 : 0;
   static constexpr int NSLOT = STREAMS_MARCH_NSLOT;            // ring-plane / RK-operand slots: loads run NSLOT - 1 planes ahead
   static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + NSLOT * RING, OFF_DFS = OFF_EPI + NSLOT * EPI,
@@ -222,7 +222,9 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const int s0 = (ty + NG) * G::ROW + tx + 4;          // this node in a shared-memory plane
 
   const unsigned bytes_c = (unsigned)SM::BUF;
-  const unsigned bytes_e = (unsigned)SM::RING + (UPD ? 5u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
+  // (the density of the old state is not fetched with the other four conserved variables: the ring's centre value of
+  // the rho slot is the same number, q[Q_RHO] being a copy of w[0])
+  const unsigned bytes_e = (unsigned)SM::RING + (UPD ? 4u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
   const int cx0 = i0 + P.ox, cy0 = j0 + NG;            // tile origin in padded coordinates
 
   auto issue_centre = [&](int k, int b) {              // thread 0 only
@@ -429,7 +431,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       for (int q = 0; q < 5; ++q) {
         double inc = sa.gam * r[q];
         if (sa.read_prev) inc = fma(sa.rhk, ep[q * G::NT], inc);
-        wn[q] = fma(dt, inc, ep[(5 + q) * G::NT]);
+        wn[q] = fma(dt, inc, q == 0 ? c0[F_RHO] : ep[(4 + q) * G::NT]);
         if (active) st_out(P.w + (long long)q * P.fs + n, wn[q]);
       }
       if (!DEFER) finish_node(k, active);
@@ -535,7 +537,7 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
   const cuuint32_t halo = 2 * (cuuint32_t)P.ng;        // MarchGeom<TY, NG>::ROW / ROWS with NG = DevP::ng
   if (make(&maps->centre, P.q, nf, MTX + 8, TY + halo, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
-  if (make(&maps->w, P.w, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
+  if (make(&maps->w, P.w + P.fs, 4, MTX, TY, 4) != CUDA_SUCCESS) return -2;     // rho u, rho v, rho w, rho E
   if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
   if (make(&maps->s_centre, P.q, nf, MTX + 8, STY + halo, 3) != CUDA_SUCCESS) return -2;
   if (make(&maps->s_ring, P.q, nf, MTX, STY, 3) != CUDA_SUCCESS) return -2;

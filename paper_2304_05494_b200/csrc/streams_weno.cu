@@ -406,19 +406,21 @@ __global__ void __launch_bounds__(128) corr_gather_dense_kernel(const DevP P) {
   corr_node(P, pidx(P, i, j, k), 0x3fu, met);
 }
 
-// hybrid mode: one thread per node, x fastest (the flag bytes of a warp are one 32-byte segment), 128 nodes of a row
-// per block (measured: larger blocks and persistent row-walking blocks are 1.4-3x slower); a thread whose byte is
-// zero is done (most of the grid).  Flagged nodes come in clusters, so the warps that
-// have work are mostly full and their loads coalesced; the many resident threads hide the latency of the gather.
-// HBM: 1 B per node + the flagged nodes' values.
-__global__ void __launch_bounds__(128) corr_gather_kernel(const DevP P) {
-  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  if (i >= P.nx) return;
-  const long long n = pidx(P, i, j, k);
-  const unsigned fl = P.nflag[n];
-  if (!fl) return;
-  const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
-  corr_node(P, n, fl, met);
+// hybrid mode: flags_kernel has compacted the nodes next to a flagged interface into a fourth work list (DevP::ilist
+// [3], count in DevP::counters[C_NIFACE + 3]); persistent blocks walk it, one thread per listed node, so every lane
+// has a gather to do (a scan of the flag bytes of the whole grid by one thread per node took 1.4 ms on config 4, of
+// which most was threads finding nothing to do).  Consecutive entries are mostly consecutive nodes: coalesced.
+__global__ void __launch_bounds__(256) corr_gather_kernel(const DevP P) {
+  const int count = P.counters[C_NIFACE + 3];
+  const int* __restrict__ list = P.ilist + 3 * P.lcap;
+  const int rowlen = (int)P.sy;
+  for (int e = blockIdx.x * 256 + threadIdx.x; e < count; e += gridDim.x * 256) {
+    const int n = list[e];
+    const unsigned fl = P.nflag[n];
+    const int j = (n / rowlen) % P.py - P.ng;        // row of the node (y metric)
+    const double met[3] = {P.inv_dx, P.eta_y_c[j], P.inv_dz};
+    corr_node(P, n, fl, met);
+  }
 }
 
 // -------------------------------------------------------------------------- launch
@@ -437,8 +439,7 @@ static int launch_weno_T(const DevP& P, cudaStream_t st) {
 int launch_corr(const DevP& P, cudaStream_t st) {
   if (P.flux_mode == FLUX_CENTRAL) return 0;
   if (P.flux_mode == FLUX_HYBRID) {
-    dim3 b(128), g((unsigned)((P.nx + 127) / 128), (unsigned)P.ny, (unsigned)P.nz);
-    corr_gather_kernel<<<g, b, 0, st>>>(P);
+    corr_gather_kernel<<<P.nsm * 8, 256, 0, st>>>(P);
   } else {
     dim3 b(128), g((unsigned)((P.nx + 127) / 128), (unsigned)P.ny, (unsigned)P.nz);
     corr_gather_dense_kernel<<<g, b, 0, st>>>(P);
