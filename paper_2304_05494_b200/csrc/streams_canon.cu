@@ -59,10 +59,11 @@ __global__ void __launch_bounds__(256) scalar_ghost_kernel(const DevP P) {
 // planes ahead), the z neighbours live in a 7-plane register ring fed by a second TMA box per plane.
 // HBM: 24 B read + 8 B (div) + 1 B (mask) write per node; every stencil offset is an immediate.
 // ---------------------------------------------------------------------------------------------
+constexpr int SKU = 2;            // planes per iteration of sensor_march_kernel
 template <int TY, int NG>
 struct SensorSmem {
   using G = MarchGeom<TY, NG>;
-  static constexpr size_t BUF = (size_t)3 * G::PLANE * 8, RING = (size_t)3 * G::NT * 8;
+  static constexpr size_t BUF = (size_t)3 * SKU * G::PLANE * 8, RING = (size_t)3 * SKU * G::NT * 8;
   static constexpr size_t OFF_RING = 2 * BUF, OFF_BAR = OFF_RING + 2 * RING, TOTAL = OFF_BAR + 64;
   static_assert(BUF % 128 == 0 && RING % 128 == 0, "TMA destinations are 128-byte aligned");
 };
@@ -77,8 +78,11 @@ __device__ __forceinline__ double ddc_g(const DevP& P, const G& g, double metric
 }
 
 #ifndef STREAMS_SENSOR_MINB
-#define STREAMS_SENSOR_MINB 3
+#define STREAMS_SENSOR_MINB 2
 #endif
+// An iteration handles the SKU = 2 planes k, k + 1 of the tile: the boxes are two planes deep, the ring holds
+// 2 NG + 2 planes (k - NG .. k + NG + 1) and shifts by two, so the register moves of the shift, the barrier, the
+// mbarrier waits and the loop bookkeeping are paid once per two nodes, and the two nodes' derivative chains interleave.
 template <int L, bool MASK, bool THETA, int TY, int NG>
 __global__ void __launch_bounds__(MTX * TY, STREAMS_SENSOR_MINB)
 sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring, const DevP P,
@@ -86,9 +90,10 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
   using G = MarchGeom<TY, NG>;             // NG = DevP::ng: ghost width / ring depth of the layout
   using SM = SensorSmem<TY, NG>;
   static_assert(L <= NG, "ring depth");
+  constexpr int NR = 2 * NG + SKU;         // ring planes
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][3][PLANE]
-  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][3][NT]
+  double* const buf = reinterpret_cast<double*>(smem_raw);                  // [2][3][SKU][PLANE]
+  double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [2][3][SKU][NT]
   unsigned long long* const full_c = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
   unsigned long long* const full_r = full_c + 2;
 
@@ -109,13 +114,15 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
   const int s0 = (ty + NG) * G::ROW + tx + 4;
   const int cx0 = i0 + P.ox, cy0 = j0 + NG;
 
-  auto issue_centre = [&](int k, int b) {
+  // (planes beyond the padded box -- the second plane of an odd tail, the ring planes of the last iterations -- are
+  // filled with zeros by the TMA unit and never used)
+  auto issue_centre = [&](int k, int b) {            // planes k, k + 1
     mbar_expect_tx(&full_c[b], (unsigned)SM::BUF);
-    tma_load_4d(buf + (size_t)b * 3 * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
+    tma_load_4d(buf + (size_t)b * 3 * SKU * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
   };
-  auto issue_ring = [&](int k, int b) {              // ring plane k+NG+1 into slot b
+  auto issue_ring = [&](int k, int b) {              // ring planes k + NG + 2, k + NG + 3 into slot b
     mbar_expect_tx(&full_r[b], (unsigned)SM::RING);
-    tma_load_4d(ring + (size_t)b * 3 * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + 1 + NG, 0);
+    tma_load_4d(ring + (size_t)b * 3 * SKU * G::NT, &tm_ring, &full_r[b], cx0, cy0, k + NG + SKU + NG, 0);
   };
   if (MASK && tid == 0 && blockIdx.x == 0 && P.flux_mode == FLUX_HYBRID) {
     // per-evaluation counters of flags_kernel (which runs after this kernel; their last readers ran before it)
@@ -132,16 +139,16 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
   __syncthreads();
   if (tid == 0) {
     issue_centre(kb, 0);
-    if (kb + 1 < ke) issue_centre(kb + 1, 1);
+    if (kb + SKU < ke) issue_centre(kb + SKU, 1);
     issue_ring(kb, 0);
   }
   const double my = P.eta_y_c[min(j, P.ny - 1)];
-  double zr[3][2 * NG + 1];
+  double zr[3][NR];                                   // planes kb - NG .. kb + NG + 1 (the last one clamped into the box)
 #pragma unroll
   for (int f = 0; f < 3; ++f) {
-    const double* __restrict__ fp = P.q + (long long)f * P.fs + ncol + (long long)(kb - NG) * P.sz;
+    const double* __restrict__ fp = P.q + (long long)f * P.fs + ncol;
 #pragma unroll
-    for (int m = 0; m < 2 * NG + 1; ++m) zr[f][m] = fp[(long long)m * P.sz];
+    for (int m = 0; m < NR; ++m) zr[f][m] = fp[(long long)(min(kb + m, P.pz - 1) - NG) * P.sz];
   }
 
   // this thread's column in the outputs, advanced plane by plane
@@ -156,17 +163,20 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
                       (j < NG && P.bc_y_lo == BC_PERIODIC) || (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) ||
                       (j == 0 && P.bc_y_lo != BC_PERIODIC) || (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC));
 
-  for (int k = kb; k < ke; ++k) {
-    const int it = k - kb, b = it & 1;
+  for (int k = kb, it = 0; k < ke; k += SKU, ++it) {
+    const int b = it & 1;
     const unsigned par = (unsigned)(it >> 1) & 1u;
     mbar_wait(&full_c[b], par);
-    const double* __restrict__ sc = buf + (size_t)b * 3 * G::PLANE + s0;
-    double gx[3], gy[3], gz[3];
+    const double* __restrict__ sc = buf + (size_t)b * 3 * SKU * G::PLANE + s0;
+    double gx[SKU][3], gy[SKU][3], gz[SKU][3];
 #pragma unroll
-    for (int f = 0; f < 3; ++f) {
-      gx[f] = ddc_g<L>(P, [&](int o) { return sc[f * G::PLANE + o]; }, P.inv_dx);
-      gy[f] = ddc_g<L>(P, [&](int o) { return sc[f * G::PLANE + o * G::ROW]; }, my);
-      gz[f] = ddc_g<L>(P, [&](int o) { return zr[f][NG + o]; }, P.inv_dz);
+    for (int z = 0; z < SKU; ++z) {
+#pragma unroll
+      for (int f = 0; f < 3; ++f) {
+        gx[z][f] = ddc_g<L>(P, [&](int o) { return sc[(f * SKU + z) * G::PLANE + o]; }, P.inv_dx);
+        gy[z][f] = ddc_g<L>(P, [&](int o) { return sc[(f * SKU + z) * G::PLANE + o * G::ROW]; }, my);
+        gz[z][f] = ddc_g<L>(P, [&](int o) { return zr[f][NG + z + o]; }, P.inv_dz);
+      }
     }
     if (tid >> 5) {
       if (b) asm volatile("bar.arrive 2, %0;" ::"n"(G::NT) : "memory");
@@ -175,71 +185,75 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
       if (b) asm volatile("bar.sync 2, %0;" ::"n"(G::NT) : "memory");
       else asm volatile("bar.sync 1, %0;" ::"n"(G::NT) : "memory");
       if (tid == 0) {
-        if (k + 1 < ke) issue_ring(k + 1, b ^ 1);       // needed first
-        if (k + 2 < ke) issue_centre(k + 2, b);
+        if (k + SKU < ke) issue_ring(k + SKU, b ^ 1);     // needed first
+        if (k + 2 * SKU < ke) issue_centre(k + 2 * SKU, b);
       }
     }
-    const double dv = (gx[0] + gy[1]) + gz[2];
-    if (active) {
-      *div_p = dv;
-      unsigned char mk = 0;
-      if (MASK || THETA) {
-        const double ox = gy[2] - gz[1], oy = gz[0] - gx[2], oz = gx[1] - gy[0];
-        const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
-        // mask = theta > thr with theta = max(-dv / sqrt(s), 0).  Without the theta output the decision is taken on
-        // the squares wherever it is clear by a margin far above the rounding of either form (1e-12 relative, the
-        // quotient is good to 2 ulp); only a node within that margin of the threshold evaluates the square root and
-        // the division -- the same operations as the definition, so the mask carries the bits of the definition.
-        const double a = -dv, a2 = a * a, t2 = P.thr2 * s;
-        bool clear_hi = a > 0.0 && a2 > t2 * (1.0 + 1e-12), clear_lo = !(a > 0.0) || a2 < t2 * (1.0 - 1e-12);
-        if (P.thr < 0.0) { clear_hi = true; clear_lo = false; }       // theta >= 0 > thr at every node
-        if (a != a) { clear_hi = false; clear_lo = true; }              // NaN: theta = 0, not above a threshold >= 0
-        if (THETA || !(clear_hi || clear_lo)) {
-          double th = -dv / sqrt(s);
-          if (!(th > 0.0)) th = 0.0;
-          if (THETA) P.theta[iidx(P, i, j, k)] = th;
-          mk = (th > P.thr) ? 1 : 0;
-        } else {
-          mk = clear_hi ? 1 : 0;
-        }
-        if (MASK && ovr_p) mk = ovr_p[(long long)k * isz];   // imposed mask (activation sweeps)
-        if (MASK) *mask_p = mk;
-      }
-      // face ghosts of div / mask (S6), written by the node they copy: its periodic image, or the NG ghost nodes
-      // beyond a non-periodic face (constant extrapolation).  Which x / y ghosts a thread owns is fixed along the
-      // march (gplan), the z faces are a property of the plane.
-      if (gplan | (zface && (per_z ? (k < NG || k >= P.nz - NG) : (k == 0 || k == P.nz - 1)))) {
-        auto put = [&](long long m) { div_p[m] = dv; if (MASK) mask_p[m] = mk; };
-        auto face = [&](int a, int na, bool per, long long st) {      // a: index along the direction, st: its stride
-          if (per) {
-            if (a < NG) put(na * st);
-            else if (a >= na - NG) put(-na * st);
+#pragma unroll
+    for (int z = 0; z < SKU; ++z) {
+      const int kk = k + z;
+      const double dv = (gx[z][0] + gy[z][1]) + gz[z][2];
+      if (active && (z == 0 || kk < ke)) {
+        div_p[z * isz] = dv;
+        unsigned char mk = 0;
+        if (MASK || THETA) {
+          const double ox = gy[z][2] - gz[z][1], oy = gz[z][0] - gx[z][2], oz = gx[z][1] - gy[z][0];
+          const double s = (((dv * dv + ox * ox) + oy * oy) + oz * oz) + P.eps_s;
+          // mask = theta > thr with theta = max(-dv / sqrt(s), 0).  Without the theta output the decision is taken on
+          // the squares wherever it is clear by a margin far above the rounding of either form (1e-12 relative, the
+          // quotient is good to 2 ulp); only a node within that margin of the threshold evaluates the square root and
+          // the division -- the same operations as the definition, so the mask carries the bits of the definition.
+          const double a = -dv, a2 = a * a, t2 = P.thr2 * s;
+          bool clear_hi = a > 0.0 && a2 > t2 * (1.0 + 1e-12), clear_lo = !(a > 0.0) || a2 < t2 * (1.0 - 1e-12);
+          if (P.thr < 0.0) { clear_hi = true; clear_lo = false; }       // theta >= 0 > thr at every node
+          if (a != a) { clear_hi = false; clear_lo = true; }              // NaN: theta = 0, not above a threshold >= 0
+          if (THETA || !(clear_hi || clear_lo)) {
+            double th = -dv / sqrt(s);
+            if (!(th > 0.0)) th = 0.0;
+            if (THETA) P.theta[iidx(P, i, j, kk)] = th;
+            mk = (th > P.thr) ? 1 : 0;
           } else {
-            if (a == 0) { for (int m = 1; m <= NG; ++m) put(-m * st); }
-            if (a == na - 1) { for (int m = 1; m <= NG; ++m) put(m * st); }
+            mk = clear_hi ? 1 : 0;
           }
-        };
-        face(i, P.nx, P.bc_x == BC_PERIODIC, 1);
-        if (j < NG || j >= P.ny - NG) {
-          if (j < NG && P.bc_y_lo == BC_PERIODIC) put(P.ny * P.sy);
-          if (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) put(-P.ny * P.sy);
-          if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(-m * P.sy); }
-          if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(m * P.sy); }
+          if (MASK && ovr_p) mk = ovr_p[(long long)kk * isz];   // imposed mask (activation sweeps)
+          if (MASK) mask_p[z * isz] = mk;
         }
-        face(k, P.nz, per_z, P.sz);
+        // face ghosts of div / mask (S6), written by the node they copy: its periodic image, or the NG ghost nodes
+        // beyond a non-periodic face (constant extrapolation).  Which x / y ghosts a thread owns is fixed along the
+        // march (gplan), the z faces are a property of the plane.
+        if (gplan | (zface && (per_z ? (kk < NG || kk >= P.nz - NG) : (kk == 0 || kk == P.nz - 1)))) {
+          auto put = [&](long long m) { div_p[z * isz + m] = dv; if (MASK) mask_p[z * isz + m] = mk; };
+          auto face = [&](int a, int na, bool per, long long st) {      // a: index along the direction, st: its stride
+            if (per) {
+              if (a < NG) put(na * st);
+              else if (a >= na - NG) put(-na * st);
+            } else {
+              if (a == 0) { for (int m = 1; m <= NG; ++m) put(-m * st); }
+              if (a == na - 1) { for (int m = 1; m <= NG; ++m) put(m * st); }
+            }
+          };
+          face(i, P.nx, P.bc_x == BC_PERIODIC, 1);
+          if (j < NG || j >= P.ny - NG) {
+            if (j < NG && P.bc_y_lo == BC_PERIODIC) put(P.ny * P.sy);
+            if (j >= P.ny - NG && P.bc_y_hi == BC_PERIODIC) put(-P.ny * P.sy);
+            if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(-m * P.sy); }
+            if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(m * P.sy); }
+          }
+          face(kk, P.nz, per_z, P.sz);
+        }
       }
     }
-    div_p += isz;
-    mask_p += isz;
+    div_p += SKU * isz;
+    mask_p += SKU * isz;
     mbar_wait(&full_r[b], par);
-    const double* __restrict__ rn = ring + (size_t)b * 3 * G::NT + tid;
-    // (register moves: renaming the ring through a phase switch measured slower, here and in rhs_march_kernel;
-    // so did 4 blocks / SM at 64 registers and 32 x 16 or 32 x 4 tiles)
+    const double* __restrict__ rn = ring + (size_t)b * 3 * SKU * G::NT + tid;
+    // (register moves: renaming the ring through a phase switch measured slower, here and in rhs_march_kernel)
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
 #pragma unroll
-      for (int m = 0; m < 2 * NG; ++m) zr[f][m] = zr[f][m + 1];
-      zr[f][2 * NG] = rn[f * G::NT];
+      for (int m = 0; m < 2 * NG; ++m) zr[f][m] = zr[f][m + SKU];
+#pragma unroll
+      for (int z = 0; z < SKU; ++z) zr[f][2 * NG + z] = rn[(f * SKU + z) * G::NT];
     }
   }
 }

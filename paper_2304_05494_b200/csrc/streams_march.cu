@@ -528,9 +528,9 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
   const cuuint32_t nf = P.visc_law != VISC_NONE ? 9 : 6;
   const cuuint64_t strides[3] = {(cuuint64_t)P.px * 8, (cuuint64_t)P.sz * 8, (cuuint64_t)P.fs * 8};
   const cuuint32_t ones[4] = {1, 1, 1, 1};
-  auto make = [&](CUtensorMap* m, void* base, cuuint64_t nfields, cuuint32_t bx, cuuint32_t by, cuuint32_t bf) {
+  auto make = [&](CUtensorMap* m, void* base, cuuint64_t nfields, cuuint32_t bx, cuuint32_t by, cuuint32_t bf, cuuint32_t bz = 1) {
     const cuuint64_t dims[4] = {(cuuint64_t)P.px, (cuuint64_t)P.py, (cuuint64_t)P.pz, nfields};
-    const cuuint32_t box[4] = {bx, by, 1, bf};
+    const cuuint32_t box[4] = {bx, by, bz, bf};
     return encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_NONE, STREAMS_TMA_L2_PROMOTION, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   };
@@ -539,8 +539,8 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
   if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->w, P.w + P.fs, 4, MTX, TY, 4) != CUDA_SUCCESS) return -2;     // rho u, rho v, rho w, rho E
   if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
-  if (make(&maps->s_centre, P.q, nf, MTX + 8, STY + halo, 3) != CUDA_SUCCESS) return -2;
-  if (make(&maps->s_ring, P.q, nf, MTX, STY, 3) != CUDA_SUCCESS) return -2;
+  if (make(&maps->s_centre, P.q, nf, MTX + 8, STY + halo, 3, 2) != CUDA_SUCCESS) return -2;   // two planes per box:
+  if (make(&maps->s_ring, P.q, nf, MTX, STY, 3, 2) != CUDA_SUCCESS) return -2;                // SKU of sensor_march_kernel
   return 0;
 }
 
