@@ -20,8 +20,9 @@ struct StageArgs {
 };
 
 // TMA descriptors of the z-marching kernels (built once per context and primitive buffer by make_march_maps):
-// centre planes with halo and ring planes of the primitives, RK operands w and R; s_*: (u, v, w) boxes of the sensor.
-struct MarchMaps { CUtensorMap centre, ring, w, r, s_centre, s_ring; };
+// centre planes with halo and ring planes of the primitives, RK operands w and R, the interface-flag bytes of a tile
+// plane (hybrid mode); s_*: (u, v, w) boxes of the sensor.
+struct MarchMaps { CUtensorMap centre, ring, w, r, flag, s_centre, s_ring; };
 // Returns 0, or a negative code: -1 driver entry point missing, -2 encode failed.
 int make_march_maps(const DevP& P, MarchMaps* maps);
 

@@ -176,8 +176,10 @@ struct MarchSmem {
   static constexpr size_t EPI = (size_t)10 * G::NT * 8;        // one RK-operand slot: R[5], w[1..4] (+ one spare field)
   static constexpr size_t DFS = WENO ? (size_t)5 * G::NT * 8 : 0;
   static constexpr int NSLOT = STREAMS_MARCH_NSLOT;            // ring-plane / RK-operand slots: loads run NSLOT - 1 planes ahead
+  static constexpr size_t FLG = WENO ? 2 * (((size_t)G::NT + 127) / 128 * 128) : 0;   // interface-flag bytes of the centre planes
   static constexpr size_t OFF_RING = 2 * BUF, OFF_EPI = OFF_RING + NSLOT * RING, OFF_DFS = OFF_EPI + NSLOT * EPI,
-                          OFF_BAR = OFF_DFS + DFS, TOTAL = OFF_BAR + 64 + 8 * 32;   // 2 + NSLOT mbarriers, rate scratch
+                          OFF_FLG = OFF_DFS + DFS, OFF_BAR = OFF_FLG + FLG,
+                          TOTAL = OFF_BAR + 64 + 8 * 32;                               // 2 + NSLOT mbarriers, rate scratch
   static_assert(BUF % 128 == 0 && RING % 128 == 0 && EPI % 128 == 0, "TMA destinations are 128-byte aligned");
   static_assert(TOTAL <= 227 * 1024, "shared memory of one block");
 };
@@ -189,7 +191,7 @@ template <int L, int LV, bool VISC, bool CONV, bool WENO, bool UPD, int TY, int 
 __global__ void __launch_bounds__(MTX * TY, STREAMS_MARCH_MINB)
 rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
                  const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r,
-                 const DevP P,
+                 const __grid_constant__ CUtensorMap tm_flag, const DevP P,
                  const StageArgs sa, int nbx, int nby, int kz) {
   using G = MarchGeom<TY, NG>;
   using SM = MarchSmem<TY, NG, VISC, WENO>;
@@ -201,6 +203,9 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   double* const ring = reinterpret_cast<double*>(smem_raw + SM::OFF_RING);  // [NSLOT][NF][NT]
   double* const epi = reinterpret_cast<double*>(smem_raw + SM::OFF_EPI);    // [NSLOT][10][NT]
   double* const dfs = reinterpret_cast<double*>(smem_raw + SM::OFF_DFS);    // [5][NT]
+  unsigned char* const flg = smem_raw + SM::OFF_FLG;                        // [2][NT] (hybrid)
+  constexpr bool FLAGS = WENO && CONV;                                      // hybrid: per-node interface flags decide
+  constexpr int FLGB = (int)(SM::FLG / 2);
   unsigned long long* const bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::OFF_BAR);
   unsigned long long* const full_c = bars;        // [2] centre plane landed
   unsigned long long* const full_e = bars + 2;    // [NSLOT] ring plane + RK operands landed
@@ -221,7 +226,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const int ncol = (int)pidx(P, ic, jc, 0);            // this thread's column at k = 0 (padded index < 2^31)
   const int s0 = (ty + NG) * G::ROW + tx + 4;          // this node in a shared-memory plane
 
-  const unsigned bytes_c = (unsigned)SM::BUF;
+  const unsigned bytes_c = (unsigned)SM::BUF + (FLAGS ? (unsigned)G::NT : 0u);
   // (the density of the old state is not fetched with the other four conserved variables: the ring's centre value of
   // the rho slot is the same number, q[Q_RHO] being a copy of w[0])
   const unsigned bytes_e = (unsigned)SM::RING + (UPD ? 4u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
@@ -230,6 +235,9 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   auto issue_centre = [&](int k, int b) {              // thread 0 only
     mbar_expect_tx(&full_c[b], bytes_c);
     tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
+    // the flag bytes of the plane's nodes ride with it (a byte loaded by its thread one plane ahead stalled every plane:
+    // the compiler tests the byte where it is requested and carries the predicate; 11 % of the kernel's samples)
+    if (FLAGS) tma_load_4d(flg + b * FLGB, &tm_flag, &full_c[b], cx0, cy0, k + NG, 0);
   };
   auto issue_ring_epi = [&](int k, int b) {            // ring plane k+NG+1 and the RK operands of plane k into slot b
     mbar_expect_tx(&full_e[b], bytes_e);
@@ -300,8 +308,6 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const int yoff = !P.own_y ? 0 : (j < NG ? P.ny * (int)P.sy : (j >= P.ny - NG ? -P.ny * (int)P.sy : 0));
   double rate = 0.0;                                  // a9 of the next step (last stage only)
   bool bad = false;                                   // a NaN rate, or a non-finite updated state
-  unsigned fl_next = 0;
-  if (WENO && CONV && active) fl_next = ld_u8_now(P.nflag + ncol + (long long)kb * P.sz);
 
   // a2 / a1 / a9 of the next stage for the node just updated (state wn of plane kk): its primitives go to the other q
   // buffer (stencils of this stage still read the current one), also at the node's periodic images in the ghost layers
@@ -340,26 +346,19 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     const unsigned par_e = (unsigned)(it / NSLOT) & 1u;
     const int n = ncol + k * isz;
     if (tid == G::NT - 32) prefetch_ring_epi(k + NSLOT - 1 + PF);   // no shared-memory hazard: any thread, off the issuing warp's path
-    // does this node have a net WENO correction (an adjacent flagged interface)?  Flags of this plane were
-    // prefetched, the next plane's are requested now; the five values are staged while the stencils run
+    // (C) the right-hand side of this node
+    mbar_wait(&full_c[b], par);
+    // does this node have a net WENO correction (an adjacent flagged interface)?  The five values are staged while
+    // the stencils run
     bool fl = false, any_fl = false;
     if (WENO) {
-      unsigned fl_new = 0;
-      if (CONV && active && k + 1 < ke) fl_new = ld_u8_now(P.nflag + n + isz);
-      // the byte loaded one plane ago is consumed only here: without this fence the compiler tests the byte it has
-      // just requested (and carries the predicate), which stalls every plane on the load
-      asm volatile("" : "+r"(fl_next));
-      fl = CONV ? (fl_next != 0) : active;
-      fl_next = fl_new;
+      fl = active && (!FLAGS || flg[b * FLGB + tid] != 0);
       any_fl = __any_sync(0xffffffffu, fl);
       if (any_fl) {
 #pragma unroll
         for (int q = 0; q < 5; ++q) cp_async8_zfill(dfs + q * G::NT + tid, P.corr + (long long)q * P.fs + n, fl);
       }
     }
-
-    // (C) the right-hand side of this node
-    mbar_wait(&full_c[b], par);
     if (DEFER && UPD) finish_node(k - 1, active && it > 0);
     const double* __restrict__ sc = buf + (size_t)b * NF * G::PLANE + s0;
     auto gx = [&](int f, int o2) { return sc[f * G::PLANE + o2]; };
@@ -479,7 +478,7 @@ static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa,
   const int tiles = nbx * nby;
   const int chunks = pick_chunks(tiles, P.nz, P.nsm * STREAMS_MARCH_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
-  kern<<<(unsigned)(tiles * chunks), G::NT, SM::TOTAL, st>>>(mp.centre, mp.ring, mp.w, mp.r, P, sa, nbx, nby, kz);
+  kern<<<(unsigned)(tiles * chunks), G::NT, SM::TOTAL, st>>>(mp.centre, mp.ring, mp.w, mp.r, mp.flag, P, sa, nbx, nby, kz);
   return 1;
 }
 
@@ -539,6 +538,15 @@ int make_march_maps(const DevP& P, MarchMaps* maps) {
   if (make(&maps->ring, P.q, nf, MTX, TY, nf) != CUDA_SUCCESS) return -2;
   if (make(&maps->w, P.w + P.fs, 4, MTX, TY, 4) != CUDA_SUCCESS) return -2;     // rho u, rho v, rho w, rho E
   if (make(&maps->r, P.R, 5, MTX, TY, 5) != CUDA_SUCCESS) return -2;
+  maps->flag = maps->r;                                // (never read outside hybrid mode)
+  if (P.flux_mode == FLUX_HYBRID) {                    // the interface-flag bytes, one per node of the padded box
+    const cuuint64_t dims[4] = {(cuuint64_t)P.px, (cuuint64_t)P.py, (cuuint64_t)P.pz, 1};
+    const cuuint64_t bstr[3] = {(cuuint64_t)P.px, (cuuint64_t)P.sz, (cuuint64_t)P.fs};
+    const cuuint32_t box[4] = {MTX, TY, 1, 1};
+    if (encode(&maps->flag, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, P.nflag, dims, bstr, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return -2;
+  }
   if (make(&maps->s_centre, P.q, nf, MTX + 8, STY + halo, 3, 2) != CUDA_SUCCESS) return -2;   // two planes per box:
   if (make(&maps->s_ring, P.q, nf, MTX, STY, 3, 2) != CUDA_SUCCESS) return -2;                // SKU of sensor_march_kernel
   return 0;
