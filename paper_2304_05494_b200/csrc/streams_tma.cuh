@@ -22,6 +22,10 @@ __device__ __forceinline__ void cp_async8_zfill(void* smem_dst, const void* gsrc
   const unsigned n = take ? 8u : 0u;
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(n) : "memory");
 }
+// 8 bytes, global -> shared
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // 16 bytes (L2 only) when `take`, zeros otherwise; both addresses 16-byte aligned
 __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool take) {
