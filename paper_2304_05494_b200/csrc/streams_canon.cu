@@ -280,8 +280,11 @@ __device__ __forceinline__ unsigned long long xshift(unsigned long long prev, un
   return (cur << (-8 * m)) | (prev >> (64 + 8 * m));
 }
 
+#ifndef STREAMS_FLAGS_MINB
+#define STREAMS_FLAGS_MINB 8
+#endif
 template <int R>
-__global__ void __launch_bounds__(256) flags_kernel(const DevP P, int nwx) {
+__global__ void __launch_bounds__(256, STREAMS_FLAGS_MINB) flags_kernel(const DevP P, int nwx) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nwords = (long long)nwx * P.ny * P.nz;
   int cnt[6] = {0, 0, 0, 0, 0, 0};   // flagged nodes, shock nodes, interfaces x, y, z, nodes next to a flagged interface

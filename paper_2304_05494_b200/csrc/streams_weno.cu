@@ -391,17 +391,24 @@ __global__ void __launch_bounds__(WTH, WenoOcc<R>::MINB) weno_list_kernel(const 
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void corr_node(const DevP& P, long long n, unsigned fl, const double met[3]) {
   const long long st[3] = {1, P.sy, P.sz};
-  double c[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  // all (up to 30) gathers first, then the sums: the loads of a node are independent and scattered, their latency is
+  // the kernel's time
+  double fp[3][5], fm[3][5];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
     const bool hp = (fl >> (2 * d + 1)) & 1u, hm = (fl >> (2 * d)) & 1u;
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      const double fp = hp ? f[q * P.fs] : 0.0;
-      const double fm = hm ? f[q * P.fs - st[d]] : 0.0;
-      c[q] = fma(met[d], fp - fm, c[q]);
+      fp[d][q] = hp ? __ldg(f + q * P.fs) : 0.0;
+      fm[d][q] = hm ? __ldg(f + q * P.fs - st[d]) : 0.0;
     }
+  }
+  double c[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) c[q] = fma(met[d], fp[d][q] - fm[d][q], c[q]);
   }
 #pragma unroll
   for (int q = 0; q < 5; ++q) P.corr[q * P.fs + n] = c[q];
