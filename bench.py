@@ -168,6 +168,11 @@ def work_model(case, act):
     I["fill_prim"] = (Np - N) * FP64_INST["fill_prim"]
     B["sensor"] = N * (24 + 8 + (1 if hyb else 0))             # read u v w, write div [mask]
     I["sensor"] = N * FP64_INST["sensor"]
+    # shared-memory wavefronts of the sensor (the pipe that binds it): per node 2 L neighbours in x and in
+    # y of three fields + three ring planes, 8-byte words: two 128-byte wavefronts per warp-wide load
+    four = max(case.central_order // 2, (case.weno_order + 1) // 2 if weno else 0, case.visc_order // 2 if visc else 0) > 3
+    Ls = 4 if four else case.central_order // 2
+    SW = {"sensor": N * (3 * 4 * Ls + 3) * 2.0 / 32.0}
     B["flags"] = N * (1 + 1) + (n_if + n_sh) * 4               # read mask, write flags byte, append to the four work lists
     I["flags"] = 0
     # fused RHS + update: read 6 convective primitives [+ T mu div], read w, write w,
@@ -190,7 +195,7 @@ def work_model(case, act):
     I["dt"] = 0                                                # the one-thread finalize (dt = CFL / rate)
     B["misc"] = 0
     I["misc"] = 0
-    return B, I, per_point
+    return B, I, per_point, SW
 
 
 # ------------------------------------------------------------------------------------------------
@@ -410,7 +415,8 @@ def run_ours(args):
     fp64_meas = {"dfma_ginst_s": binding.measure_fp64(0, 5, gpu.stream), "dadd_dmul_ginst_s": binding.measure_fp64(1, 5, gpu.stream),
                  "nominal_ginst_s": nominal_inst / 1e9}
     peak_inst = fp64_meas["dfma_ginst_s"] * 1e9
-    B, I, per_point = work_model(case, act)
+    B, I, per_point, SW = work_model(case, act)
+    peak_wave = N_SM * sm_mhz * 1e6                              # shared-memory wavefronts / s: one per SM and clock
     if args.order_family != 3:                  # the instruction counts were taken on the 6/5/6 instances
         I = {k: 0 for k in I}
     kernels = {}
@@ -424,6 +430,12 @@ def run_ours(args):
         kernels[name] = {"launches": cnt, "avg_ms": t * 1e3, "share": kms / ms_prof, "alg_bytes": B[name], "gbs": gbs,
                          "frac_hbm": gbs / peak, "fp64_ginst_s": ginst, "frac_fp64": ginst * 1e9 / peak_inst,
                          "bound": "alu" if t_alu > t_hbm else "hbm", "frac": max(t_hbm, t_alu) / t if t > 0 else 0.0}
+        if name in SW and t > 0:                # a kernel bound by the shared-memory data pipe (model count; ncu: profiles/)
+            t_sm = SW[name] / peak_wave
+            kernels[name].update({"smem_wavefronts": SW[name], "frac_smem": t_sm / t,
+                                  "smem_peak": "148 SMs x 1 wavefront (128 B) / clk x %.0f MHz" % sm_mhz})
+            if t_sm > max(t_hbm, t_alu):
+                kernels[name].update({"bound": "smem", "frac": t_sm / t})
     dom = max(kernels, key=lambda k: kernels[k]["avg_ms"] * kernels[k]["launches"])
     kd = kernels[dom]
     if kd["bound"] == "hbm":
