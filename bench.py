@@ -48,7 +48,7 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def make_case(index: int, seed_offset: int = 0):
+def make_case(index: int, seed_offset: int = 0, cube: int = 256):
     """BASELINE.json configs[index] with the rank's seed (replicas differ only by seed: base + 100 * rank,
     paper_2304_05494_b200.replicas.replica_seed)."""
     if index == 0:
@@ -66,6 +66,9 @@ def make_case(index: int, seed_offset: int = 0):
     if index == 5:   # SURVEY 8(d) "opt": the paper's own grid shape, not divisible by any tile
         return W.isotropic_turbulence(nx=420, ny=250, nz=320, mach_t=0.6, k0=4.0, kmax=32, seed=5 + 100 * seed_offset,
                                       nsteps=20, name="opt_iso_420x250x320")
+    if index == 6:   # size sweep (Fig. 5: throughput against the number of grid points): --cube N
+        return W.isotropic_turbulence(n=cube, mach_t=0.6, k0=4.0, kmax=min(32, cube // 4), seed=6 + 100 * seed_offset,
+                                      nsteps=20, name=f"sweep_iso_{cube}")
     raise SystemExit(f"unknown config {index}")
 
 
@@ -77,6 +80,7 @@ WORKLOAD_TEXT = {
     3: "configs[3]: supersonic flat-plate boundary-layer box 1024x256x256, stretched y, hybrid, seeded shocklets",
     4: "configs[4]: capacity run 640^3 periodic compressible turbulence Mach_t 0.8, k0=8, hybrid",
     5: "sweep grid 420x250x320 (the paper's grid shape, PAPER:355), periodic turbulence as configs[1]",
+    6: "size sweep: N^3 periodic turbulence as configs[1] (--cube N)",
 }
 
 
@@ -297,7 +301,7 @@ def run_ours(args):
     if dist is not None:
         dist.barrier()
 
-    case = make_case(args.config, seed_offset=rank)
+    case = make_case(args.config, seed_offset=rank, cube=args.cube)
     # sweep knobs (not used by the default run): order family, flux mode, imposed activation
     m = args.order_family
     case = case.replace(central_order=2 * m, weno_order=2 * m - 1, visc_order=2 * m)
@@ -588,6 +592,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4,
                     help="index into BASELINE.json configs (default 4: the largest single-GPU configuration)")
+    ap.add_argument("--cube", type=int, default=256, help="--config 6 (size sweep): N of the N^3 periodic box")
     ap.add_argument("--repeats", type=int, default=5, help="timed regions from the same state; value = median")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
