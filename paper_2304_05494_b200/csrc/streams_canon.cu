@@ -285,15 +285,14 @@ __device__ __forceinline__ unsigned long long xshift(unsigned long long prev, un
 #endif
 template <int R>
 __global__ void __launch_bounds__(256, STREAMS_FLAGS_MINB) flags_kernel(const DevP P, int nwx) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long nwords = (long long)nwx * P.ny * P.nz;
+  // one block row per plane (blockIdx.y = k): a thread finds its word of the plane with one 32-bit division
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned nwords = (unsigned)nwx * (unsigned)P.ny;             // words of a plane
   int cnt[6] = {0, 0, 0, 0, 0, 0};   // flagged nodes, shock nodes, interfaces x, y, z, nodes next to a flagged interface
   unsigned long long hiw[4] = {0ull, 0ull, 0ull, 0ull}, first[4] = {0ull, 0ull, 0ull, 0ull};   // flagged interfaces named by their
   int n0w = 0;                                                                    // left node: plus sides, pencil starts
   if (t < nwords) {
-    const int iw = (int)(t % nwx);
-    const long long t2 = t / nwx;
-    const int j = (int)(t2 % P.ny), k = (int)(t2 / P.ny);
+    const int j = (int)(t / (unsigned)nwx), iw = (int)(t - (unsigned)j * (unsigned)nwx), k = (int)blockIdx.y;
     const int i0 = iw * 8;
     const long long n0 = pidx(P, i0, j, k);
     const unsigned char* m = P.mask + n0;
@@ -601,8 +600,8 @@ int launch_sensor(const DevP& P, const MarchMaps& mp, int L, bool mask, bool the
 
 int launch_flags(const DevP& P, int r, cudaStream_t st) {
   const int nwx = (P.nx + 7) / 8;
-  const long long nwords = (long long)nwx * P.ny * P.nz;
-  dim3 b(256), g((unsigned)((nwords + 255) / 256));       // (sensor_march_kernel has reset the per-evaluation counters)
+  const long long nwords = (long long)nwx * P.ny;        // per plane
+  dim3 b(256), g((unsigned)((nwords + 255) / 256), (unsigned)P.nz);   // (sensor_march_kernel has reset the per-evaluation counters)
   switch (r) {
     case 1: flags_kernel<1><<<g, b, 0, st>>>(P, nwx); break;
     case 2: flags_kernel<2><<<g, b, 0, st>>>(P, nwx); break;
