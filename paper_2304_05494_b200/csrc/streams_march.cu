@@ -356,7 +356,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       any_fl = __any_sync(0xffffffffu, fl);
       if (any_fl) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) cp_async8_zfill(dfs + q * G::NT + tid, P.corr + (long long)q * P.fs + n, fl);
+        for (int q = 0; q < 5; ++q) cp_async8_zfill(dfs + q * G::NT + tid, P.corr + (long long)n * 5 + q, fl);   // the node's record
       }
     }
     if (DEFER && UPD) finish_node(k - 1, active && it > 0);

@@ -311,9 +311,9 @@ __device__ __forceinline__ void weno_dense_item(const DevP& P, long long t, doub
   double fw[5], lam[3];
   weno_stencil<D, M, R>(P, n, s, s_st + threadIdx.x, lam);
   weno_flux<D, M, R, Z>(P, lam, fw, s_st + threadIdx.x);
-  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
+  double* __restrict__ out = P.dF + ((long long)D * P.fs + n) * 5;      // record of the interface: five consecutive values
 #pragma unroll
-  for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q];
+  for (int q = 0; q < 5; ++q) out[q] = fw[q];
 }
 
 template <int M, int R, bool Z>
@@ -340,9 +340,9 @@ __device__ __forceinline__ void weno_list_item(const DevP& P, long long n, doubl
   weno_stencil<D, M, R>(P, n, s, s_st + threadIdx.x, lam);
   central_flux_st<D, M>(P, fc, s_st + threadIdx.x);        // first: its registers are free before the WENO rows are live
   weno_flux<D, M, R, Z>(P, lam, fw, s_st + threadIdx.x);
-  double* __restrict__ out = P.dF + (long long)(D * 5) * P.fs + n;
+  double* __restrict__ out = P.dF + ((long long)D * P.fs + n) * 5;      // record of the interface: five consecutive values
 #pragma unroll
-  for (int q = 0; q < 5; ++q) out[q * P.fs] = fw[q] - fc[q];
+  for (int q = 0; q < 5; ++q) out[q] = fw[q] - fc[q];
 }
 
 template <int M, int R, bool Z>
@@ -396,12 +396,12 @@ __device__ __forceinline__ void corr_node(const DevP& P, long long n, unsigned f
   double fp[3][5], fm[3][5];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    const double* __restrict__ f = P.dF + (long long)(d * 5) * P.fs + n;
+    const double* __restrict__ f = P.dF + ((long long)d * P.fs + n) * 5;
     const bool hp = (fl >> (2 * d + 1)) & 1u, hm = (fl >> (2 * d)) & 1u;
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
-      fp[d][q] = hp ? __ldg(f + q * P.fs) : 0.0;
-      fm[d][q] = hm ? __ldg(f + q * P.fs - st[d]) : 0.0;
+      fp[d][q] = hp ? __ldg(f + q) : 0.0;
+      fm[d][q] = hm ? __ldg(f + q - 5 * st[d]) : 0.0;
     }
   }
   double c[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -411,7 +411,7 @@ __device__ __forceinline__ void corr_node(const DevP& P, long long n, unsigned f
     for (int q = 0; q < 5; ++q) c[q] = fma(met[d], fp[d][q] - fm[d][q], c[q]);
   }
 #pragma unroll
-  for (int q = 0; q < 5; ++q) P.corr[q * P.fs + n] = c[q];
+  for (int q = 0; q < 5; ++q) P.corr[n * 5 + q] = c[q];                  // record of the node: five consecutive values
 }
 
 // full-WENO mode: every node, one thread each
