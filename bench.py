@@ -546,9 +546,11 @@ def run_sharded(args):
     rep = replicas.Replicas(dist, sh.device)
     N = case.npoints
     sh.step(args.warmup)
+    snap = sh.snapshot()                            # every region starts from the same state (the activation grows with time)
     clocks = ClockSampler(local) if rank == 0 else None
     reps = []
     for _ in range(max(1, args.repeats)):
+        sh.restore(snap)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         rep.barrier(); torch.cuda.synchronize(sh.device)
         e0.record(sh.stream)

@@ -144,6 +144,19 @@ class ShardedStreams:
         """The conserved state of the local slabs stacked along z: [5, sum of local nz, ny, nx]."""
         return np.concatenate([self.slabs[r].get_fields() for r in sorted(self.slabs)], axis=1)
 
+    def snapshot(self):
+        """The conserved state of every local slab as device tensors (for restore)."""
+        out = {}
+        for r, g in self.slabs.items():
+            t = self.torch.empty((5,) + tuple(g.shape), dtype=self.torch.float64, device=self.device)
+            out[r] = g.get_fields(t)
+        return out
+
+    def restore(self, snap):
+        """Back to a snapshot: the next step starts from it like from streams_set_fields."""
+        for r, g in self.slabs.items():
+            g.set_fields(snap[r])
+
     def kernel_launches(self):
         return sum(g.kernel_launches() for g in self.slabs.values())
 

@@ -69,3 +69,19 @@ def test_other_flux_modes_and_four_ghost_layers(mods, mode):
     dt0, t0, w0 = _single(binding, case, 4)
     dt1, t1, w1, _ = _sharded(sharded, case, 2, 4)
     assert dt1 == dt0 and t1 == t0 and np.array_equal(w1, w0)
+
+
+def test_snapshot_restore_repeats_the_same_steps(mods):
+    """bench.py --sharded times every region from one state: restore must bring all slabs back to it."""
+    _, sharded = mods
+    case = W.isotropic_turbulence(nx=40, ny=36, nz=41, mach_t=0.6, k0=3.0, kmax=8, seed=93, dilatational=0.5)
+    s = sharded.ShardedStreams(case, 2, [0, 1])
+    s.step(2)
+    snap = s.snapshot()
+    dt1, t1 = s.step(3)
+    w1 = s.get_fields()
+    s.restore(snap)
+    dt2, _ = s.step(3)
+    w2 = s.get_fields()
+    s.destroy()
+    assert dt1 == dt2 and np.array_equal(w1, w2)
