@@ -145,7 +145,7 @@ class ClockSampler:
 # (profiles/r1c_fp64_counts.md; static SASS counts overstate kernels with branches: the IEEE-divide slow paths and
 # the wall branch of fill_prim are rarely taken)
 FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 5, "corr_gather": 30,
-             "weno_hybrid": 987, "weno_dense": 897, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 97,
+             "weno_hybrid": 868, "weno_dense": 778, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 97,
              "prims": 60}      # prims: cons -> prim of the updated node in the fused RHS epilogue (shared reciprocal, no IEEE divide)
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
 

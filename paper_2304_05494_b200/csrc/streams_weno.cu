@@ -43,20 +43,26 @@ __device__ __forceinline__ double weno_rec2(const double* v, double eps) {
 template <> __device__ __forceinline__ double weno_rec<2, false>(const double* v, double eps) { return weno_rec2<false>(v, eps); }
 template <> __device__ __forceinline__ double weno_rec<2, true>(const double* v, double eps) { return weno_rec2<true>(v, eps); }
 
+// Fifth order, written on the undivided differences d_m = v[m+1] - v[m], which the candidate values and the smoothness
+// indicators share (the same real-number function as the textbook form, 49 instead of 59 operations):
+//   q0 = v2 + (5 d1 - 2 d0)/6, q1 = v2 + (d1 + 2 d2)/6, q2 = v2 + (4 d2 - d3)/6,
+//   beta0 = 13/12 (d1 - d0)^2 + 1/4 (3 d1 - d0)^2, beta1 = 13/12 (d2 - d1)^2 + 1/4 (d1 + d2)^2,
+//   beta2 = 13/12 (d3 - d2)^2 + 1/4 (d3 - 3 d2)^2;  result = v2 + sum_k a_k (q_k - v2) / sum_k a_k.
 template <bool Z>
 __device__ __forceinline__ double weno_rec3(const double* v, double eps) {
-  const double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) * (1.0 / 6.0);
-  const double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) * (1.0 / 6.0);
-  const double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) * (1.0 / 6.0);
-  const double s0 = eps + ((13.0 / 12.0) * sq(v[0] - 2.0 * v[1] + v[2]) + 0.25 * sq(v[0] - 4.0 * v[1] + 3.0 * v[2]));
-  const double s1 = eps + ((13.0 / 12.0) * sq(v[1] - 2.0 * v[2] + v[3]) + 0.25 * sq(v[1] - v[3]));
-  const double s2 = eps + ((13.0 / 12.0) * sq(v[2] - 2.0 * v[3] + v[4]) + 0.25 * sq(3.0 * v[2] - 4.0 * v[3] + v[4]));
+  const double d0 = v[1] - v[0], d1 = v[2] - v[1], d2 = v[3] - v[2], d3 = v[4] - v[3];
+  const double e0 = fma(5.0 / 6.0, d1, (-2.0 / 6.0) * d0);
+  const double e1 = fma(2.0 / 6.0, d2, (1.0 / 6.0) * d1);
+  const double e2 = fma(4.0 / 6.0, d2, (-1.0 / 6.0) * d3);
+  const double s0 = fma(13.0 / 12.0, sq(d1 - d0), fma(0.25, sq(fma(3.0, d1, -d0)), eps));
+  const double s1 = fma(13.0 / 12.0, sq(d2 - d1), fma(0.25, sq(d1 + d2), eps));
+  const double s2 = fma(13.0 / 12.0, sq(d3 - d2), fma(0.25, sq(fma(-3.0, d2, d3)), eps));
   double a0 = 0.1 * sq(s1 * s2), a1 = 0.6 * sq(s0 * s2), a2 = 0.3 * sq(s0 * s1);
   if (Z) {
     const double t2 = sq(s0 - s2);                    // tau^2, tau = |beta_0 - beta_2|
     a0 *= sq(s0) + t2; a1 *= sq(s1) + t2; a2 *= sq(s2) + t2;
   }
-  return (a0 * q0 + a1 * q1 + a2 * q2) * rcp_pos((a0 + a1) + a2);
+  return fma(fma(a0, e0, fma(a1, e1, a2 * e2)), rcp_pos((a0 + a1) + a2), v[2]);
 }
 template <> __device__ __forceinline__ double weno_rec<3, false>(const double* v, double eps) { return weno_rec3<false>(v, eps); }
 template <> __device__ __forceinline__ double weno_rec<3, true>(const double* v, double eps) { return weno_rec3<true>(v, eps); }
