@@ -201,6 +201,45 @@ int streams_step_forced(streams_ctx* ctx, int nsteps, int direction, double targ
 enum { STREAMS_SUM_STATE = 0, STREAMS_SUM_RESIDUAL = 1 };
 int streams_get_sums(streams_ctx* ctx, int kind, double* out5);
 
+/* The same sum reductions (PAPER:218-236 compute_residual; Table 2 "forcing term evaluations (sum reduction)") for a
+ * caller that cannot provide device scratch memory -- no context, no workspace, and the call allocates nothing.
+ * Who needs it: everything else in this header runs inside a context whose workspace the caller allocated, and the
+ * per-block partial sums of streams_get_sums live there.  That does not suit a program that took all the device memory
+ * it may use into its own arena at start-up, a hook that another solver calls in the middle of its time step with
+ * borrowed device pointers (cudaMalloc / cudaFree there would synchronise the device and undo the overlap the host
+ * application arranged, and a failed allocation would stop the run for the sake of a diagnostic), or a tool that only
+ * wants the integrals of a field it already holds.  Here the partial sums go to an array that is part of the library's
+ * own device image instead: STREAMS_SUMS_STATIC_MAX_FIELDS x 592 doubles = 75 776 bytes, held on every GPU on which the
+ * library's device code is loaded until the process exits.  No cudaMalloc, cudaFree or allocating library routine is
+ * called, now or later.
+ *   f_dev          DEVICE, nfields arrays [nz][ny][nx] one after the other (C order, no ghost layers): e.g. the w that
+ *                  streams_get_fields(.., dst_is_device = 1) wrote, or the rhs_out_dev of streams_rhs.  Read only.
+ *   nfields        1 .. STREAMS_SUMS_STATIC_MAX_FIELDS.  The limit is what the static array holds; more fields in one
+ *                  call fail with STREAMS_ENOMEM (split the call).  nx, ny, nz are not limited by the scratch.
+ *   row_weight_dev DEVICE, ny doubles, or NULL (= 1): the weight of a node of row j for STREAMS_SUM_STATE, i.e. the cell
+ *                  volume dx dz / (d eta/dy)(j) if the sums are to be volume integrals.  Ignored by STREAMS_SUM_RESIDUAL.
+ *   kind           STREAMS_SUM_STATE: out[q] = sum of f_q * row_weight(j);  STREAMS_SUM_RESIDUAL: out[q] = sum of f_q^2.
+ *   out_dev        DEVICE, nfields doubles, written by the last kernel of the call (the call itself does not
+ *                  synchronise: read it in stream order).  Owned by the caller like every other argument.
+ *   cuda_stream    a cudaStream_t (NULL = default stream) of the CURRENT device; f_dev, row_weight_dev and out_dev must
+ *                  be memory of that device.
+ *   err, err_len   HOST buffer for the error text, nullable: set to "" on success, to a message on failure (this call
+ *                  has no context to keep it in; streams_last_error does not report it).
+ * The summation order is that of streams_get_sums, so for the same numbers and weights the results are bit-identical
+ * to it and from call to call.  Returns STREAMS_OK once the two kernels are enqueued, STREAMS_EINVAL (null pointer, bad
+ * kind, non-positive extent or nfields), STREAMS_ENOMEM (nfields above the maximum), STREAMS_ECUDA.
+ * Set-up: the first call on each device looks up the device address of the static array (cudaGetSymbolAddress, with
+ * that device current; this may load the library's device code there) and keeps it; make that first call outside any
+ * stream capture.  Later calls on that device only launch the two kernels.
+ * Sharing: there is ONE such array per device and process, every call uses it and finds the previous call's partials
+ * in it.  No call relies on them: each slot is written before it is read within the call, so nothing needs clearing.
+ * Calls issued to the same stream are ordered and safe.  Two calls whose kernels may run on the GPU at the same time
+ * (different streams without an event between them, different host threads) race on the array and return garbage:
+ * order them with an event, or serialise them on one stream. */
+#define STREAMS_SUMS_STATIC_MAX_FIELDS 16
+int streams_sums_static(const double* f_dev, int nfields, int nx, int ny, int nz, const double* row_weight_dev,
+                        int kind, double* out_dev, void* cuda_stream, char* err, size_t err_len);
+
 /* Number of kernels the library has launched on this context since streams_init (kernels replayed from a CUDA graph
  * count one by one), and the number of graph submissions among them: streams_step captures the launches of one RK3
  * step once per variant of its launch sequence and replays them afterwards (small grids cannot hide the

@@ -20,9 +20,10 @@ EXPORTS = ("streams_workspace_bytes", "streams_init", "streams_set_fields", "str
            "streams_shard_finish", "streams_halo_slabs", "streams_get_fields", "streams_get_sensor", "streams_set_mask_override", "streams_get_sums", "streams_set_body_force", "streams_get_activation", "streams_get_activation_totals",
            "streams_kernel_launches", "streams_graph_launches",
            "streams_profile", "streams_get_profile", "streams_kernel_name", "streams_measure_fp64",
-           "streams_measure_fp64_scratch_bytes",
+           "streams_measure_fp64_scratch_bytes", "streams_sums_static",
            "streams_last_error", "streams_destroy")
 STREAMS_K_COUNT = 8
+SUMS_STATIC_MAX_FIELDS = 16          # STREAMS_SUMS_STATIC_MAX_FIELDS
 
 _dp = C.POINTER(C.c_double)
 
@@ -93,6 +94,8 @@ def load_library(path: str = None):
     lib.streams_measure_fp64_scratch_bytes.restype = C.c_size_t
     lib.streams_measure_fp64_scratch_bytes.argtypes = []
     lib.streams_measure_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, _dp]
+    lib.streams_sums_static.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p,
+                                        C.c_void_p, C.c_char_p, C.c_size_t]
     lib.streams_kernel_name.restype = C.c_char_p
     lib.streams_kernel_name.argtypes = [C.c_int]
     lib.streams_last_error.restype = C.c_char_p
@@ -140,6 +143,38 @@ def measure_fp64(kind: int = 0, repeats: int = 5, stream=None) -> float:
     if rc != STREAMS_OK:
         raise StreamsError(rc, lib.streams_last_error(None).decode())
     return out.value
+
+
+def sums_static(f, kind: int = 0, row_weight=None, out=None, stream=None):
+    """streams_sums_static: the sums of streams_get_sums for callers who cannot hand the library device scratch memory
+    (a fixed arena, a hook inside another solver's step; include/streams.h says who and why).  The partial sums go to
+    an array inside the library's device image, the C call allocates nothing.
+
+    f: CUDA float64 tensor [nfields, nz, ny, nx] (at most 16 fields), contiguous; row_weight: CUDA float64 [ny] or None;
+    kind 0: sum of f_q * row_weight[j], kind 1: sum of f_q ** 2.  out: CUDA float64 [nfields], given by the caller (only
+    this Python convenience makes one with torch when it is None).  Enqueued on `stream` (default: torch's current
+    stream) and not synchronised.  Do not let two calls overlap on the GPU: they share the one static array."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: libstreams has no CPU fallback")
+    lib = load_library()
+    assert f.is_cuda and f.dtype == torch.float64 and f.is_contiguous() and f.dim() == 4
+    nf, nz, ny, nx = (int(n) for n in f.shape)
+    if row_weight is not None:
+        assert row_weight.is_cuda and row_weight.dtype == torch.float64 and row_weight.is_contiguous()
+        assert tuple(row_weight.shape) == (ny,) and row_weight.device == f.device
+    if out is None:
+        out = torch.empty(max(nf, 1), dtype=torch.float64, device=f.device)[:nf]
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= nf and out.device == f.device
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(f.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.streams_sums_static(C.c_void_p(f.data_ptr()), nf, nx, ny, nz,
+                                     C.c_void_p(row_weight.data_ptr()) if row_weight is not None else None, int(kind),
+                                     C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream), err, len(err))
+    if rc != STREAMS_OK:
+        raise StreamsError(rc, err.value.decode())
+    return out
 
 
 class StreamsError(RuntimeError):

@@ -23,7 +23,7 @@ LIB = os.path.join(OUT, "libstreams.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", *ARCH]
 UNITS = [("streams_march.cu", []), ("streams_weno.cu", []), ("streams_canon.cu", ["-fmad=false"]), ("streams_fill.cu", []),
-         ("streams_api.cu", [])]
+         ("streams_api.cu", []), ("streams_static.cu", [])]
 
 
 def _newest_source() -> float:

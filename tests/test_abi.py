@@ -75,6 +75,20 @@ def test_fp64_probe_takes_its_scratch_from_the_caller(lib):
     assert lib.streams_measure_fp64(None, 7, 1, None, 0, C.byref(out)) == binding.STREAMS_EINVAL
 
 
+def test_static_scratch_sums_refuse_what_the_static_array_cannot_hold(lib):
+    """streams_sums_static checks its arguments before it touches CUDA: the field limit of its static scratch array and
+    the plain argument errors come back with a message in the caller's buffer, with or without a device."""
+    from paper_2304_05494_b200 import binding
+    err = C.create_string_buffer(256)
+    fake = C.c_void_p(256)
+    rc = lib.streams_sums_static(fake, binding.SUMS_STATIC_MAX_FIELDS + 1, 4, 4, 4, None, 0, fake, None, err, len(err))
+    assert rc == binding.STREAMS_ENOMEM and b"16" in err.value and b"streams_sums_static" in err.value
+    assert lib.streams_sums_static(fake, 0, 4, 4, 4, None, 0, fake, None, err, len(err)) == binding.STREAMS_EINVAL
+    assert lib.streams_sums_static(fake, 5, 4, 0, 4, None, 0, fake, None, err, len(err)) == binding.STREAMS_EINVAL
+    assert lib.streams_sums_static(fake, 5, 4, 4, 4, None, 2, fake, None, err, len(err)) == binding.STREAMS_EINVAL
+    assert lib.streams_sums_static(None, 5, 4, 4, 4, None, 0, fake, None, None, 0) == binding.STREAMS_EINVAL
+
+
 def test_init_without_device_or_workspace_fails_loudly(lib):
     import torch
     from paper_2304_05494_b200 import binding
