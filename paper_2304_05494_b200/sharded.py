@@ -14,6 +14,9 @@ planes between the slabs after each phase and max-reduces the time-step rate.  T
 Only z is cut and z must be periodic in the whole domain (all five BASELINE configs are).  The exchange is synchronous:
 it is enqueued on the slab's stream between two phases (the paper's asynchronous mode gains 1.4-2.5 %; the
 interior-first split that would overlap it is not built).
+
+With torch.distributed every process holds exactly ONE slab and the slab index is the process rank (`exchange` uses it
+as the peer of its sends and receives); several slabs per process exist only without torch.distributed (one GPU).
 """
 from __future__ import annotations
 
@@ -66,6 +69,8 @@ def exchange(slabs, world: int, dist=None):
     field)} for the ranks that live in this process.  A slab's lo_send goes to the hi_recv of the slab below
     (rank - 1, periodic), its hi_send to the lo_recv of the slab above; copies inside the process are direct, the
     others one batch of point-to-point operations."""
+    if dist is not None and world > 1 and len(slabs) != 1:
+        raise ValueError("with torch.distributed a process holds exactly one slab (slab index = process rank)")
     ops = []
     for r, s in slabs.items():
         lo, hi = (r - 1) % world, (r + 1) % world
@@ -99,8 +104,12 @@ class ShardedStreams:
         self.device = torch.device(device)
         cls = solver_cls or binding.Streams
         ng = 4 if max(case.central_order, case.visc_order if case.visc_law else 0, case.weno_order + 1) >= 8 else 3
-        with torch.cuda.device(self.device):
-            self.stream = torch.cuda.Stream(self.device)        # one stream for all local slabs: phases stay ordered
+        if dist is not None and world > 1 and len(list(ranks)) != 1:
+            raise ValueError("with torch.distributed a process holds exactly one slab (slab index = process rank)")
+        self.stream = None                                      # CPU tensors (stub solvers in the gloo tests): no stream
+        if self.device.type == "cuda":
+            with torch.cuda.device(self.device):
+                self.stream = torch.cuda.Stream(self.device)    # one stream for all local slabs: phases stay ordered
         self.slabs = {r: cls(slab_case(case, r, world, ng), device=device, stream=self.stream) for r in ranks}
         self.hybrid = case.flux_mode == 2
         self.visc = case.visc_law != 0
@@ -117,16 +126,30 @@ class ShardedStreams:
             out[r] = v
         return out
 
+    def _on_stream(self):
+        import contextlib
+        return self.torch.cuda.stream(self.stream) if self.stream is not None else contextlib.nullcontext()
+
     def _exchange(self, what):
-        with self.torch.cuda.stream(self.stream):
+        with self._on_stream():
             exchange(self._views(what), self.world, self.dist)
+
+    def halo_bytes_per_stage(self):
+        """Bytes one slab SENDS per RK stage (both neighbours, every exchange of the stage), from the slab sizes the
+        library reports (streams_halo_slabs) and the fields this mode exchanges."""
+        r = next(iter(self.slabs))
+        total = 0
+        for what in [HALO_PRIMS] + ([HALO_DIV] if (self.hybrid or self.visc) else []) + ([HALO_MASK] if self.hybrid else []):
+            v = self._views(what)[r]
+            total += sum(int(t.numel()) * t.element_size() for k in ("lo_send", "hi_send") for t in v[k])
+        return total
 
     def step(self, nsteps: int):
         for _ in range(int(nsteps)):
             for stage in range(3):
                 local_rate = [g.shard_fill(stage) for g in self.slabs.values()]
                 if any(local_rate):
-                    with self.torch.cuda.stream(self.stream):
+                    with self._on_stream():
                         rate_bits_max([g.halo_slabs(HALO_RATE)["lo_send"][0] for g in self.slabs.values()], self.dist)
                 self._exchange(HALO_PRIMS)
                 for g in self.slabs.values():
@@ -137,7 +160,23 @@ class ShardedStreams:
                     self._exchange(HALO_MASK)
                 for g in self.slabs.values():
                     g.shard_rhs(stage)
-        out = [g.shard_finish() for g in self.slabs.values()]
+        out, err = [], None
+        for g in self.slabs.values():
+            try:
+                out.append(g.shard_finish())
+            except RuntimeError as e:                            # e.g. STREAMS_ENAN on this slab only
+                err = e
+        # every rank learns of a failure before anybody raises: a rank that raised alone would leave its peers blocked
+        # in the next exchange
+        d = self.dist
+        if d is not None and d.is_initialized() and d.get_world_size() > 1:
+            flag_dev = self.device if d.get_backend() == "nccl" else "cpu"
+            flag = self.torch.tensor([1 if err is not None else 0], dtype=self.torch.int32, device=flag_dev)
+            d.all_reduce(flag, op=d.ReduceOp.MAX)
+            if err is None and int(flag.item()):
+                err = RuntimeError("the step failed on another rank's slab")
+        if err is not None:
+            raise err
         return out[0]
 
     def get_fields(self):
