@@ -142,12 +142,16 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # fp64 instructions per unit of work: EXECUTED thread-level DFMA + DADD + DMUL (+ DSETP, MUFU.RCP64H) per node /
 # padded node / flagged interface, orders 6/5/6, from the per-instruction execution counts of the ncu source page
-# (profiles/r1c_fp64_counts.md; static SASS counts overstate kernels with branches: the IEEE-divide slow paths and
-# the wall branch of fill_prim are rarely taken)
+# / the executed-instruction counters of profiles/r2_traffic_cfg4.md and profiles/r2_order_sweep.md (static SASS counts
+# overstate kernels with branches: the IEEE-divide slow paths and the wall branch of fill_prim are rarely taken)
 FP64_INST = {"rhs_main_cv": 463, "rhs_main_c": 200, "rhs_main_v": 265, "rhs_main_0": 15, "rhs_corr": 5, "corr_gather": 30,
              "weno_hybrid": 868, "weno_dense": 778, "fill_prim": 120, "fill_prim_dt": 50, "sensor": 97,
              "prims": 60}      # prims: cons -> prim of the updated node in the fused RHS epilogue (shared reciprocal, no IEEE divide)
 FP64_LANES_PER_SM, N_SM = 64, 148       # B200: 64 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz), 148 SMs
+
+
+def case_is_hybrid(case):
+    return case.flux_mode == 2
 
 
 def work_model(case, act):
@@ -318,17 +322,6 @@ def run_ours(args):
         gpu.set_mask_override(imposed)
     state_bytes = 5 * N * 8
 
-    if args.ignore_nan:                         # measurement builds (STREAMS_LIB=...) do not produce the solution
-        _step = gpu.step
-
-        def step_anyway(n):
-            try:
-                return _step(n)
-            except binding.StreamsError as e:
-                if e.code != binding.STREAMS_ENAN:
-                    raise
-                return float("nan"), float("nan")
-        gpu.step = step_anyway
 
     rep = replicas.Replicas(dist, dev)          # barrier + max over ranks (tests/test_replicas_gloo.py)
     max_over_ranks = rep.max_over_ranks
@@ -402,7 +395,7 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
     e2e_value = world * N * n_e2e / (e2e_ms * 1e-3)
-    assert args.ignore_nan or np.isfinite(h_a.numpy()).all()
+    assert np.isfinite(h_a.numpy()).all()
 
     if rank != 0:
         gpu.destroy()
@@ -459,8 +452,16 @@ def run_ours(args):
             tr = json.load(f)
         key = f"cfg{args.config}:{dom}"
         if key in tr:
-            roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
+            # the capture is a separate run under ncu: say at which activation (flagged interfaces per node) and step
+            # counts it was taken, and do not quote its bytes beside a timed region that sat elsewhere (the traffic of
+            # every kernel but the sensor grows with the activation)
+            cap_act, here = tr[key].get("iface_per_node"), act["iface"]
+            comparable = (not case_is_hybrid(case)) or (cap_act is not None and abs(cap_act - here) <= 0.2 * max(here, 1e-12))
+            roofline["traffic"] = tr[key]["dram_bytes_per_launch"] if comparable else None
             roofline["traffic_source"] = tr[key].get("source")
+            roofline["traffic_capture"] = {"iface_per_node": cap_act, "command": tr[key].get("command"),
+                                           "iface_per_node_timed_region": here, "comparable": comparable,
+                                           "dram_bytes_per_launch": tr[key]["dram_bytes_per_launch"]}
 
     # ---- the oracle on this box's host cores (bounded sample, rank 0, N = 1 only)
     cpu = None
@@ -561,12 +562,12 @@ def run_sharded(args):
     clk = clocks.stop() if clocks else None
     ms = float(np.median(reps))
     launches = sh.kernel_launches()
+    halo_bytes = sh.halo_bytes_per_stage()          # from the slab sizes streams_halo_slabs reports (any ghost width)
     w = sh.get_fields()
     ok = bool(np.isfinite(w).all())
     sh.destroy()
     if rank == 0:
         ranges = sharded.slab_ranges(case.nz, nslabs)
-        halo_bytes = 2 * 3 * 3 * (case.nx + 32) * (case.ny + 6) * 8 * (9 + 1) + 2 * 3 * 3 * (case.nx + 32) * (case.ny + 6)
         line = {
             "metric": METRIC, "value": N * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps,
@@ -575,7 +576,7 @@ def run_sharded(args):
             "config": {"workload": WORKLOAD_TEXT[args.config], "grid": [case.nx, case.ny, case.nz], "points": N,
                        "parallelism": (f"{nslabs} z slabs, one per GPU, halo exchange by NCCL send / receive" if world > 1 else
                                        f"{nslabs} z slabs in one process on one GPU (exchange = device copies)"),
-                       "slab_planes": [b - a for a, b in ranges], "halo_bytes_per_slab_per_stage_approx": halo_bytes,
+                       "slab_planes": [b - a for a, b in ranges], "halo_bytes_sent_per_slab_per_stage": halo_bytes,
                        "l2": "inputs larger than L2" if N * 400 > 4 * 126e6 else "L2-resident"},
             "clocks": clk, "gpu_launches": launches, "state_finite": ok, "roofline": None, "cpu_baseline": None,
             "e2e": None,
@@ -598,8 +599,6 @@ def main():
     ap.add_argument("--repeats", type=int, default=5, help="timed regions from the same state; value = median")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--ignore-nan", action="store_true",
-                    help="keep timing when the state goes non-finite (measurement builds selected with STREAMS_LIB)")
     ap.add_argument("--order-family", type=int, default=3, choices=[1, 2, 3, 4],
                     help="m: central order 2m / WENO order 2m-1 / viscous order 2m (default 3 = 6/5/6)")
     ap.add_argument("--flux-mode", default=None, choices=["central", "weno", "hybrid"], help="override the config's flux mode")
@@ -611,7 +610,7 @@ def main():
                     help="hybrid mode: impose the node mask on this fraction of the z planes (PAPER:497-501 sweep)")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = {0: 10, 1: 50, 2: 50, 3: 20, 4: 10, 5: 20}[args.config] if args.impl == "ours" else 3
+        args.steps = {0: 10, 1: 50, 2: 50, 3: 20, 4: 10, 5: 20}.get(args.config, 20) if args.impl == "ours" else 3
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":
