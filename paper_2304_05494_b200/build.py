@@ -3,8 +3,8 @@
     python -m paper_2304_05494_b200.build [--force] [--verbose] [--define NAME[=VALUE] ...] [--tag TAG]
 
 --define adds -DNAME[=VALUE] to every translation unit and --tag TAG writes the result to lib_TAG/libstreams.so instead
-of lib/ (measurement builds, e.g. --define STREAMS_MARCH_SKELETON --tag skeleton: the data movement of the fused RHS
-kernel without its stencil arithmetic; select it at run time with STREAMS_LIB=<path>).
+of lib/ (builds with another tuning constant, e.g. --define STREAMS_MARCH_NSLOT=3 --tag nslot3; select one at run time
+with STREAMS_LIB=<path>).
 
 streams_canon.cu is compiled with -fmad=false (canonical, contraction-free evaluation of the
 sensor path); the other translation units use the default FMA contraction.

@@ -571,16 +571,18 @@ static int run_one_step(streams_ctx* ctx) {
       const int rc = enqueue_step(ctx, want_dt, want_rate);
       cudaGraph_t graph = nullptr;
       const cudaError_t ee = cudaStreamEndCapture(ctx->stream, &graph);
+      // nothing ran during the capture, whether it succeeded or not: rewind the host state it advanced (the replay
+      // below advances it again; on an error return the context still describes the state on the device)
+      const int captured = (int)(ctx->launches - l0);
+      ctx->launches = l0;
+      use_qbuf(ctx, cur0);
+      ctx->rate_ready = rr0;
       if (rc < 0) { if (graph) cudaGraphDestroy(graph); return launch_fail(ctx, rc); }
       if (ee != cudaSuccess) return cuda_fail(ctx, ee, "cudaStreamEndCapture");
       const cudaError_t ei = cudaGraphInstantiate(&ctx->step_graph[key], graph, 0);
       cudaGraphDestroy(graph);
       if (ei != cudaSuccess) { ctx->step_graph[key] = nullptr; return cuda_fail(ctx, ei, "cudaGraphInstantiate"); }
-      ctx->step_graph_launches[key] = (int)(ctx->launches - l0);
-      // nothing ran during the capture: rewind the host state it advanced, the replay below advances it again
-      ctx->launches = l0;
-      use_qbuf(ctx, cur0);
-      ctx->rate_ready = rr0;
+      ctx->step_graph_launches[key] = captured;
     }
     CU(cudaGraphLaunch(ctx->step_graph[key], ctx->stream));
     ctx->graph_launches += 1;

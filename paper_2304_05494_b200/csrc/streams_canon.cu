@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(256) scalar_ghost_kernel(const DevP P) {
 
 // ---------------------------------------------------------------------------------------------
 // sensor_march_kernel: the same sensor (identical operations in identical order, so identical bits) as a
-// z-marching kernel like rhs_march_kernel (streams_rhs.cu): a block owns a 32 x TY tile and a chunk of z
+// z-marching kernel like rhs_march_kernel (streams_march.cu): a block owns a 32 x TY tile and a chunk of z
 // planes; the centre plane of (u, v, w) with its halo is one 4-D TMA box per plane (two buffers, issued two
 // planes ahead), the z neighbours live in a 7-plane register ring fed by a second TMA box per plane.
 // HBM: 24 B read + 8 B (div) + 1 B (mask) write per node; every stencil offset is an immediate.
@@ -239,7 +239,7 @@ sensor_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_
             if (j == 0 && P.bc_y_lo != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(-m * P.sy); }
             if (j == P.ny - 1 && P.bc_y_hi != BC_PERIODIC) { for (int m = 1; m <= NG; ++m) put(m * P.sy); }
           }
-          face(kk, P.nz, per_z, P.sz);
+          if (P.bc_z != BC_HALO) face(kk, P.nz, per_z, P.sz);     // halo planes belong to the caller's exchange (streams.h)
         }
       }
     }

@@ -2,7 +2,7 @@
 //   fill_prim_kernel  : the whole padded box, first evaluation after streams_set_fields (optionally with the
 //                       time-step rate of every interior node, a9)
 //   fill_ghost_kernel : the ghost shell of the non-periodic directions, every other stage
-// Built with the default FMA contraction like streams_rhs.cu, whose epilogue writes the same primitives through the same
+// Built with the default FMA contraction like streams_march.cu, whose epilogue writes the same primitives through the same
 // prims_from_state (streams_dev.cuh): both translation units then compile its library calls (pow of the power-law
 // viscosity) identically and a state gets the same primitive bits whichever kernel produced them.  The arithmetic that
 // reaches the sensor mask (ghost velocities: wall image, u = rho u / rho) is written with explicit single-rounded

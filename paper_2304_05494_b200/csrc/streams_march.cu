@@ -184,11 +184,9 @@ struct MarchSmem {
   static_assert(TOTAL <= 227 * 1024, "shared memory of one block");
 };
 
-#ifndef STREAMS_MARCH_MINB
-#define STREAMS_MARCH_MINB 1
-#endif
+constexpr int MARCH_MINB = 1;                        // one block of 8 warps per SM (253 registers per thread)
 template <int L, int LV, bool VISC, bool CONV, bool WENO, bool UPD, int TY, int NG>
-__global__ void __launch_bounds__(MTX * TY, STREAMS_MARCH_MINB)
+__global__ void __launch_bounds__(MTX * TY, MARCH_MINB)
 rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_constant__ CUtensorMap tm_ring,
                  const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_r,
                  const __grid_constant__ CUtensorMap tm_flag, const DevP P,
@@ -252,11 +250,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   // The streams that miss L2 (the new ring plane and the RK operands) are needed one plane after they are
   // issued, which keeps too few bytes in flight to cover the DRAM latency: PF planes further ahead the same
   // boxes are requested into L2 only.
-#ifdef STREAMS_MARCH_PF_ALL
-  constexpr int PF = STREAMS_MARCH_PF;
-#else
   constexpr int PF = (VISC || WENO) ? 0 : STREAMS_MARCH_PF;   // measured: helps the lean variant only
-#endif
   auto prefetch_ring_epi = [&](int k) {                // thread 0 only
     if (PF > 0 && k < ke) {
       tma_prefetch_4d(&tm_ring, cx0, cy0, k + NG + 1 + NG, 0);
@@ -315,10 +309,7 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   // finiteness check of the last stage.  DEFER: evaluated one plane late, inside the stencil phase of the next plane,
   // so that its long dependent chain (reciprocal, square roots, Newton steps) overlaps the wide stencil arithmetic
   // instead of running alone between two barriers.
-#ifndef STREAMS_MARCH_DEFER
-#define STREAMS_MARCH_DEFER 1
-#endif
-  constexpr bool DEFER = STREAMS_MARCH_DEFER != 0;
+  constexpr bool DEFER = true;
   double wn[5] = {1.0, 0.0, 0.0, 0.0, 1.0};
   // (no branch around the arithmetic: `ok` only predicates the stores, so the chain sits in the stencil phase's block)
   auto finish_node = [&](int kk, bool ok) {
@@ -372,7 +363,6 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
     for (int l = 0; l < 4; ++l) alr[l] = P.kc[l] * c0[F_RHO];
     double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     Visc V;
-#ifndef STREAMS_MARCH_SKELETON
     if (VISC) {
       double gT[3], lapT = 0.0;
       scalar_terms<0, LV>(P, gx, ym, gT, lapT, V);
@@ -386,15 +376,10 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
       V.vm[0] = V.vm[1] = V.vm[2] = 0.0;
       V.dv = 0.0; V.ph = 0.0;
     }
-#endif
-#ifdef STREAMS_MARCH_SKELETON   // measurement build: the kernel's data movement without its stencil arithmetic
-    r[0] = gx(0, 1) + gy(1, -1); r[1] = gz(2, 1) + c0[3]; r[2] = gx(4, -2); r[3] = gy(5, 2); r[4] = gz(VISC ? 8 : 0, -3) + gx(VISC ? 7 : 1, 3) + gy(VISC ? 6 : 2, 3);
-#else
     dir_terms<0, L, LV, CONV, VISC>(P, gx, ym, c0, alr, r, V);
     dir_terms<1, L, LV, CONV, VISC>(P, gy, ym, c0, alr, r, V);
     dir_terms<2, L, LV, CONV, VISC>(P, gz, ym, c0, alr, r, V);
     if (VISC) viscous_close(P, c0, zr[VISC ? F_MU : 0][NG], sb2, r, V);
-#endif
 
     // every warp is done with buf[b] and with the ring / RK-operand slot of the previous plane: the issuing thread
     // refills them
@@ -476,7 +461,7 @@ static int launch_march(const DevP& P, const MarchMaps& mp, const StageArgs& sa,
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::TOTAL) == cudaSuccess ? 0 : -2;
   const int nbx = (P.nx + MTX - 1) / MTX, nby = (P.ny + TY - 1) / TY;
   const int tiles = nbx * nby;
-  const int chunks = pick_chunks(tiles, P.nz, P.nsm * STREAMS_MARCH_MINB);
+  const int chunks = pick_chunks(tiles, P.nz, P.nsm * MARCH_MINB);
   const int kz = (P.nz + chunks - 1) / chunks;
   kern<<<(unsigned)(tiles * chunks), G::NT, SM::TOTAL, st>>>(mp.centre, mp.ring, mp.w, mp.r, mp.flag, P, sa, nbx, nby, kz);
   return 1;
@@ -562,15 +547,10 @@ int march_family(int L, int Lv, int ng) { return ng == 4 ? 4 : (L > Lv ? L : Lv)
 int launch_rhs_main(const DevP& P, const MarchMaps& mp, int L, int Lv, const StageArgs& sa, cudaStream_t st, bool configure) {
   const int m = march_family(P.flux_mode != FLUX_WENO ? L : 1, P.visc_law != VISC_NONE ? Lv : 1, P.ng);
   if (m < 1 || m > 4 || (P.ng != 3 && P.ng != 4)) return -1;
-#ifdef STREAMS_ONLY_FAMILY3                            // development builds: the production family only
-  if (m != 3) return -1;
-  return launch_main_T<3, 3>(P, mp, sa, st, configure);
-#else
   if (m == 1) return launch_main_T<1, 3>(P, mp, sa, st, configure);
   if (m == 2) return launch_main_T<2, 3>(P, mp, sa, st, configure);
   if (m == 3) return launch_main_T<3, 3>(P, mp, sa, st, configure);
   return launch_main_T<4, 4>(P, mp, sa, st, configure);
-#endif
 }
 
 }  // namespace streams

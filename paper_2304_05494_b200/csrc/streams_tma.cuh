@@ -1,5 +1,5 @@
 // TMA / mbarrier / cp.async primitives and the tile geometry shared by the z-marching kernels
-// (rhs_march_kernel in streams_rhs.cu, sensor_march_kernel in streams_canon.cu).  sm_100a only.
+// (rhs_march_kernel in streams_march.cu, sensor_march_kernel in streams_canon.cu).  sm_100a only.
 #pragma once
 #include <cuda.h>
 #include "streams_dev.cuh"

@@ -104,12 +104,11 @@ template <> __device__ __forceinline__ double weno_rec<4, true>(const double* v,
 // Both reconstructions of a characteristic field (upwind and mirrored stencil) as ONE call with the arguments by
 // value, in registers: the five fields of an interface then share one copy of the code instead of ten inlined
 // reconstructions (instruction-cache footprint: the list kernel's straight-line code shrinks by 30 %), while the two
-// reconstructions of a field still interleave.  STREAMS_WENO_REC_INLINE restores the inlined form.
+// reconstructions of a field still interleave.
 template <int R, bool Z>
 __device__ __forceinline__ double weno_rec_pair(const double* gp, const double* gm, double eps) {
   return weno_rec<R, Z>(gp, eps) + weno_rec<R, Z>(gm, eps);
 }
-#ifndef STREAMS_WENO_REC_INLINE
 __device__ __noinline__ double weno_rec5_pair_call(double p0, double p1, double p2, double p3, double p4, double m0, double m1,
                                                   double m2, double m3, double m4, double eps) {
   const double gp[5] = {p0, p1, p2, p3, p4}, gm[5] = {m0, m1, m2, m3, m4};
@@ -119,7 +118,6 @@ template <>
 __device__ __forceinline__ double weno_rec_pair<3, false>(const double* gp, const double* gm, double eps) {
   return weno_rec5_pair_call(gp[0], gp[1], gp[2], gp[3], gp[4], gm[0], gm[1], gm[2], gm[3], gm[4], eps);
 }
-#endif
 
 // ---------------------------------------------------------------------------------------------
 // WENO characteristic flux at interface n+1/2 along D (O3), and the central flux (O1) it replaces.

@@ -270,3 +270,27 @@ def test_restart_through_get_fields_set_fields_is_bit_reproducible(S, visc):
     w_b = b.get_fields()
     assert np.array_equal(w_a, w_b)
     a.destroy(); b.destroy()
+
+
+def test_graph_replay_is_taken_and_changes_nothing(S, monkeypatch):
+    """streams_step replays every step after the first from a CUDA graph (two graphs, one per primitive buffer the step
+    starts from; the first step runs the full ghost + primitive pass and is launched kernel by kernel): the count of
+    graph submissions says so, and STREAMS_NO_GRAPH=1 -- every kernel launched on its own -- gives the same bits and the
+    same number of kernels.  A capture that silently fell back to direct launches would show up as a count of zero."""
+    for dt_every, calls in ((1, (2, 4)), (3, (1, 1, 5))):
+        case = W.isotropic_turbulence(nx=44, ny=40, nz=36, mach_t=0.6, k0=3.0, kmax=8, seed=73, dilatational=0.5).replace(dt_every=dt_every)
+        out = []
+        for no_graph in (False, True):
+            if no_graph:
+                monkeypatch.setenv("STREAMS_NO_GRAPH", "1")
+            else:
+                monkeypatch.delenv("STREAMS_NO_GRAPH", raising=False)
+            gpu = S(case)
+            for n in calls:
+                dt, t = gpu.step(n)
+            out.append((dt, t, gpu.get_fields(), gpu.graph_launches(), gpu.kernel_launches()))
+            gpu.destroy()
+        monkeypatch.delenv("STREAMS_NO_GRAPH", raising=False)
+        assert out[0][3] == sum(calls) - 1 and out[1][3] == 0, (out[0][3], out[1][3])
+        assert out[0][4] == out[1][4]
+        assert out[0][0] == out[1][0] and out[0][1] == out[1][1] and np.array_equal(out[0][2], out[1][2])
