@@ -230,30 +230,18 @@ rhs_march_kernel(const __grid_constant__ CUtensorMap tm_centre, const __grid_con
   const unsigned bytes_e = (unsigned)SM::RING + (UPD ? 4u * G::NT * 8u : 0u) + (sa.read_prev ? 5u * G::NT * 8u : 0u);
   const int cx0 = i0 + P.ox, cy0 = j0 + NG;            // tile origin in padded coordinates
 
-#ifndef STREAMS_MARCH_HINT
-#define STREAMS_MARCH_HINT 0
-#endif
-  // bit 0: the boxes read once per launch (RK operands, flag bytes) are loaded with the evict-first L2 policy, so that
-  // L2 keeps the primitive planes between their ring read and their centre read; bit 2: the centre box too (its second
-  // and last read by this block).  (Stores: STREAMS_ST_CS.)
-  const unsigned long long pol_once = l2_policy_evict_first();
-  auto load_once = [&](void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1, int c2) {
-    if (STREAMS_MARCH_HINT & 1) tma_load_4d_hint(dst, map, bar, c0, c1, c2, 0, pol_once);
-    else tma_load_4d(dst, map, bar, c0, c1, c2, 0);
-  };
   auto issue_centre = [&](int k, int b) {              // thread 0 only
     mbar_expect_tx(&full_c[b], bytes_c);
-    if (STREAMS_MARCH_HINT & 4) tma_load_4d_hint(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0, pol_once);
-    else tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
+    tma_load_4d(buf + (size_t)b * NF * G::PLANE, &tm_centre, &full_c[b], cx0 - 4, cy0 - NG, k + NG, 0);
     // the flag bytes of the plane's nodes ride with it (a byte loaded by its thread one plane ahead stalled every plane:
     // the compiler tests the byte where it is requested and carries the predicate; 11 % of the kernel's samples)
-    if (FLAGS) load_once(flg + b * FLGB, &tm_flag, &full_c[b], cx0, cy0, k + NG);
+    if (FLAGS) tma_load_4d(flg + b * FLGB, &tm_flag, &full_c[b], cx0, cy0, k + NG, 0);
   };
   auto issue_ring_epi = [&](int k, int b) {            // ring plane k+NG+1 and the RK operands of plane k into slot b
     mbar_expect_tx(&full_e[b], bytes_e);
     tma_load_4d(ring + (size_t)b * NF * G::NT, &tm_ring, &full_e[b], cx0, cy0, k + NG + 1 + NG, 0);
-    if (sa.read_prev) load_once(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + NG);
-    if (UPD) load_once(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + NG);
+    if (sa.read_prev) tma_load_4d(epi + (size_t)b * 10 * G::NT, &tm_r, &full_e[b], cx0, cy0, k + NG, 0);
+    if (UPD) tma_load_4d(epi + (size_t)b * 10 * G::NT + 5 * G::NT, &tm_w, &full_e[b], cx0, cy0, k + NG, 0);
   };
 
 #ifndef STREAMS_MARCH_PF

@@ -74,22 +74,6 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, u
       : "memory");
 }
 
-// L2 eviction policy for data read or written once in a launch (the RK operands, the flag bytes, the results): such
-// lines are the first to go, which leaves L2 to the primitive planes a block reads twice (ring box, then centre box)
-__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
-  unsigned long long pol;
-  asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  return pol;
-}
-// tma_load_4d with an L2 eviction policy
-__device__ __forceinline__ void tma_load_4d_hint(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1,
-                                                 int c2, int c3, unsigned long long pol) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;" ::
-          "r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol)
-      : "memory");
-}
-
 // the same box brought into L2 only (no shared-memory destination, no completion tracking)
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
   asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2),
