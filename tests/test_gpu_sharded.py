@@ -85,3 +85,22 @@ def test_snapshot_restore_repeats_the_same_steps(mods):
     w2 = s.get_fields()
     s.destroy()
     assert dt1 == dt2 and np.array_equal(w1, w2)
+
+
+def test_sharded_run_against_the_oracle(mods):
+    """The sharded step compared with the oracle itself, not only through the single-context run: three slabs of a
+    channel with walls (hybrid, viscous, stretched y), six steps with dt recomputed every other step; fields to the step
+    tolerance of the parity tests (1e-9), time step and time to 1e-12."""
+    from oracle.oracle import Oracle
+    from tests.helpers import field_err, natural_scales
+    _, sharded = mods
+    case = W.channel(48, 40, 36, seed=93).replace(dt_every=2)
+    ora = Oracle(case)
+    dt_o, t_o = ora.step(6)
+    w_o = ora.get_fields()
+    ora.close()
+    dt_s, t_s, w_s, _ = _sharded(sharded, case, 3, 6, chunks=(4, 2))
+    assert abs(dt_s - dt_o) <= 1e-12 * dt_o and abs(t_s - t_o) <= 1e-12 * t_o
+    floor_w, _ = natural_scales(case)
+    errs = [field_err(w_s[q], w_o[q], floor_w[q]) for q in range(5)]
+    assert max(errs) <= 1e-9, errs
